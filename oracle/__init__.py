@@ -1,0 +1,213 @@
+"""CPU oracle of the LBM-IMB-DEM hot path -- TEST INFRASTRUCTURE ONLY.
+
+numpy-facing wrappers (argument marshalling only) around
+oracle/lbmimb_oracle.c, the plain fp64 restatement of PAPER.md eq. (1)-(5).
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+`--impl reference` leg may import this package; the product
+(paper_1011_2613_b200) never does, and this package never imports the product.
+
+Array conventions (identical to include/lbmimb.h so that the same seeded inputs
+serve both sides): f[Q][nz][ny][nx] (x fastest), particle arrays [D][P],
+omega [1][P] (2D) / [3][P] (3D), eps_cnt uint8[N], pid int32[N], s[D][N].
+"""
+import ctypes as C
+
+import numpy as np
+
+from .build import build as _build
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build())
+        _lib.orc_beta.restype = C.c_double
+        _lib.orc_beta.argtypes = [C.c_double, C.c_double]
+        _lib.orc_contact_duration.restype = C.c_double
+        _lib.orc_contact_duration.argtypes = [C.c_double] * 4
+        _lib.orc_damping.restype = C.c_double
+        _lib.orc_damping.argtypes = [C.c_double] * 3
+        _lib.orc_map.restype = C.c_int
+        _lib.orc_dem_step.restype = C.c_int
+        _lib.orc_num_threads.restype = C.c_int
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _n3(n):
+    n = list(n) + [1] * (3 - len(n))
+    return np.array(n, dtype=np.int64)
+
+
+def _bc3(bc):
+    bc = list(bc) + [0] * (3 - len(bc))
+    return np.array(bc, dtype=np.int32)
+
+
+def _g3(g):
+    g = list(g) + [0.0] * (3 - len(g))
+    return np.array(g, dtype=np.float64)
+
+
+def nq(dim):
+    return 9 if dim == 2 else 19
+
+
+def num_threads():
+    return int(lib().orc_num_threads())
+
+
+def velocity_set(dim):
+    Q = nq(dim)
+    c = np.zeros((Q, 3), dtype=np.int32)
+    w = np.zeros(Q)
+    o = np.zeros(Q, dtype=np.int32)
+    lib().orc_velocity_set(C.c_int(dim), _p(c), _p(w), _p(o))
+    return c, w, o
+
+
+def feq(dim, rho, u):
+    u = _g3(u)
+    out = np.zeros(nq(dim))
+    lib().orc_feq(C.c_int(dim), C.c_double(rho), _p(u), _p(out))
+    return out
+
+
+def beta(eps, tau):
+    return float(lib().orc_beta(eps, tau))
+
+
+def collide_node(dim, tau, g, f, beta_, vs):
+    """-> (fstar[Q], s[3], rho, u[3]) of one node (eq. (1)-(2) before streaming)."""
+    f = _f64(f)
+    g = _g3(g)
+    vs = _g3(vs)
+    fstar = np.zeros(nq(dim))
+    s = np.zeros(3)
+    rho = C.c_double(0.0)
+    u = np.zeros(3)
+    lib().orc_collide_node(C.c_int(dim), C.c_double(tau), _p(g), _p(f),
+                           C.c_double(beta_), _p(vs), _p(fstar), _p(s),
+                           C.byref(rho), _p(u))
+    return fstar, s, rho.value, u
+
+
+def init(dim, n):
+    n3 = _n3(n)
+    N = int(n3.prod())
+    f = np.empty((nq(dim), int(n3[2]), int(n3[1]), int(n3[0])))
+    lib().orc_init(C.c_int(dim), C.c_int64(N), _p(f))
+    return f
+
+
+def macros(dim, f):
+    """-> rho[nz,ny,nx], u[dim,nz,ny,nx] (bare u, R2)."""
+    f = _f64(f)
+    shp = f.shape[1:]
+    N = int(np.prod(shp))
+    rho = np.empty(shp)
+    u = np.empty((dim,) + shp)
+    lib().orc_macros(C.c_int(dim), C.c_int64(N), _p(f), _p(rho), _p(u))
+    return rho, u
+
+
+def map_particles(dim, n, bc, S, pos, radius):
+    """-> eps_cnt uint8[nz,ny,nx], pid int32[nz,ny,nx]."""
+    n3, bc3 = _n3(n), _bc3(bc)
+    pos = _f64(pos).reshape(dim, -1)
+    radius = _f64(radius)
+    P = pos.shape[1]
+    shp = (int(n3[2]), int(n3[1]), int(n3[0]))
+    eps = np.zeros(shp, dtype=np.uint8)
+    pid = np.empty(shp, dtype=np.int32)
+    rc = lib().orc_map(C.c_int(dim), _p(n3), _p(bc3), C.c_int(S), C.c_int64(P),
+                       _p(pos), _p(radius), _p(eps), _p(pid))
+    if rc != 0:
+        raise RuntimeError("orc_map failed (S^D > 255 or out of memory)")
+    return eps, pid
+
+
+def step(dim, n, bc, tau, g, S, f, eps_cnt=None, pid=None, pos=None, vel=None,
+         omega=None, want_s=False):
+    """One step of eq. (1): returns f(t+1) (and s[dim,nz,ny,nx] if want_s)."""
+    n3, bc3, g3 = _n3(n), _bc3(bc), _g3(g)
+    f = _f64(f)
+    out = np.empty_like(f)
+    shp = f.shape[1:]
+    s = np.zeros((dim,) + shp) if want_s else None
+    if eps_cnt is None:
+        P = 0
+        args = [None] * 5
+    else:
+        pos = _f64(pos).reshape(dim, -1)
+        vel = _f64(vel).reshape(dim, -1)
+        omega = _f64(omega).reshape(1 if dim == 2 else 3, -1)
+        P = pos.shape[1]
+        eps_cnt = np.ascontiguousarray(eps_cnt, dtype=np.uint8)
+        pid = np.ascontiguousarray(pid, dtype=np.int32)
+        args = [_p(eps_cnt), _p(pid), _p(pos), _p(vel), _p(omega)]
+    lib().orc_step(C.c_int(dim), _p(n3), _p(bc3), C.c_double(tau), _p(g3),
+                   C.c_int(S), _p(f), _p(out), args[0], args[1], C.c_int64(P),
+                   args[2], args[3], args[4], _p(s) if want_s else None)
+    return (out, s) if want_s else out
+
+
+def forces(dim, n, bc, s, pid, pos):
+    """Literal eq. (3) with the sign of R6 -> force[dim,P], torque[1|3,P], abs_f[P], abs_t[P]."""
+    n3, bc3 = _n3(n), _bc3(bc)
+    s = _f64(s)
+    pid = np.ascontiguousarray(pid, dtype=np.int32)
+    pos = _f64(pos).reshape(dim, -1)
+    P = pos.shape[1]
+    force = np.zeros((dim, P))
+    torque = np.zeros((1 if dim == 2 else 3, P))
+    abs_f = np.zeros(P)
+    abs_t = np.zeros(P)
+    lib().orc_forces(C.c_int(dim), _p(n3), _p(bc3), _p(s), _p(pid), C.c_int64(P),
+                     _p(pos), _p(force), _p(torque), _p(abs_f), _p(abs_t))
+    return force, torque, abs_f, abs_t
+
+
+def contact_duration(kn, e, mi, mj):
+    return float(lib().orc_contact_duration(kn, e, mi, mj))
+
+
+def damping(kn, e, meff):
+    return float(lib().orc_damping(kn, e, meff))
+
+
+def contact_forces(dim, n, bc, pos, vel, radius, mass, kn, e):
+    n3, bc3 = _n3(n), _bc3(bc)
+    pos = _f64(pos).reshape(dim, -1)
+    vel = _f64(vel).reshape(dim, -1)
+    P = pos.shape[1]
+    fc = np.zeros((dim, P))
+    lib().orc_contact_forces(C.c_int(dim), _p(n3), _p(bc3), C.c_int64(P), _p(pos),
+                             _p(vel), _p(_f64(radius)), _p(_f64(mass)),
+                             C.c_double(kn), C.c_double(e), _p(fc))
+    return fc
+
+
+def dem_step(dim, n, bc, pos, vel, omega, radius, mass, fh, th, kn, e, gp, dt=1.0):
+    """One velocity-Verlet DEM step (R11); returns new (pos, vel, omega) copies."""
+    n3, bc3, gp3 = _n3(n), _bc3(bc), _g3(gp)
+    pos = _f64(pos).reshape(dim, -1).copy()
+    vel = _f64(vel).reshape(dim, -1).copy()
+    omega = _f64(omega).reshape(1 if dim == 2 else 3, -1).copy()
+    P = pos.shape[1]
+    rc = lib().orc_dem_step(C.c_int(dim), _p(n3), _p(bc3), C.c_int64(P), _p(pos),
+                            _p(vel), _p(omega), _p(_f64(radius)), _p(_f64(mass)),
+                            _p(_f64(fh)), _p(_f64(th)), C.c_double(kn),
+                            C.c_double(e), _p(gp3), C.c_double(dt))
+    if rc != 0:
+        raise RuntimeError("orc_dem_step failed")
+    return pos, vel, omega
