@@ -1,0 +1,313 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the LBM-IMB-DEM hot path on B200 (BASELINE.json:metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3|C4|C2|C5] [--impl reference]
+
+One "step" is one pass of the whole hot path over the workload (SURVEY.md 8(a) rows a1-a3, and a4
+where the configuration has moving particles): lbmimb_map_particles -> lbmimb_step(1) ->
+lbmimb_reduce_particle_forces [-> lbmimb_dem_step for C5].  Default workload: C3
+(BASELINE.json:configs[2], D3Q19 fp64 256x1008x256, 24,600 spheres), the configuration the
+north_star target (>= 70 % of HBM bandwidth for the fused D3Q19 step) is quoted on.
+
+`value`   = lattice updates of all ranks / max-over-ranks device time, inputs resident in HBM.
+`e2e`     = the same through the C-ABI with HOST buffers: every step uploads the particle state from
+            pinned host memory (lbmimb_set_particles) and reads force/torque back to the host.
+`roofline`= the fused collide-stream kernel alone: algorithmic bytes (2*Q*8 + 1 + 4 per node) / its
+            launch duration measured with CUDA events on the launching stream inside the timed region.
+`cpu_baseline` = the CPU oracle (tests' reference, never tuned) timed on a bounded sample.
+N > 1: "replicas only": N independent replicas, one per GPU, no data-path collective.
+`--impl reference` times the oracle itself (rank 0 only).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 LBM-IMB MLUPS on 1 B200 and % of HBM roofline (bytes/update counted)"
+UNIT = "MLUPS"
+
+
+def measured_peak_gbs():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples SM clocks and throttle reasons with nvidia-smi DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) >= 7:
+                self.rows.append(parts)
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def get_workload(name):
+    from paper_1011_2613_b200 import inputs
+    return inputs.FULL[name]()
+
+
+def oracle_sample(name, target_s=15.0, max_steps=50):
+    """The oracle as it stands, timed on a bounded sample of the workload: a y-slab of the lattice with
+    the same recipe and solid fraction.  Returns (mlups, cores, description, seconds)."""
+    import oracle as orc
+    from paper_1011_2613_b200 import inputs
+    if name == "C3":
+        w = inputs.c3(n=(256, 48, 256), P=1171, steps=1)
+    elif name == "C4":
+        w = inputs.c4(n=(8192, 512), grid=(540, 34), steps=1)
+    elif name == "C2":
+        w = inputs.c2(n=(1024, 1024), P=3500, steps=1)
+    elif name == "C5":
+        w = inputs.c5(n=(128, 128, 128), P=1024, steps=1)
+    else:
+        raise KeyError(name)
+    f = orc.init(w.dim, w.n)
+    pos, vel, om = w.pos.copy(), w.vel.copy(), w.omega.copy()
+
+    def one_step(f, pos, vel, om):
+        eps, pid = orc.map_particles(w.dim, w.n, w.bc, w.subsamples, pos, w.radius)
+        f, s = orc.step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, eps_cnt=eps, pid=pid, pos=pos, vel=vel,
+                        omega=om, want_s=True)
+        F, T, _, _ = orc.forces(w.dim, w.n, w.bc, s, pid, pos)
+        if w.dem:
+            d = w.dem
+            pos, vel, om = orc.dem_step(w.dim, w.n, w.bc, pos, vel, om, w.radius, w.mass, F, T, d["kn"],
+                                        d["restitution"], d["g_particle"], d["dt"])
+        return f, pos, vel, om
+
+    f, pos, vel, om = one_step(f, pos, vel, om)          # warm-up (page faults, OpenMP pool)
+    t0 = time.perf_counter()
+    steps = 0
+    while steps < max_steps and (steps < 2 or time.perf_counter() - t0 < target_s):
+        f, pos, vel, om = one_step(f, pos, vel, om)
+        steps += 1
+    dt = time.perf_counter() - t0
+    desc = "%s recipe on a %s slab (%d nodes, %d particles), %d whole-path steps" % (
+        name, "x".join(str(v) for v in w.n), w.nodes, w.P, steps)
+    return w.nodes * steps / dt / 1e6, orc.num_threads(), desc, dt
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the same config / metric (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    per_step = max(2.0, 60.0 / max(1, args.steps + args.warmup))
+    vals = []
+    desc = cores = None
+    for it in range(args.warmup + args.steps):
+        v, cores, desc, _ = oracle_sample(args.workload, target_s=min(per_step, 10.0), max_steps=4)
+        if it >= args.warmup:
+            vals.append(v)
+    value = float(np.mean(vals))
+    w = {"C3": (256, 1008, 256), "C4": (8192, 32768), "C2": (1024, 4096), "C5": (128, 512, 128)}[args.workload]
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": None, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "lattice": list(w), "note": "CPU oracle on a bounded sample"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="C3", choices=["C2", "C3", "C4", "C5"])
+    ap.add_argument("--impl", default="lbmimb", choices=["lbmimb", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.warmup < 3:
+        args.warmup = 3
+
+    import torch
+    from paper_1011_2613_b200 import binding as lb, replicas
+    rank, world, local = replicas.init_from_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the lbmimb path has no CPU fallback")
+    torch.cuda.set_device(local)
+    w = get_workload(args.workload)
+    lat = lb.from_workload(w, device=local)
+    dem = w.dem
+    Q = w.Q
+    bytes_per_node = 2 * Q * 8 + 1 + 4
+    N = w.nodes
+
+    def whole_step():
+        lat.map_particles()
+        lat.step(1)
+        lat.reduce_particle_forces(to_host=False)
+        if dem:
+            lat.dem_step(dem["kn"], dem["restitution"], dem["g_particle"], dem["dt"])
+
+    for _ in range(args.warmup):
+        whole_step()
+    lat.synchronize()
+
+    # ---- timed region: device-resident inputs -------------------------------------------------
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    replicas.barrier()
+    torch.cuda.synchronize()
+    launches0 = lat.launch_count()
+    for k in range(args.steps):
+        ev[k][0].record()
+        lat.map_particles()
+        ev[k][1].record()
+        lat.step(1)
+        ev[k][2].record()
+        lat.reduce_particle_forces(to_host=False)
+        ev[k][3].record()
+        if dem:
+            lat.dem_step(dem["kn"], dem["restitution"], dem["g_particle"], dem["dt"])
+        ev[k][4].record()
+    torch.cuda.synchronize()
+    replicas.barrier()
+    launches = lat.launch_count() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = ev[0][0].elapsed_time(ev[-1][4])
+    seg = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(4)] for e in ev])
+    kern_ms = float(seg[:, 1].mean())
+    units, ms_max = replicas.aggregate(float(N) * args.steps, total_ms)
+    value = replicas.mlups(units, ms_max)
+
+    # ---- end to end through host buffers ------------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        P, D, nt = w.P, w.dim, (1 if w.dim == 2 else 3)
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+        hpos, hvel, hom, hrad, hmass = pin(w.pos), pin(w.vel), pin(w.omega), pin(w.radius), pin(w.mass)
+        hF = torch.empty((D, P), dtype=torch.float64).pin_memory().numpy()
+        hT = torch.empty((nt, P), dtype=torch.float64).pin_memory().numpy()
+        h2d = (hpos.nbytes + hvel.nbytes + hom.nbytes + hrad.nbytes + hmass.nbytes)
+        d2h = hF.nbytes + hT.nbytes
+
+        def e2e_step():
+            if dem:
+                p_, v_, o_ = lat.get_particles()          # moving particles: the host owns the state
+                hpos[...], hvel[...], hom[...] = p_, v_, o_
+            lat.set_particles(hpos, hvel, hom, hrad, hmass)
+            lat.map_particles()
+            lat.step(1)
+            lat.reduce_particle_forces(out=(hF, hT))
+            if dem:
+                lat.dem_step(dem["kn"], dem["restitution"], dem["g_particle"], dem["dt"])
+
+        for _ in range(3):
+            e2e_step()
+        replicas.barrier()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(args.steps):
+            e2e_step()
+        b.record()
+        torch.cuda.synchronize()
+        replicas.barrier()
+        e_units, e_ms = replicas.aggregate(float(N) * args.steps, a.elapsed_time(b))
+        if dem:
+            h2d, d2h = h2d, d2h + hpos.nbytes + hvel.nbytes + hom.nbytes
+        e2e = {"value": replicas.mlups(e_units, e_ms), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": e_ms / args.steps}
+
+    lat.synchronize()
+    if rank != 0:
+        lat.close()
+        replicas.shutdown()
+        return 0
+
+    peak, peak_src = measured_peak_gbs()
+    achieved = bytes_per_node * N / (kern_ms * 1e-3) / 1e9
+    roof = {"bound": "hbm", "kernel": "collide_stream_kernel<%d,IMB,EMIT>" % w.dim, "achieved": achieved,
+            "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+            "bytes_per_node": bytes_per_node, "nodes_per_launch": N, "kernel_ms": kern_ms,
+            "kernel_mlups": N / (kern_ms * 1e-3) / 1e6, "frac_of_nominal_8TBs": achieved / 8000.0,
+            "kernel_share_of_step": kern_ms / (total_ms / args.steps)}
+    cpu = None
+    if not args.no_cpu_baseline:
+        v, cores, desc, secs = oracle_sample(args.workload)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": secs}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "lattice": list(w.n), "Q": Q, "particles": w.P, "tau": w.tau,
+                       "bc": list(w.bc), "step": "map_particles + step(1) + reduce_particle_forces" +
+                       (" + dem_step" if dem else ""), "parallelism": "replicas x%d" % world,
+                       "l2": "inputs (%.1f GB of distributions) exceed the 126 MB L2; no flush needed" %
+                       (2 * Q * N * 8 / 1e9)},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
+            "breakdown_ms": {"map_particles": float(seg[:, 0].mean()), "step": kern_ms,
+                             "reduce_particle_forces": float(seg[:, 2].mean()),
+                             "dem_step": float(seg[:, 3].mean()) if dem else 0.0},
+            "version": lb.version()}
+    print(json.dumps(line))
+    lat.close()
+    replicas.shutdown()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

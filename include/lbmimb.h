@@ -1,0 +1,184 @@
+/*
+ * lbmimb.h -- C-ABI of the B200-native LBM-IMB-DEM hot path of arxiv/paper_1011_2613
+ * ("Large-Scale DNS of Gas-Solid Flow on Mole-8.5").  Implemented by
+ * paper_1011_2613_b200/csrc (hand-written CUDA, sm_100a), built into
+ * paper_1011_2613_b200/liblbmimb.so.  No torch / C++ types cross this boundary.
+ *
+ * Citations are PAPER.md:<line> (the paper) and DESIGN.md R<k> (readings of the paper
+ * where it is silent or garbled; R<k> = SURVEY.md 8(c) G<k>).
+ *
+ * ---------------------------------------------------------------------------------------
+ * Conventions
+ * ---------------------------------------------------------------------------------------
+ * Lattice units h = dt = 1.  Node (i,j,k) sits at the integer position (i,j,k); its cell is
+ * the unit square/cube centred on it, so the domain is [-1/2, n-1/2) per axis.
+ * Node index  x = (k*ny + j)*nx + i  (x is the fastest-varying axis); nz = 1 in 2D.
+ * Distributions f[q][k][j][i] (SoA, fp64), Q = 9 (dim 2) or 19 (dim 3).
+ * Direction order (part of the ABI, R1); opposite of odd q is q+1:
+ *   D2Q9 : 0:(0,0) 1:(1,0) 2:(-1,0) 3:(0,1) 4:(0,-1) 5:(1,1) 6:(-1,-1) 7:(1,-1) 8:(-1,1)
+ *   D3Q19: 0 rest; 1..6 = +x,-x,+y,-y,+z,-z; 7:(1,1,0) 8:(-1,-1,0) 9:(1,-1,0) 10:(-1,1,0)
+ *          11:(1,0,1) 12:(-1,0,-1) 13:(1,0,-1) 14:(-1,0,1) 15:(0,1,1) 16:(0,-1,-1)
+ *          17:(0,1,-1) 18:(0,-1,1)
+ *   weights 4/9, 1/9, 1/36 (D2Q9); 1/3, 1/18, 1/36 (D3Q19); c_s^2 = 1/3.
+ * Particle arrays are SoA: pos[D][P], vel[D][P], omega[1][P] (2D, z component) or
+ * omega[3][P] (3D), radius[P], mass[P], force[D][P], torque[1|3][P].
+ *
+ * Pointers: every pointer argument is a HOST pointer owned by the caller unless its name
+ * ends in _dev (then it is a device pointer on the handle's device, e.g. a torch tensor's
+ * data_ptr()).  The library never keeps a caller's host pointer after the call returns.
+ * Device memory is owned by the handle, or by the caller when params.workspace is given.
+ *
+ * Errors: every call returns an lbmimb_status; nothing throws or aborts across the ABI.
+ * On error the handle stays valid and, where possible, unchanged; lbmimb_last_error()
+ * returns a thread-local description of the last failure on the calling thread.
+ *
+ * Ordering: the set_, get_ and fetch_ calls and reduce_particle_forces with non-NULL host outputs are
+ * complete when they return; map_particles, step, dem_step and the _dev variants are
+ * asynchronous on the handle's stream.  One handle must not be used from two threads at
+ * the same time.  There is no CPU fallback: without a CUDA device create_lattice fails.
+ */
+#ifndef LBMIMB_H
+#define LBMIMB_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lbmimb_lattice lbmimb_lattice; /* opaque; owns (or borrows) all device memory */
+
+typedef enum {
+  LBMIMB_OK = 0,
+  LBMIMB_EINVAL = 1, /* bad argument */
+  LBMIMB_ENOMEM = 2, /* device or host allocation failed / workspace too small */
+  LBMIMB_ECUDA = 3,  /* a CUDA runtime call or kernel failed */
+  LBMIMB_ESTATE = 4  /* call out of order (e.g. step with particles set but not mapped) */
+} lbmimb_status;
+
+typedef struct {
+  int32_t dim;        /* 2 -> D2Q9, 3 -> D3Q19 */
+  int32_t subsamples; /* S per axis for the solid-fraction sampling; 1 <= S, S^dim <= 255 */
+  int64_t n[3];       /* nodes per axis, n[2] = 1 in 2D; each >= 1 */
+  int32_t bc[3];      /* per axis: 0 periodic, 1 half-way bounce-back walls at both ends (R15) */
+  int32_t device;     /* CUDA ordinal */
+  double tau;         /* relaxation time of eq. (1), > 0.5 */
+  double g_fluid[3];  /* acceleration g in F_i = 3 w_i rho (c_i . g)  (R3) */
+  void *stream;       /* cudaStream_t to run on (e.g. torch.cuda.current_stream().cuda_stream), NULL = default */
+  void *workspace_dev;      /* optional caller-owned device buffer, 256-byte aligned; NULL = library allocates */
+  uint64_t workspace_bytes; /* size of workspace_dev; must be >= lbmimb_workspace_bytes() */
+} lbmimb_params;
+
+typedef struct {
+  double kn;            /* stiffness k_n of eq. (4) */
+  double restitution;   /* e of eq. (5), 0 < e <= 1 */
+  double g_particle[3]; /* gravitational acceleration on the particles */
+  double dt;            /* DEM time step (1 = one LBM step, R11) */
+} lbmimb_dem_params;
+
+/* selectors of lbmimb_fetch_fields */
+enum {
+  LBMIMB_FIELD_F = 0,       /* double [Q][box]  distributions f_i(x, t) (post-streaming, pre-collision) */
+  LBMIMB_FIELD_RHO = 1,     /* double [box]     rho = sum_i f_i */
+  LBMIMB_FIELD_U = 2,       /* double [D][box]  bare u = sum_i f_i c_i / rho (no half-force shift, R2) */
+  LBMIMB_FIELD_EPS_CNT = 3, /* uint8  [box]     inside-sample count n_s, eps = n_s / S^D */
+  LBMIMB_FIELD_PID = 4,     /* int32  [box]     covering particle, -1 = none */
+  LBMIMB_FIELD_S = 5        /* double [D][box]  exchange vector s of the last step (0 where eps = 0) */
+};
+
+/* Bytes of device memory a lattice of these parameters needs (0 on invalid parameters). */
+uint64_t lbmimb_workspace_bytes(const lbmimb_params *params, int64_t max_particles);
+
+/*
+ * a0. Creates a lattice at rest: f_i = f_i^eq(rho=1, u=0) = w_i on every node, time t = 0, no
+ * particles.  max_particles >= 0 bounds later set_particles calls.  *out receives the handle.
+ * EINVAL: bad dim / n / bc / tau <= 0.5 / S^dim > 255; ENOMEM; ECUDA (no device, ...).
+ */
+lbmimb_status lbmimb_create_lattice(const lbmimb_params *params, int64_t max_particles,
+                                    lbmimb_lattice **out);
+lbmimb_status lbmimb_destroy_lattice(lbmimb_lattice *h); /* NULL is allowed */
+
+/*
+ * Replaces the particle set (P <= max_particles; P = 0 removes all particles).  omega may be
+ * NULL (= 0).  radius > 0, mass > 0.  Centres must lie in [-1/2, n) per axis (the domain is
+ * [-1/2, n-1/2); dem_step wraps periodic coordinates into [0, n)).
+ * Invalidates the particle map: the next step needs map_particles first (else ESTATE).
+ */
+lbmimb_status lbmimb_set_particles(lbmimb_lattice *h, int64_t P, const double *pos, const double *vel,
+                                   const double *omega, const double *radius, const double *mass);
+/* Replaces velocities only (prescribed-velocity runs); keeps the map valid. */
+lbmimb_status lbmimb_set_particle_velocities(lbmimb_lattice *h, const double *vel, const double *omega);
+/* Reads the particle state back; any of the outputs may be NULL. */
+lbmimb_status lbmimb_get_particles(lbmimb_lattice *h, double *pos, double *vel, double *omega);
+int64_t lbmimb_num_particles(const lbmimb_lattice *h);
+
+/*
+ * a1. Particle -> lattice mapping (PAPER.md:46 definition of eps; :71-77 why it is hard; R4, R5).
+ * For every node the number n_s of the S^D sub-cell sample points
+ *   p = x_node + ((a + 1/2)/S - 1/2) per axis, a = 0..S-1,
+ * that lie inside any particle (|p - c|^2 <= R^2, minimum image in periodic axes, evaluated in
+ * fp64 without FMA contraction, left to right), and the covering particle: the one with most
+ * samples in the cell, ties -> lowest index, -1 if none.  Integer results, bit-exact against
+ * the definition.  Uses a cell list over the particles.  Asynchronous.
+ */
+lbmimb_status lbmimb_map_particles(lbmimb_lattice *h);
+
+/*
+ * a2. nsteps fused collide-and-stream steps of eq. (1) with beta,
+ * Omega^S of eq. (2) driven by V_S = v_p + omega_p x (x_node - x_p), the body
+ * force F_i (R3) and periodic / half-way bounce-back streaming.  Advances t by nsteps.
+ * The per-node exchange vectors s = beta sum_i Omega_i c_i are kept for the LAST step only.
+ * ESTATE if particles are set but not mapped.  nsteps = 0 is a no-op.  Asynchronous.
+ */
+lbmimb_status lbmimb_step(lbmimb_lattice *h, int32_t nsteps);
+
+/*
+ * a3. Hydrodynamic force and torque on every particle from the last step's exchange vectors,
+ * eq. (3) with the sign of R6 (force ON the particle):
+ *   F_p = - sum_{n: pid=p} s_n,   T_p = - sum_n (x_n - x_p) x s_n   (minimum image), h^D/dt = 1.
+ * Deterministic (fixed summation order).  force / torque may be NULL: results stay on the
+ * device for dem_step; otherwise they are copied to the host and the call is synchronous.
+ * ESTATE if no step has run since the last map_particles.
+ */
+lbmimb_status lbmimb_reduce_particle_forces(lbmimb_lattice *h, double *force, double *torque);
+
+/*
+ * a4. One soft-sphere DEM step (eq. (4)-(5); R8-R11): linear spring-dashpot
+ * normal contacts found with a cell list, wall contacts on wall axes, velocity-Verlet
+ *   a0 = (F_h + F_c(x,v))/m + g_p; v' = v + dt/2 a0; x' = x + dt v' (wrapped into [0,n) on
+ *   periodic axes); a1 = (F_h + F_c(x',v'))/m + g_p; v'' = v' + dt/2 a1; omega' = omega + dt T_h/I
+ * with F_h, T_h of the last reduce_particle_forces (zero if none ran since set_particles).
+ * Invalidates the particle map.  Asynchronous.
+ */
+lbmimb_status lbmimb_dem_step(lbmimb_lattice *h, const lbmimb_dem_params *dem);
+
+/*
+ * a5. Copies a field of the sub-box [lo, hi) (node coordinates, x first; 2D: lo[2]=0, hi[2]=1)
+ * into dst, laid out [component][k][j][i] over the box, x fastest.  `what` is one of
+ * LBMIMB_FIELD_*.  Synchronous.  EPS_CNT / PID need a valid map, S needs a step after it.
+ */
+lbmimb_status lbmimb_fetch_fields(lbmimb_lattice *h, int32_t what, const int64_t lo[3],
+                                  const int64_t hi[3], void *dst);
+
+/* Replaces all distributions: f[Q][nz][ny][nx] = f_i(x, t) as LBMIMB_FIELD_F returns them. */
+lbmimb_status lbmimb_set_distributions(lbmimb_lattice *h, const double *f);
+
+/* Device-pointer variants (asynchronous on the handle's stream; same layouts). */
+lbmimb_status lbmimb_set_particles_dev(lbmimb_lattice *h, int64_t P, const double *pos_dev,
+                                       const double *vel_dev, const double *omega_dev,
+                                       const double *radius_dev, const double *mass_dev);
+lbmimb_status lbmimb_reduce_particle_forces_dev(lbmimb_lattice *h, double *force_dev, double *torque_dev);
+
+/* Blocks until all work queued on the handle's stream has finished. */
+lbmimb_status lbmimb_synchronize(lbmimb_lattice *h);
+/* Number of steps taken since creation / set_distributions. */
+int64_t lbmimb_time(const lbmimb_lattice *h);
+/* Kernels launched by this handle so far (bench.py's gpu_launches). */
+int64_t lbmimb_launch_count(const lbmimb_lattice *h);
+const char *lbmimb_last_error(void); /* thread-local, never NULL */
+const char *lbmimb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBMIMB_H */

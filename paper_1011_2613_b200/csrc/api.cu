@@ -1,0 +1,529 @@
+// C-ABI entry points of liblbmimb.so (include/lbmimb.h): argument checks, device
+// memory layout, state machine.  All arithmetic of the method runs in the kernels
+// of lattice.cu / particles.cu; nothing here computes on the host.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "lbmimb_internal.cuh"
+
+namespace lbmimb {
+
+static thread_local char g_err[512] = "";
+
+lbmimb_status fail(lbmimb_status st, const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return st;
+}
+
+lbmimb_status cuda_fail(cudaError_t e, const char *what) {
+  snprintf(g_err, sizeof(g_err), "CUDA error %d (%s) in %s", (int)e, cudaGetErrorString(e), what);
+  return e == cudaErrorMemoryAllocation ? LBMIMB_ENOMEM : LBMIMB_ECUDA;
+}
+
+static uint64_t align_up(uint64_t v) { return (v + 255) & ~(uint64_t)255; }
+
+static bool valid_params(const lbmimb_params *p, int64_t maxp) {
+  if (!p) return fail(LBMIMB_EINVAL, "params is NULL"), false;
+  if (p->dim != 2 && p->dim != 3) return fail(LBMIMB_EINVAL, "dim must be 2 or 3"), false;
+  for (int a = 0; a < 3; ++a) {
+    if (p->n[a] < 1 || p->n[a] > 0x7fffffff) return fail(LBMIMB_EINVAL, "n[%d] out of range", a), false;
+    if (p->bc[a] != 0 && p->bc[a] != 1) return fail(LBMIMB_EINVAL, "bc[%d] must be 0 or 1", a), false;
+  }
+  if (p->dim == 2 && p->n[2] != 1) return fail(LBMIMB_EINVAL, "n[2] must be 1 in 2D"), false;
+  if (!(p->tau > 0.5) || !std::isfinite(p->tau)) return fail(LBMIMB_EINVAL, "tau must be > 0.5"), false;
+  for (int a = 0; a < 3; ++a)
+    if (!std::isfinite(p->g_fluid[a])) return fail(LBMIMB_EINVAL, "g_fluid not finite"), false;
+  int64_t sd = 1;
+  if (p->subsamples < 1) return fail(LBMIMB_EINVAL, "subsamples must be >= 1"), false;
+  for (int a = 0; a < p->dim; ++a) sd *= p->subsamples;
+  if (sd > 255) return fail(LBMIMB_EINVAL, "subsamples^dim must be <= 255"), false;
+  if (maxp < 0 || maxp > 0x7fffffff) return fail(LBMIMB_EINVAL, "max_particles out of range"), false;
+  double nn = (double)p->n[0] * (double)p->n[1] * (double)p->n[2];
+  if (nn > 4.0e12) return fail(LBMIMB_EINVAL, "lattice too large"), false;
+  return true;
+}
+
+// One place that decides the device memory layout; used for sizing and for carving.
+struct Layout {
+  uint64_t off_f[2], off_eps, off_pid, off_s, off_beta, off_contested, off_counters;
+  uint64_t off_pos, off_vel, off_omega, off_radius, off_mass, off_force, off_torque, off_fc, off_prec;
+  uint64_t off_count, off_start, off_fill, off_items, off_cell_of, off_bsums;
+  uint64_t total;
+  int64_t N, contested_cap, ncells_max;
+};
+
+static Layout make_layout(const lbmimb_params *p, int64_t maxp) {
+  Layout L;
+  memset(&L, 0, sizeof(L));
+  int Q = p->dim == 2 ? 9 : 19;
+  L.N = p->n[0] * p->n[1] * p->n[2];
+  int64_t pm = maxp > 0 ? maxp : 1;
+  L.contested_cap = L.N / 4 + 65536;
+  L.ncells_max = 1;
+  for (int a = 0; a < p->dim; ++a) L.ncells_max *= (p->n[a] / 2 > 0 ? p->n[a] / 2 : 1);
+  uint64_t o = 0;
+  auto take = [&](uint64_t bytes) {
+    uint64_t r = o;
+    o = align_up(o + bytes);
+    return r;
+  };
+  L.off_f[0] = take((uint64_t)Q * L.N * 8);
+  L.off_f[1] = take((uint64_t)Q * L.N * 8);
+  L.off_eps = take((uint64_t)L.N);
+  L.off_pid = take((uint64_t)L.N * 4);
+  L.off_s = take((uint64_t)p->dim * L.N * 8);
+  L.off_beta = take(256 * 8);
+  L.off_contested = take((uint64_t)L.contested_cap * 8);
+  L.off_counters = take(64);
+  L.off_pos = take((uint64_t)3 * pm * 8);
+  L.off_vel = take((uint64_t)3 * pm * 8);
+  L.off_omega = take((uint64_t)3 * pm * 8);
+  L.off_radius = take((uint64_t)pm * 8);
+  L.off_mass = take((uint64_t)pm * 8);
+  L.off_force = take((uint64_t)3 * pm * 8);
+  L.off_torque = take((uint64_t)3 * pm * 8);
+  L.off_fc = take((uint64_t)3 * pm * 8);
+  L.off_prec = take((uint64_t)10 * pm * 8);
+  L.off_count = take((uint64_t)(L.ncells_max + 1) * 4);
+  L.off_start = take((uint64_t)(L.ncells_max + 1) * 4);
+  L.off_fill = take((uint64_t)(L.ncells_max + 1) * 4);
+  L.off_items = take((uint64_t)pm * 4);
+  L.off_cell_of = take((uint64_t)pm * 4);
+  L.off_bsums = take((uint64_t)((L.ncells_max + 1) / 1024 + 2) * 4);
+  L.total = o;
+  return L;
+}
+
+static lbmimb_status copy_in(lbmimb_lattice *h, void *dst, const void *src, uint64_t bytes) {
+  LBMIMB_CUDA(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, h->stream));
+  return LBMIMB_OK;
+}
+
+static lbmimb_status use_device(const lbmimb_lattice *h) {
+  LBMIMB_CUDA(cudaSetDevice(h->prm.device));
+  return LBMIMB_OK;
+}
+
+// Host-side refresh of the beta table: beta(n_s/S^D, tau).  Plain IEEE
+// + - * / in the paper's order (it is a parameter table, like tau itself).
+static void fill_beta_table(double tau, int SD, double *tab) {
+  for (int c = 0; c < 256; ++c) {
+    double eps = c <= SD ? (double)c / (double)SD : 1.0;
+    tab[c] = eps * (tau - 0.5) / ((1.0 - eps) + (tau - 0.5));
+  }
+}
+
+}  // namespace lbmimb
+
+using namespace lbmimb;
+
+extern "C" {
+
+const char *lbmimb_last_error(void) { return g_err; }
+const char *lbmimb_version(void) { return "lbmimb 0.1 (sm_100a, pull AB fused collide-stream)"; }
+
+uint64_t lbmimb_workspace_bytes(const lbmimb_params *params, int64_t max_particles) {
+  if (!valid_params(params, max_particles)) return 0;
+  return make_layout(params, max_particles).total;
+}
+
+lbmimb_status lbmimb_create_lattice(const lbmimb_params *params, int64_t max_particles, lbmimb_lattice **out) {
+  if (!out) return fail(LBMIMB_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!valid_params(params, max_particles)) return LBMIMB_EINVAL;
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0)
+    return fail(LBMIMB_ECUDA, "no CUDA device available (%s); this library has no CPU fallback",
+                cudaGetErrorString(e));
+  if (params->device < 0 || params->device >= ndev) return fail(LBMIMB_EINVAL, "device ordinal out of range");
+  LBMIMB_CUDA(cudaSetDevice(params->device));
+
+  lbmimb_lattice *h = new (std::nothrow) lbmimb_lattice;
+  if (!h) return fail(LBMIMB_ENOMEM, "host allocation failed");
+  memset(h, 0, sizeof(*h));
+  h->prm = *params;
+  h->g.dim = params->dim;
+  h->g.nx = (int)params->n[0];
+  h->g.ny = (int)params->n[1];
+  h->g.nz = (int)params->n[2];
+  h->g.bcx = params->bc[0];
+  h->g.bcy = params->bc[1];
+  h->g.bcz = params->dim == 3 ? params->bc[2] : 0;
+  h->g.N = params->n[0] * params->n[1] * params->n[2];
+  h->Q = params->dim == 2 ? 9 : 19;
+  h->SD = 1;
+  for (int a = 0; a < params->dim; ++a) h->SD *= params->subsamples;
+  h->stream = (cudaStream_t)params->stream;
+  h->Pmax = max_particles;
+
+  Layout L = make_layout(params, max_particles);
+  if (params->workspace_dev) {
+    if (params->workspace_bytes < L.total || ((uintptr_t)params->workspace_dev & 255)) {
+      delete h;
+      return fail(LBMIMB_ENOMEM, "workspace too small (%llu < %llu bytes) or not 256-byte aligned",
+                  (unsigned long long)params->workspace_bytes, (unsigned long long)L.total);
+    }
+    h->ws = (char *)params->workspace_dev;
+    h->owns_ws = false;
+  } else {
+    void *p = nullptr;
+    e = cudaMalloc(&p, L.total);
+    if (e != cudaSuccess) {
+      delete h;
+      return cuda_fail(e, "cudaMalloc(workspace)");
+    }
+    h->ws = (char *)p;
+    h->owns_ws = true;
+  }
+  h->ws_bytes = L.total;
+  h->f[0] = (double *)(h->ws + L.off_f[0]);
+  h->f[1] = (double *)(h->ws + L.off_f[1]);
+  h->eps_cnt = (uint8_t *)(h->ws + L.off_eps);
+  h->pid = (int32_t *)(h->ws + L.off_pid);
+  h->s = (double *)(h->ws + L.off_s);
+  h->beta_tab = (double *)(h->ws + L.off_beta);
+  h->contested = (int64_t *)(h->ws + L.off_contested);
+  h->contested_cap = L.contested_cap;
+  h->counters = (int32_t *)(h->ws + L.off_counters);
+  h->pos = (double *)(h->ws + L.off_pos);
+  h->vel = (double *)(h->ws + L.off_vel);
+  h->omega = (double *)(h->ws + L.off_omega);
+  h->radius = (double *)(h->ws + L.off_radius);
+  h->mass = (double *)(h->ws + L.off_mass);
+  h->force = (double *)(h->ws + L.off_force);
+  h->torque = (double *)(h->ws + L.off_torque);
+  h->fc = (double *)(h->ws + L.off_fc);
+  h->prec = (double *)(h->ws + L.off_prec);
+  h->cl.count = (int32_t *)(h->ws + L.off_count);
+  h->cl.start = (int32_t *)(h->ws + L.off_start);
+  h->cl.fill = (int32_t *)(h->ws + L.off_fill);
+  h->cl.items = (int32_t *)(h->ws + L.off_items);
+  h->cl.cell_of = (int32_t *)(h->ws + L.off_cell_of);
+  h->cl.block_sums = (int32_t *)(h->ws + L.off_bsums);
+  h->cl.ncells_max = L.ncells_max;
+
+  lbmimb_status st = LBMIMB_OK;
+  double tab[256];
+  fill_beta_table(params->tau, h->SD, tab);
+  auto body = [&]() -> lbmimb_status {
+    LBMIMB_CUDA(cudaMemcpyAsync(h->beta_tab, tab, sizeof(tab), cudaMemcpyHostToDevice, h->stream));
+    LBMIMB_CUDA(cudaMemsetAsync(h->eps_cnt, 0, (size_t)h->g.N, h->stream));
+    LBMIMB_CUDA(cudaMemsetAsync(h->pid, 0xFF, (size_t)h->g.N * 4, h->stream));
+    LBMIMB_CUDA(cudaMemsetAsync(h->counters, 0, 64, h->stream));
+    LBMIMB_CUDA(cudaMemsetAsync(h->force, 0, (size_t)3 * (h->Pmax > 0 ? h->Pmax : 1) * 8, h->stream));
+    LBMIMB_CUDA(cudaMemsetAsync(h->torque, 0, (size_t)3 * (h->Pmax > 0 ? h->Pmax : 1) * 8, h->stream));
+    lbmimb_status s2 = launch_init_rest(h);
+    if (s2 != LBMIMB_OK) return s2;
+    LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+    return LBMIMB_OK;
+  };
+  st = body();
+  if (st != LBMIMB_OK) {
+    if (h->owns_ws) cudaFree(h->ws);
+    delete h;
+    return st;
+  }
+  h->cur = 0;
+  h->P = 0;
+  h->map_valid = true;  // no particles: the all-zero map is the map
+  h->s_valid = false;
+  h->forces_valid = false;
+  h->t = 0;
+  *out = h;
+  return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_destroy_lattice(lbmimb_lattice *h) {
+  if (!h) return LBMIMB_OK;
+  cudaSetDevice(h->prm.device);
+  cudaStreamSynchronize(h->stream);
+  if (h->owns_ws) cudaFree(h->ws);
+  delete h;
+  return LBMIMB_OK;
+}
+
+static lbmimb_status after_particles_changed(lbmimb_lattice *h, bool positions) {
+  if (positions) {
+    h->map_valid = (h->P == 0);
+    h->cl_valid = false;
+    h->s_valid = false;
+    h->forces_valid = false;
+  }
+  if (h->P > 0) return launch_pack_records(h);
+  return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_set_particles(lbmimb_lattice *h, int64_t P, const double *pos, const double *vel,
+                                   const double *omega, const double *radius, const double *mass) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (P < 0 || P > h->Pmax) return fail(LBMIMB_EINVAL, "P = %lld exceeds max_particles = %lld", (long long)P,
+                                        (long long)h->Pmax);
+  if (P > 0 && (!pos || !vel || !radius || !mass)) return fail(LBMIMB_EINVAL, "NULL particle array");
+  int D = h->g.dim, nt = D == 2 ? 1 : 3;
+  double rmax = 0.0;
+  for (int64_t p = 0; p < P; ++p) {
+    if (!(radius[p] > 0.0) || !(mass[p] > 0.0) || !std::isfinite(radius[p]) || !std::isfinite(mass[p]))
+      return fail(LBMIMB_EINVAL, "particle %lld: radius and mass must be positive and finite", (long long)p);
+    for (int a = 0; a < D; ++a) {
+      double x = pos[(int64_t)a * P + p];
+      if (!(x >= -0.5) || !(x < (double)h->prm.n[a] - 0.5 + 0.5))  // [ -1/2, n ) accepted (DEM wraps into [0,n))
+        return fail(LBMIMB_EINVAL, "particle %lld: centre outside the domain on axis %d", (long long)p, a);
+    }
+    if (radius[p] > rmax) rmax = radius[p];
+  }
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  if (P > 0) {
+    if ((st = copy_in(h, h->pos, pos, (uint64_t)D * P * 8)) != LBMIMB_OK) return st;
+    if ((st = copy_in(h, h->vel, vel, (uint64_t)D * P * 8)) != LBMIMB_OK) return st;
+    if (omega) {
+      if ((st = copy_in(h, h->omega, omega, (uint64_t)nt * P * 8)) != LBMIMB_OK) return st;
+    } else {
+      LBMIMB_CUDA(cudaMemsetAsync(h->omega, 0, (size_t)nt * P * 8, h->stream));
+    }
+    if ((st = copy_in(h, h->radius, radius, (uint64_t)P * 8)) != LBMIMB_OK) return st;
+    if ((st = copy_in(h, h->mass, mass, (uint64_t)P * 8)) != LBMIMB_OK) return st;
+    LBMIMB_CUDA(cudaMemsetAsync(h->force, 0, (size_t)D * P * 8, h->stream));
+    LBMIMB_CUDA(cudaMemsetAsync(h->torque, 0, (size_t)nt * P * 8, h->stream));
+  }
+  h->P = P;
+  h->rmax = rmax;
+  if (P == 0) {
+    LBMIMB_CUDA(cudaMemsetAsync(h->eps_cnt, 0, (size_t)h->g.N, h->stream));
+    LBMIMB_CUDA(cudaMemsetAsync(h->pid, 0xFF, (size_t)h->g.N * 4, h->stream));
+  }
+  st = after_particles_changed(h, true);
+  if (st != LBMIMB_OK) return st;
+  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+  return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_set_particles_dev(lbmimb_lattice *h, int64_t P, const double *pos_dev, const double *vel_dev,
+                                       const double *omega_dev, const double *radius_dev, const double *mass_dev) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (P < 0 || P > h->Pmax) return fail(LBMIMB_EINVAL, "P exceeds max_particles");
+  if (P > 0 && (!pos_dev || !vel_dev || !radius_dev || !mass_dev)) return fail(LBMIMB_EINVAL, "NULL particle array");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  int D = h->g.dim, nt = D == 2 ? 1 : 3;
+  double rmax = 0.0;
+  if (P > 0) {
+    auto d2d = [&](void *dst, const void *src, uint64_t bytes) -> lbmimb_status {
+      LBMIMB_CUDA(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, h->stream));
+      return LBMIMB_OK;
+    };
+    if ((st = d2d(h->pos, pos_dev, (uint64_t)D * P * 8)) != LBMIMB_OK) return st;
+    if ((st = d2d(h->vel, vel_dev, (uint64_t)D * P * 8)) != LBMIMB_OK) return st;
+    if (omega_dev) {
+      if ((st = d2d(h->omega, omega_dev, (uint64_t)nt * P * 8)) != LBMIMB_OK) return st;
+    } else {
+      LBMIMB_CUDA(cudaMemsetAsync(h->omega, 0, (size_t)nt * P * 8, h->stream));
+    }
+    if ((st = d2d(h->radius, radius_dev, (uint64_t)P * 8)) != LBMIMB_OK) return st;
+    if ((st = d2d(h->mass, mass_dev, (uint64_t)P * 8)) != LBMIMB_OK) return st;
+    LBMIMB_CUDA(cudaMemsetAsync(h->force, 0, (size_t)D * P * 8, h->stream));
+    LBMIMB_CUDA(cudaMemsetAsync(h->torque, 0, (size_t)nt * P * 8, h->stream));
+    // the cell-list geometry needs the largest radius on the host: one scalar read-back
+    std::vector<double> r((size_t)P);
+    LBMIMB_CUDA(cudaMemcpyAsync(r.data(), h->radius, (size_t)P * 8, cudaMemcpyDeviceToHost, h->stream));
+    LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+    for (int64_t p = 0; p < P; ++p) {
+      if (!(r[p] > 0.0) || !std::isfinite(r[p])) return fail(LBMIMB_EINVAL, "particle %lld: bad radius", (long long)p);
+      if (r[p] > rmax) rmax = r[p];
+    }
+  }
+  h->P = P;
+  h->rmax = rmax;
+  if (P == 0) {
+    LBMIMB_CUDA(cudaMemsetAsync(h->eps_cnt, 0, (size_t)h->g.N, h->stream));
+    LBMIMB_CUDA(cudaMemsetAsync(h->pid, 0xFF, (size_t)h->g.N * 4, h->stream));
+  }
+  return after_particles_changed(h, true);
+}
+
+lbmimb_status lbmimb_set_particle_velocities(lbmimb_lattice *h, const double *vel, const double *omega) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (h->P == 0) return LBMIMB_OK;
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  int D = h->g.dim, nt = D == 2 ? 1 : 3;
+  if (vel && (st = copy_in(h, h->vel, vel, (uint64_t)D * h->P * 8)) != LBMIMB_OK) return st;
+  if (omega && (st = copy_in(h, h->omega, omega, (uint64_t)nt * h->P * 8)) != LBMIMB_OK) return st;
+  st = after_particles_changed(h, false);
+  if (st != LBMIMB_OK) return st;
+  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+  return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_get_particles(lbmimb_lattice *h, double *pos, double *vel, double *omega) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  int D = h->g.dim, nt = D == 2 ? 1 : 3;
+  if (h->P > 0) {
+    if (pos) LBMIMB_CUDA(cudaMemcpyAsync(pos, h->pos, (size_t)D * h->P * 8, cudaMemcpyDeviceToHost, h->stream));
+    if (vel) LBMIMB_CUDA(cudaMemcpyAsync(vel, h->vel, (size_t)D * h->P * 8, cudaMemcpyDeviceToHost, h->stream));
+    if (omega)
+      LBMIMB_CUDA(cudaMemcpyAsync(omega, h->omega, (size_t)nt * h->P * 8, cudaMemcpyDeviceToHost, h->stream));
+  }
+  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+  return LBMIMB_OK;
+}
+
+int64_t lbmimb_num_particles(const lbmimb_lattice *h) { return h ? h->P : -1; }
+int64_t lbmimb_time(const lbmimb_lattice *h) { return h ? h->t : -1; }
+int64_t lbmimb_launch_count(const lbmimb_lattice *h) { return h ? h->launches : -1; }
+
+lbmimb_status lbmimb_synchronize(lbmimb_lattice *h) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+  int32_t c[4];
+  LBMIMB_CUDA(cudaMemcpy(c, h->counters, sizeof(c), cudaMemcpyDeviceToHost));
+  if (c[1] != 0) return fail(LBMIMB_ESTATE, "particle map: contested-node list overflowed (particles overlap too much)");
+  return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_map_particles(lbmimb_lattice *h) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  if (h->P > 0) {
+    if ((st = launch_map(h)) != LBMIMB_OK) return st;
+  }
+  h->map_valid = true;
+  h->s_valid = false;
+  h->forces_valid = false;
+  return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_step(lbmimb_lattice *h, int32_t nsteps) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (nsteps < 0) return fail(LBMIMB_EINVAL, "nsteps < 0");
+  if (!h->map_valid) return fail(LBMIMB_ESTATE, "particles were set or moved but not mapped: call lbmimb_map_particles first");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  for (int32_t it = 0; it < nsteps; ++it) {
+    bool emit = (h->P > 0) && (it == nsteps - 1);
+    if ((st = launch_collide_stream(h, emit)) != LBMIMB_OK) return st;
+    h->cur ^= 1;
+    h->t += 1;
+    if (emit) h->s_valid = true;
+    h->forces_valid = false;
+  }
+  return LBMIMB_OK;
+}
+
+static lbmimb_status reduce_common(lbmimb_lattice *h) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (h->P > 0 && !h->s_valid)
+    return fail(LBMIMB_ESTATE, "no exchange vectors: call lbmimb_step after lbmimb_map_particles first");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  if (h->P > 0) {
+    if ((st = launch_reduce(h)) != LBMIMB_OK) return st;
+  }
+  h->forces_valid = true;
+  return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_reduce_particle_forces(lbmimb_lattice *h, double *force, double *torque) {
+  lbmimb_status st = reduce_common(h);
+  if (st != LBMIMB_OK) return st;
+  int D = h->g.dim, nt = D == 2 ? 1 : 3;
+  if (h->P > 0 && (force || torque)) {
+    if (force) LBMIMB_CUDA(cudaMemcpyAsync(force, h->force, (size_t)D * h->P * 8, cudaMemcpyDeviceToHost, h->stream));
+    if (torque)
+      LBMIMB_CUDA(cudaMemcpyAsync(torque, h->torque, (size_t)nt * h->P * 8, cudaMemcpyDeviceToHost, h->stream));
+    LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+  }
+  return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_reduce_particle_forces_dev(lbmimb_lattice *h, double *force_dev, double *torque_dev) {
+  lbmimb_status st = reduce_common(h);
+  if (st != LBMIMB_OK) return st;
+  int D = h->g.dim, nt = D == 2 ? 1 : 3;
+  if (h->P > 0) {
+    if (force_dev)
+      LBMIMB_CUDA(cudaMemcpyAsync(force_dev, h->force, (size_t)D * h->P * 8, cudaMemcpyDeviceToDevice, h->stream));
+    if (torque_dev)
+      LBMIMB_CUDA(cudaMemcpyAsync(torque_dev, h->torque, (size_t)nt * h->P * 8, cudaMemcpyDeviceToDevice, h->stream));
+  }
+  return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_dem_step(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (!dem) return fail(LBMIMB_EINVAL, "dem params is NULL");
+  if (!(dem->kn > 0.0) || !(dem->restitution > 0.0) || !(dem->restitution <= 1.0) || !(dem->dt > 0.0))
+    return fail(LBMIMB_EINVAL, "dem params: need kn > 0, 0 < restitution <= 1, dt > 0");
+  if (h->P == 0) return LBMIMB_OK;
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  if ((st = launch_dem(h, dem)) != LBMIMB_OK) return st;
+  // positions moved: the map and the exchange vectors are stale; the cell list was rebuilt at
+  // the new positions inside the step and stays valid; force/torque stay "the last reduction"
+  h->map_valid = false;
+  h->s_valid = false;
+  return launch_pack_records(h);
+}
+
+lbmimb_status lbmimb_fetch_fields(lbmimb_lattice *h, int32_t what, const int64_t lo[3], const int64_t hi[3], void *dst) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (!lo || !hi || !dst) return fail(LBMIMB_EINVAL, "NULL argument");
+  int64_t box = 1;
+  for (int a = 0; a < 3; ++a) {
+    int64_t na = a == 0 ? h->g.nx : (a == 1 ? h->g.ny : h->g.nz);
+    if (lo[a] < 0 || hi[a] > na || lo[a] >= hi[a]) return fail(LBMIMB_EINVAL, "box out of range on axis %d", a);
+    box *= hi[a] - lo[a];
+  }
+  int comps;
+  size_t esz;
+  switch (what) {
+    case LBMIMB_FIELD_F: comps = h->Q; esz = 8; break;
+    case LBMIMB_FIELD_RHO: comps = 1; esz = 8; break;
+    case LBMIMB_FIELD_U: comps = h->g.dim; esz = 8; break;
+    case LBMIMB_FIELD_EPS_CNT: comps = 1; esz = 1; break;
+    case LBMIMB_FIELD_PID: comps = 1; esz = 4; break;
+    case LBMIMB_FIELD_S: comps = h->g.dim; esz = 8; break;
+    default: return fail(LBMIMB_EINVAL, "unknown field selector %d", what);
+  }
+  if ((what == LBMIMB_FIELD_EPS_CNT || what == LBMIMB_FIELD_PID) && !h->map_valid)
+    return fail(LBMIMB_ESTATE, "particle map is stale");
+  if (what == LBMIMB_FIELD_S && h->P > 0 && !h->s_valid) return fail(LBMIMB_ESTATE, "no exchange vectors yet");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  // the idle distribution buffer is the staging area: every field of a sub-box fits in Q*N doubles
+  void *stage = h->f[h->cur ^ 1];
+  if ((st = launch_fetch(h, what, lo, hi, stage)) != LBMIMB_OK) return st;
+  LBMIMB_CUDA(cudaMemcpyAsync(dst, stage, (size_t)comps * box * esz, cudaMemcpyDeviceToHost, h->stream));
+  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+  return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_set_distributions(lbmimb_lattice *h, const double *f) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (!f) return fail(LBMIMB_EINVAL, "f is NULL");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  double *stage = h->f[h->cur ^ 1];
+  LBMIMB_CUDA(cudaMemcpyAsync(stage, f, (size_t)h->Q * h->g.N * 8, cudaMemcpyHostToDevice, h->stream));
+  if ((st = launch_unstream(h, stage, h->f[h->cur])) != LBMIMB_OK) return st;
+  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+  h->t = 0;
+  h->s_valid = false;
+  h->forces_valid = false;
+  return LBMIMB_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,150 @@
+// Internal declarations of the lbmimb CUDA library (sm_100a).  Not part of the ABI.
+// Shares nothing with oracle/ (the tests' CPU oracle): tables, helpers and kernels
+// here are written independently from PAPER.md / DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/lbmimb.h"
+
+namespace lbmimb {
+
+// ---------------------------------------------------------------------------
+// Velocity sets (R1, ABI order of include/lbmimb.h).  constexpr
+// functions so that every use in a fully unrolled loop folds to an immediate.
+// ---------------------------------------------------------------------------
+template <int D>
+struct Lat;
+
+template <>
+struct Lat<2> {
+  static constexpr int Q = 9;
+  __host__ __device__ static constexpr int cx(int q) {
+    constexpr int t[9] = {0, 1, -1, 0, 0, 1, -1, 1, -1};
+    return t[q];
+  }
+  __host__ __device__ static constexpr int cy(int q) {
+    constexpr int t[9] = {0, 0, 0, 1, -1, 1, -1, -1, 1};
+    return t[q];
+  }
+  __host__ __device__ static constexpr int cz(int) { return 0; }
+  __host__ __device__ static constexpr double w(int q) {
+    return q == 0 ? 4.0 / 9.0 : (q < 5 ? 1.0 / 9.0 : 1.0 / 36.0);
+  }
+};
+
+template <>
+struct Lat<3> {
+  static constexpr int Q = 19;
+  __host__ __device__ static constexpr int cx(int q) {
+    constexpr int t[19] = {0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 0, 0, 0, 0};
+    return t[q];
+  }
+  __host__ __device__ static constexpr int cy(int q) {
+    constexpr int t[19] = {0, 0, 0, 1, -1, 0, 0, 1, -1, -1, 1, 0, 0, 0, 0, 1, -1, 1, -1};
+    return t[q];
+  }
+  __host__ __device__ static constexpr int cz(int q) {
+    constexpr int t[19] = {0, 0, 0, 0, 0, 1, -1, 0, 0, 0, 0, 1, -1, -1, 1, 1, -1, -1, 1};
+    return t[q];
+  }
+  __host__ __device__ static constexpr double w(int q) {
+    return q == 0 ? 1.0 / 3.0 : (q < 7 ? 1.0 / 18.0 : 1.0 / 36.0);
+  }
+};
+
+__host__ __device__ constexpr int opposite(int q) { return q == 0 ? 0 : ((q & 1) ? q + 1 : q - 1); }
+
+// Packed per-particle record the fused kernel gathers on covered nodes.
+//   3D: x y z vx vy vz wx wy wz R   (10 doubles)      2D: x y vx vy w R (6 doubles)
+__host__ __device__ constexpr int prec_stride(int dim) { return dim == 3 ? 10 : 6; }
+
+struct Geom {
+  int dim;
+  int nx, ny, nz;   // nodes per axis (each < 2^31)
+  int bcx, bcy, bcz;  // 0 periodic, 1 walls
+  int64_t N;        // nx*ny*nz
+};
+
+// Cell list over the particles (mapping fix-up pass and DEM contacts).
+struct CellList {
+  int ncx, ncy, ncz;     // cells per axis
+  double inv_ex, inv_ey, inv_ez;  // 1 / cell edge
+  int64_t ncells;
+  int32_t *count;   // [ncells_max + 1]
+  int32_t *start;   // [ncells_max + 1] exclusive scan of count
+  int32_t *fill;    // [ncells_max]
+  int32_t *items;   // [Pmax] particle indices, ascending inside a cell
+  int32_t *cell_of; // [Pmax]
+  int32_t *block_sums;  // scan scratch
+  int64_t ncells_max;
+};
+
+}  // namespace lbmimb
+
+struct lbmimb_lattice {
+  lbmimb_params prm;
+  lbmimb::Geom g;
+  int Q;
+  int SD;            // S^dim
+  cudaStream_t stream;
+  bool owns_ws;
+  char *ws;
+  uint64_t ws_bytes;
+
+  // lattice state.  f[cur] holds the POST-COLLISION distributions f*(x, t-1) of the last step
+  // ("pull" representation): f_i(x,t) = f*_i(x - c_i) or, through a wall, f*_{-i}(x).
+  double *f[2];
+  int cur;
+  uint8_t *eps_cnt;   // [N]
+  int32_t *pid;       // [N]
+  double *s;          // [dim][N] exchange vectors of the last step
+  double *beta_tab;   // [256] beta(n_s / S^D, tau)
+  int64_t *contested; // mapping fix-up list
+  int64_t contested_cap;
+  int32_t *counters;  // [0] contested count, [1] overflow flag, [2] bad-particle flag
+
+  // particles (SoA, device)
+  int64_t Pmax, P;
+  double *pos, *vel, *omega, *radius, *mass, *force, *torque, *fc, *prec;
+  double rmax;        // max radius of the current set
+  lbmimb::CellList cl;
+  bool cl_valid;
+
+  bool map_valid;     // eps_cnt/pid match the particle positions
+  bool s_valid;       // s holds the exchange vectors of the last step under the current map
+  bool forces_valid;  // force/torque hold the reduction of s
+  int64_t t;
+  int64_t launches;
+};
+
+namespace lbmimb {
+
+lbmimb_status fail(lbmimb_status st, const char *fmt, ...);
+lbmimb_status cuda_fail(cudaError_t e, const char *what);
+
+#define LBMIMB_CUDA(call)                                            \
+  do {                                                               \
+    cudaError_t e__ = (call);                                        \
+    if (e__ != cudaSuccess) return ::lbmimb::cuda_fail(e__, #call);  \
+  } while (0)
+
+#define LBMIMB_LAUNCH_CHECK(h, name)                                 \
+  do {                                                               \
+    (h)->launches += 1;                                              \
+    cudaError_t e__ = cudaGetLastError();                            \
+    if (e__ != cudaSuccess) return ::lbmimb::cuda_fail(e__, name);   \
+  } while (0)
+
+// kernels.cu entry points used by api.cu
+lbmimb_status launch_init_rest(lbmimb_lattice *h);
+lbmimb_status launch_collide_stream(lbmimb_lattice *h, bool emit);
+lbmimb_status launch_unstream(lbmimb_lattice *h, const double *f_pre, double *f_post);
+lbmimb_status launch_fetch(lbmimb_lattice *h, int what, const int64_t lo[3], const int64_t hi[3], void *dst_dev);
+lbmimb_status launch_pack_records(lbmimb_lattice *h);
+lbmimb_status build_cell_list(lbmimb_lattice *h);
+lbmimb_status launch_map(lbmimb_lattice *h);
+lbmimb_status launch_reduce(lbmimb_lattice *h);
+lbmimb_status launch_dem(lbmimb_lattice *h, const lbmimb_dem_params *dem);
+
+}  // namespace lbmimb

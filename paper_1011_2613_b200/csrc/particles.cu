@@ -1,0 +1,769 @@
+// Particle-side kernels: packed records, cell list (counting sort), the particle ->
+// lattice mapping (a1), the force/torque reduction (a3) and the soft-sphere DEM (a4).
+#include <cmath>
+
+#include "lbmimb_internal.cuh"
+
+namespace lbmimb {
+
+// ---------------------------------------------------------------------------
+// helpers
+// ---------------------------------------------------------------------------
+__device__ __forceinline__ double min_image_d(double d, int n) {
+  const double hn = 0.5 * (double)n;
+  if (d > hn) return d - (double)n;
+  if (d < -hn) return d + (double)n;
+  return d;
+}
+
+__device__ __forceinline__ int wrap_i(int i, int n) {
+  i %= n;
+  return i < 0 ? i + n : i;
+}
+
+// neighbour-cell offsets along one axis: periodic axes must not visit a cell twice
+__device__ __forceinline__ int off_lo(int nc, int periodic) { return periodic ? (nc >= 3 ? -1 : 0) : -1; }
+__device__ __forceinline__ int off_hi(int nc, int periodic) { return periodic ? (nc >= 2 ? 1 : 0) : 1; }
+
+static int blocks_for(int64_t n, int threads) { return (int)((n + threads - 1) / threads > 0 ? (n + threads - 1) / threads : 1); }
+
+// ---------------------------------------------------------------------------
+// packed records for the fused step kernel
+// ---------------------------------------------------------------------------
+__global__ void pack_records_kernel(int dim, int64_t P, const double *__restrict__ pos, const double *__restrict__ vel,
+                                    const double *__restrict__ omega, const double *__restrict__ radius,
+                                    double *__restrict__ prec) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  if (dim == 2) {
+    double *r = prec + p * 6;
+    r[0] = pos[p];
+    r[1] = pos[P + p];
+    r[2] = vel[p];
+    r[3] = vel[P + p];
+    r[4] = omega[p];
+    r[5] = radius[p];
+  } else {
+    double *r = prec + p * 10;
+    r[0] = pos[p];
+    r[1] = pos[P + p];
+    r[2] = pos[2 * P + p];
+    r[3] = vel[p];
+    r[4] = vel[P + p];
+    r[5] = vel[2 * P + p];
+    r[6] = omega[p];
+    r[7] = omega[P + p];
+    r[8] = omega[2 * P + p];
+    r[9] = radius[p];
+  }
+}
+
+lbmimb_status launch_pack_records(lbmimb_lattice *h) {
+  pack_records_kernel<<<blocks_for(h->P, 256), 256, 0, h->stream>>>(h->g.dim, h->P, h->pos, h->vel, h->omega,
+                                                                    h->radius, h->prec);
+  LBMIMB_LAUNCH_CHECK(h, "pack_records_kernel");
+  return LBMIMB_OK;
+}
+
+// ---------------------------------------------------------------------------
+// cell list: counting sort of the particles into cells of edge >= max(2 R_max, R_max + 1, 2)
+// ---------------------------------------------------------------------------
+struct CellGeom {
+  int dim;
+  int nc[3];
+  double inv_e[3];
+  int periodic[3];
+};
+
+__device__ __forceinline__ int cell_coord(double x, const CellGeom &cg, int a) {
+  int c = (int)floor((x + 0.5) * cg.inv_e[a]);
+  if (cg.periodic[a]) {
+    c = wrap_i(c, cg.nc[a]);
+  } else {
+    c = c < 0 ? 0 : (c >= cg.nc[a] ? cg.nc[a] - 1 : c);
+  }
+  return c;
+}
+
+__global__ void cl_count_kernel(CellGeom cg, int64_t P, const double *__restrict__ pos, int32_t *__restrict__ cell_of,
+                                int32_t *__restrict__ count) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  const int cx = cell_coord(pos[p], cg, 0);
+  const int cy = cell_coord(pos[P + p], cg, 1);
+  const int cz = cg.dim == 3 ? cell_coord(pos[2 * P + p], cg, 2) : 0;
+  const int c = (cz * cg.nc[1] + cy) * cg.nc[0] + cx;
+  cell_of[p] = c;
+  atomicAdd(count + c, 1);
+}
+
+constexpr int kScanChunk = 2048;  // elements per block (256 threads x 8)
+
+__global__ void scan_reduce_kernel(const int32_t *__restrict__ in, int64_t n, int32_t *__restrict__ block_sums) {
+  __shared__ int32_t sh[8];
+  const int64_t base = (int64_t)blockIdx.x * kScanChunk;
+  int32_t v = 0;
+  for (int e = threadIdx.x; e < kScanChunk; e += 256) {
+    const int64_t idx = base + e;
+    if (idx < n) v += in[idx];
+  }
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int32_t t = 0;
+    for (int w = 0; w < 8; ++w) t += sh[w];
+    block_sums[blockIdx.x] = t;
+  }
+}
+
+// exclusive scan of the block sums by one block (serial over chunks of 1024 with a carry)
+__global__ void scan_block_sums_kernel(int32_t *__restrict__ block_sums, int nb) {
+  __shared__ int32_t sh[1024];
+  __shared__ int32_t carry;
+  if (threadIdx.x == 0) carry = 0;
+  __syncthreads();
+  for (int base = 0; base < nb; base += 1024) {
+    const int idx = base + threadIdx.x;
+    const int32_t v = idx < nb ? block_sums[idx] : 0;
+    sh[threadIdx.x] = v;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {
+      int32_t t = threadIdx.x >= o ? sh[threadIdx.x - o] : 0;
+      __syncthreads();
+      sh[threadIdx.x] += t;
+      __syncthreads();
+    }
+    const int32_t incl = sh[threadIdx.x];
+    if (idx < nb) block_sums[idx] = carry + incl - v;
+    __syncthreads();
+    if (threadIdx.x == 1023) carry += incl;
+    __syncthreads();
+  }
+}
+
+__global__ void scan_final_kernel(const int32_t *__restrict__ in, int64_t n, const int32_t *__restrict__ block_sums,
+                                  int32_t *__restrict__ out) {
+  // one thread scans 8 consecutive elements; warp/block scan of the per-thread sums
+  __shared__ int32_t wsum[8];
+  const int64_t base = (int64_t)blockIdx.x * kScanChunk + (int64_t)threadIdx.x * 8;
+  int32_t v[8], tot = 0;
+#pragma unroll
+  for (int e = 0; e < 8; ++e) {
+    v[e] = (base + e < n) ? in[base + e] : 0;
+    tot += v[e];
+  }
+  int32_t incl = tot;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int o = 1; o < 32; o <<= 1) {
+    int32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += t;
+  }
+  if (lane == 31) wsum[wid] = incl;
+  __syncthreads();
+  int32_t woff = 0;
+  for (int w = 0; w < wid; ++w) woff += wsum[w];
+  int32_t run = block_sums[blockIdx.x] + woff + incl - tot;
+#pragma unroll
+  for (int e = 0; e < 8; ++e) {
+    if (base + e < n) out[base + e] = run;
+    run += v[e];
+  }
+}
+
+__global__ void cl_fill_kernel(int64_t P, const int32_t *__restrict__ cell_of, const int32_t *__restrict__ start,
+                               int32_t *__restrict__ fill, int32_t *__restrict__ items) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  const int c = cell_of[p];
+  const int slot = atomicAdd(fill + c, 1);
+  items[start[c] + slot] = (int32_t)p;
+}
+
+// ascending particle index inside each cell: makes every later traversal order deterministic
+__global__ void cl_sort_kernel(int64_t ncells, const int32_t *__restrict__ start, int32_t *__restrict__ items) {
+  const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncells) return;
+  const int b = start[c], e = start[c + 1];
+  for (int a = b + 1; a < e; ++a) {
+    const int32_t v = items[a];
+    int q = a - 1;
+    while (q >= b && items[q] > v) {
+      items[q + 1] = items[q];
+      --q;
+    }
+    items[q + 1] = v;
+  }
+}
+
+static CellGeom cell_geom(const lbmimb_lattice *h) {
+  CellGeom cg;
+  cg.dim = h->g.dim;
+  cg.nc[0] = h->cl.ncx;
+  cg.nc[1] = h->cl.ncy;
+  cg.nc[2] = h->cl.ncz;
+  cg.inv_e[0] = h->cl.inv_ex;
+  cg.inv_e[1] = h->cl.inv_ey;
+  cg.inv_e[2] = h->cl.inv_ez;
+  cg.periodic[0] = !h->g.bcx;
+  cg.periodic[1] = !h->g.bcy;
+  cg.periodic[2] = !h->g.bcz;
+  return cg;
+}
+
+lbmimb_status build_cell_list(lbmimb_lattice *h) {
+  double edge = 2.0 * h->rmax;
+  if (edge < h->rmax + 1.0) edge = h->rmax + 1.0;
+  if (edge < 2.0) edge = 2.0;
+  int n[3] = {h->g.nx, h->g.ny, h->g.nz};
+  int nc[3] = {1, 1, 1};
+  double inv_e[3] = {1.0, 1.0, 1.0};
+  for (int a = 0; a < h->g.dim; ++a) {
+    nc[a] = (int)floor((double)n[a] / edge);
+    if (nc[a] < 1) nc[a] = 1;
+    inv_e[a] = (double)nc[a] / (double)n[a];
+  }
+  CellList &cl = h->cl;
+  cl.ncx = nc[0];
+  cl.ncy = nc[1];
+  cl.ncz = nc[2];
+  cl.inv_ex = inv_e[0];
+  cl.inv_ey = inv_e[1];
+  cl.inv_ez = inv_e[2];
+  cl.ncells = (int64_t)nc[0] * nc[1] * nc[2];
+  if (cl.ncells > cl.ncells_max) return fail(LBMIMB_EINVAL, "internal: cell list larger than planned");
+  const int64_t n1 = cl.ncells + 1;
+  LBMIMB_CUDA(cudaMemsetAsync(cl.count, 0, (size_t)n1 * 4, h->stream));
+  LBMIMB_CUDA(cudaMemsetAsync(cl.fill, 0, (size_t)cl.ncells * 4, h->stream));
+  CellGeom cg = cell_geom(h);
+  cl_count_kernel<<<blocks_for(h->P, 256), 256, 0, h->stream>>>(cg, h->P, h->pos, cl.cell_of, cl.count);
+  LBMIMB_LAUNCH_CHECK(h, "cl_count_kernel");
+  const int nb = (int)((n1 + kScanChunk - 1) / kScanChunk);
+  scan_reduce_kernel<<<nb, 256, 0, h->stream>>>(cl.count, n1, cl.block_sums);
+  LBMIMB_LAUNCH_CHECK(h, "scan_reduce_kernel");
+  scan_block_sums_kernel<<<1, 1024, 0, h->stream>>>(cl.block_sums, nb);
+  LBMIMB_LAUNCH_CHECK(h, "scan_block_sums_kernel");
+  scan_final_kernel<<<nb, 256, 0, h->stream>>>(cl.count, n1, cl.block_sums, cl.start);
+  LBMIMB_LAUNCH_CHECK(h, "scan_final_kernel");
+  cl_fill_kernel<<<blocks_for(h->P, 256), 256, 0, h->stream>>>(h->P, cl.cell_of, cl.start, cl.fill, cl.items);
+  LBMIMB_LAUNCH_CHECK(h, "cl_fill_kernel");
+  cl_sort_kernel<<<blocks_for(cl.ncells, 256), 256, 0, h->stream>>>(cl.ncells, cl.start, cl.items);
+  LBMIMB_LAUNCH_CHECK(h, "cl_sort_kernel");
+  h->cl_valid = true;
+  return LBMIMB_OK;
+}
+
+// ---------------------------------------------------------------------------
+// a1: mapping.  The inside test of ONE sample point, rounded exactly like the
+// definition (include/lbmimb.h a1): every operation is a separate IEEE op, no FMA.
+// ---------------------------------------------------------------------------
+struct MapArgs {
+  Geom g;
+  int S, SD;
+  int64_t P;
+  const double *pos;
+  const double *radius;
+  uint8_t *eps_cnt;
+  int32_t *pid;
+  int64_t *contested;
+  int64_t contested_cap;
+  int32_t *counters;
+  double h_in, h_out;  // half extent of the sample cloud -/+ safety margin
+};
+
+__device__ __forceinline__ double sub_offset(int a, int S) {
+  return __dsub_rn(__ddiv_rn(__dadd_rn((double)a, 0.5), (double)S), 0.5);
+}
+
+template <int D>
+__device__ __forceinline__ bool sample_inside(const Geom &g, int i, int j, int k, double sx, double sy, double sz,
+                                              double cx, double cy, double cz, double R2) {
+  double dx = __dsub_rn(__dadd_rn((double)i, sx), cx);
+  double dy = __dsub_rn(__dadd_rn((double)j, sy), cy);
+  if (!g.bcx) dx = min_image_d(dx, g.nx);
+  if (!g.bcy) dy = min_image_d(dy, g.ny);
+  double d2 = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
+  if (D == 3) {
+    double dz = __dsub_rn(__dadd_rn((double)k, sz), cz);
+    if (!g.bcz) dz = min_image_d(dz, g.nz);
+    d2 = __dadd_rn(d2, __dmul_rn(dz, dz));
+  }
+  return d2 <= R2;
+}
+
+// number of inside samples of node (i,j,k) for one particle, computed by one warp
+// (lane l tests samples l, l+32, ...); also returns this lane's inside bits in `bits`.
+template <int D>
+__device__ __forceinline__ int warp_count_samples(const Geom &g, int S, int SD, const double *sub, int i, int j, int k,
+                                                  double cx, double cy, double cz, double R2, unsigned &bits) {
+  const int lane = threadIdx.x & 31;
+  int cnt = 0;
+  bits = 0;
+  for (int m = 0, b = lane; m * 32 < SD; ++m, b += 32) {
+    bool in = false;
+    if (b < SD) {
+      const int ax = b % S, t = b / S;
+      const int ay = t % S, az = t / S;
+      in = sample_inside<D>(g, i, j, k, sub[ax], sub[ay], D == 3 ? sub[az] : 0.0, cx, cy, cz, R2);
+    }
+    const unsigned bal = __ballot_sync(0xffffffffu, in);
+    cnt += __popc(bal);
+    if (in) bits |= 1u << m;
+  }
+  return cnt;
+}
+
+__device__ __forceinline__ void bbox_axis(double c, double R, int n, int bc, int &lo, int &ext) {
+  int l = (int)floor(c - R) - 1;
+  int hgh = (int)ceil(c + R) + 1;
+  if (bc) {
+    if (l < 0) l = 0;
+    if (hgh > n - 1) hgh = n - 1;
+  } else if (hgh - l + 1 > n) {  // box wider than the periodic axis: every node once
+    l = 0;
+    hgh = n - 1;
+  }
+  lo = l;
+  ext = hgh - l + 1;
+  if (ext < 0) ext = 0;
+}
+
+constexpr int kMapChunk = 1024;
+
+// pass 1: one group of G threads per particle walks the particle's bounding box.
+template <int D, int G>
+__global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
+  constexpr int groups = 128 / G;
+  __shared__ double sub[256];
+  __shared__ int list[groups][kMapChunk];
+  __shared__ int nlist[groups];
+  for (int t = threadIdx.x; t < a.S; t += blockDim.x) sub[t] = sub_offset(t, a.S);
+  const int grp = threadIdx.x / G, gl = threadIdx.x % G;
+  const int64_t p = (int64_t)blockIdx.x * groups + grp;
+  const bool active = p < a.P;
+  double cx = 0, cy = 0, cz = 0, R = 1;
+  int lo[3] = {0, 0, 0}, ext[3] = {0, 0, 1};
+  if (active) {
+    cx = a.pos[p];
+    cy = a.pos[a.P + p];
+    cz = D == 3 ? a.pos[2 * a.P + p] : 0.0;
+    R = a.radius[p];
+    bbox_axis(cx, R, a.g.nx, a.g.bcx, lo[0], ext[0]);
+    bbox_axis(cy, R, a.g.ny, a.g.bcy, lo[1], ext[1]);
+    if (D == 3) bbox_axis(cz, R, a.g.nz, a.g.bcz, lo[2], ext[2]);
+  }
+  const int nbox = active ? ext[0] * ext[1] * ext[2] : 0;
+  const double R2 = __dmul_rn(R, R);
+  const double rin = R - a.h_in, rout = R + a.h_out;
+  const double rin2 = rin > 0.0 ? rin * rin : -1.0, rout2 = rout * rout;
+  // all groups of the block iterate the same number of chunks (block-wide barriers)
+  int maxbox = nbox;
+  __shared__ int smax;
+  if (threadIdx.x == 0) smax = 0;
+  __syncthreads();
+  atomicMax(&smax, nbox);
+  __syncthreads();
+  maxbox = smax;
+
+  auto node_of = [&](int b, int &i, int &j, int &k) {
+    const int bi = b % ext[0], t = b / ext[0];
+    const int bj = t % ext[1], bk = t / ext[1];
+    i = lo[0] + bi;
+    j = lo[1] + bj;
+    k = lo[2] + bk;
+    if (!a.g.bcx) i = wrap_i(i, a.g.nx);
+    if (!a.g.bcy) j = wrap_i(j, a.g.ny);
+    if (D == 3 && !a.g.bcz) k = wrap_i(k, a.g.nz);
+  };
+  auto commit = [&](int i, int j, int k, int cnt) {
+    const int64_t x = ((int64_t)k * a.g.ny + j) * a.g.nx + i;
+    const int32_t old = atomicExch(a.pid + x, (int32_t)p);
+    a.eps_cnt[x] = (uint8_t)cnt;
+    if (old != -1 && old != (int32_t)p) {
+      const int slot = atomicAdd(a.counters, 1);
+      if (slot < a.contested_cap) a.contested[slot] = x;
+      else a.counters[1] = 1;
+    }
+  };
+
+  for (int base = 0; base < maxbox; base += kMapChunk) {
+    if (gl == 0) nlist[grp] = 0;
+    __syncthreads();
+    // phase A: classify nodes by the distance of the node centre
+    for (int b = base + gl; b < nbox && b < base + kMapChunk; b += G) {
+      int i, j, k;
+      node_of(b, i, j, k);
+      double dx = (double)i - cx, dy = (double)j - cy, dz = D == 3 ? (double)k - cz : 0.0;
+      if (!a.g.bcx) dx = min_image_d(dx, a.g.nx);
+      if (!a.g.bcy) dy = min_image_d(dy, a.g.ny);
+      if (D == 3 && !a.g.bcz) dz = min_image_d(dz, a.g.nz);
+      const double d2 = dx * dx + dy * dy + dz * dz;
+      if (d2 <= rin2) {
+        commit(i, j, k, a.SD);          // every sample is inside (triangle inequality + margin)
+      } else if (d2 <= rout2) {
+        const int slot = atomicAdd(&nlist[grp], 1);
+        list[grp][slot] = b;            // boundary cell: sample it
+      }
+    }
+    __syncthreads();
+    // phase B: one warp per boundary node, lanes over the samples
+    const int nl = nlist[grp];
+    constexpr int wpg = G / 32;
+    for (int e = gl / 32; e < nl; e += wpg) {
+      int i, j, k;
+      node_of(list[grp][e], i, j, k);
+      unsigned bits;
+      const int cnt = warp_count_samples<D>(a.g, a.S, a.SD, sub, i, j, k, cx, cy, cz, R2, bits);
+      if ((threadIdx.x & 31) == 0 && cnt > 0) commit(i, j, k, cnt);
+    }
+    __syncthreads();
+  }
+}
+
+// pass 2: nodes reached by more than one particle are recomputed from the definition:
+// union of the inside samples, covering particle = most samples, ties -> lowest index.
+template <int D>
+__global__ void __launch_bounds__(128) map_contested_kernel(const MapArgs a, const CellGeom cg,
+                                                            const int32_t *__restrict__ start,
+                                                            const int32_t *__restrict__ items) {
+  __shared__ double sub[256];
+  for (int t = threadIdx.x; t < a.S; t += blockDim.x) sub[t] = sub_offset(t, a.S);
+  __syncthreads();
+  int total = a.counters[0];
+  if (total > a.contested_cap) total = (int)a.contested_cap;
+  const int warps = (gridDim.x * blockDim.x) >> 5;
+  const int wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  for (int e = wid; e < total; e += warps) {
+    const int64_t x = a.contested[e];
+    const int i = (int)(x % a.g.nx);
+    const int64_t r = x / a.g.nx;
+    const int j = (int)(r % a.g.ny), k = (int)(r / a.g.ny);
+    const int ccx = cell_coord((double)i, cg, 0), ccy = cell_coord((double)j, cg, 1);
+    const int ccz = D == 3 ? cell_coord((double)k, cg, 2) : 0;
+    unsigned ubits = 0;
+    int best_cnt = 0, best_p = -1;
+    for (int oz = D == 3 ? off_lo(cg.nc[2], cg.periodic[2]) : 0; oz <= (D == 3 ? off_hi(cg.nc[2], cg.periodic[2]) : 0); ++oz)
+      for (int oy = off_lo(cg.nc[1], cg.periodic[1]); oy <= off_hi(cg.nc[1], cg.periodic[1]); ++oy)
+        for (int ox = off_lo(cg.nc[0], cg.periodic[0]); ox <= off_hi(cg.nc[0], cg.periodic[0]); ++ox) {
+          int nx_ = ccx + ox, ny_ = ccy + oy, nz_ = ccz + oz;
+          if (cg.periodic[0]) nx_ = wrap_i(nx_, cg.nc[0]);
+          else if (nx_ < 0 || nx_ >= cg.nc[0]) continue;
+          if (cg.periodic[1]) ny_ = wrap_i(ny_, cg.nc[1]);
+          else if (ny_ < 0 || ny_ >= cg.nc[1]) continue;
+          if (D == 3) {
+            if (cg.periodic[2]) nz_ = wrap_i(nz_, cg.nc[2]);
+            else if (nz_ < 0 || nz_ >= cg.nc[2]) continue;
+          }
+          const int c = (nz_ * cg.nc[1] + ny_) * cg.nc[0] + nx_;
+          for (int it = start[c]; it < start[c + 1]; ++it) {
+            const int p = items[it];
+            const double pcx = a.pos[p], pcy = a.pos[a.P + p], pcz = D == 3 ? a.pos[2 * a.P + p] : 0.0;
+            const double R = a.radius[p];
+            unsigned bits;
+            const int cnt = warp_count_samples<D>(a.g, a.S, a.SD, sub, i, j, k, pcx, pcy, pcz, __dmul_rn(R, R), bits);
+            ubits |= bits;
+            if (cnt > best_cnt || (cnt == best_cnt && cnt > 0 && p < best_p)) {
+              best_cnt = cnt;
+              best_p = p;
+            }
+          }
+        }
+    int ucnt = 0;
+    for (int m = 0; m * 32 < a.SD; ++m) ucnt += __popc(__ballot_sync(0xffffffffu, (ubits >> m) & 1u));
+    if (lane == 0) {
+      a.eps_cnt[x] = (uint8_t)ucnt;
+      a.pid[x] = best_p;
+    }
+  }
+}
+
+lbmimb_status launch_map(lbmimb_lattice *h) {
+  lbmimb_status st;
+  if (!h->cl_valid && (st = build_cell_list(h)) != LBMIMB_OK) return st;
+  LBMIMB_CUDA(cudaMemsetAsync(h->eps_cnt, 0, (size_t)h->g.N, h->stream));
+  LBMIMB_CUDA(cudaMemsetAsync(h->pid, 0xFF, (size_t)h->g.N * 4, h->stream));
+  LBMIMB_CUDA(cudaMemsetAsync(h->counters, 0, 4, h->stream));
+  MapArgs a;
+  a.g = h->g;
+  a.S = h->prm.subsamples;
+  a.SD = h->SD;
+  a.P = h->P;
+  a.pos = h->pos;
+  a.radius = h->radius;
+  a.eps_cnt = h->eps_cnt;
+  a.pid = h->pid;
+  a.contested = h->contested;
+  a.contested_cap = h->contested_cap;
+  a.counters = h->counters;
+  const double hs = sqrt((double)h->g.dim) * (0.5 - 0.5 / (double)a.S);
+  a.h_in = hs + 1e-6;
+  a.h_out = hs + 1e-6;
+  if (h->g.dim == 2) {
+    map_particles_kernel<2, 32><<<blocks_for(h->P, 4), 128, 0, h->stream>>>(a);
+  } else {
+    map_particles_kernel<3, 128><<<blocks_for(h->P, 1), 128, 0, h->stream>>>(a);
+  }
+  LBMIMB_LAUNCH_CHECK(h, "map_particles_kernel");
+  CellGeom cg = cell_geom(h);
+  if (h->g.dim == 2)
+    map_contested_kernel<2><<<148 * 4, 128, 0, h->stream>>>(a, cg, h->cl.start, h->cl.items);
+  else
+    map_contested_kernel<3><<<148 * 4, 128, 0, h->stream>>>(a, cg, h->cl.start, h->cl.items);
+  LBMIMB_LAUNCH_CHECK(h, "map_contested_kernel");
+  return LBMIMB_OK;
+}
+
+// ---------------------------------------------------------------------------
+// a3: force / torque reduction, eq. (3) with the sign of R6.  One group of G threads per
+// particle gathers the exchange vectors of the nodes it covers inside its bounding box;
+// fixed traversal and tree order => bitwise reproducible.
+// ---------------------------------------------------------------------------
+template <int D, int G>
+__global__ void __launch_bounds__(128) reduce_forces_kernel(Geom g, int64_t P, const double *__restrict__ pos,
+                                                            const double *__restrict__ radius,
+                                                            const int32_t *__restrict__ pid,
+                                                            const double *__restrict__ s, double *__restrict__ force,
+                                                            double *__restrict__ torque) {
+  constexpr int groups = 128 / G;
+  constexpr int NV = D == 2 ? 3 : 6;
+  __shared__ double sh[groups][G / 32][NV];
+  const int grp = threadIdx.x / G, gl = threadIdx.x % G;
+  const int64_t p = (int64_t)blockIdx.x * groups + grp;
+  double acc[NV];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) acc[v] = 0.0;
+  if (p < P) {
+    const double cx = pos[p], cy = pos[P + p], cz = D == 3 ? pos[2 * P + p] : 0.0, R = radius[p];
+    int lo[3] = {0, 0, 0}, ext[3] = {0, 0, 1};
+    bbox_axis(cx, R, g.nx, g.bcx, lo[0], ext[0]);
+    bbox_axis(cy, R, g.ny, g.bcy, lo[1], ext[1]);
+    if (D == 3) bbox_axis(cz, R, g.nz, g.bcz, lo[2], ext[2]);
+    const int nbox = ext[0] * ext[1] * ext[2];
+    for (int b = gl; b < nbox; b += G) {
+      const int bi = b % ext[0], t = b / ext[0];
+      const int bj = t % ext[1], bk = t / ext[1];
+      int i = lo[0] + bi, j = lo[1] + bj, k = lo[2] + bk;
+      if (!g.bcx) i = wrap_i(i, g.nx);
+      if (!g.bcy) j = wrap_i(j, g.ny);
+      if (D == 3 && !g.bcz) k = wrap_i(k, g.nz);
+      const int64_t x = ((int64_t)k * g.ny + j) * g.nx + i;
+      if (pid[x] != (int32_t)p) continue;
+      double rx = (double)i - cx, ry = (double)j - cy, rz = D == 3 ? (double)k - cz : 0.0;
+      if (!g.bcx) rx = min_image_d(rx, g.nx);
+      if (!g.bcy) ry = min_image_d(ry, g.ny);
+      if (D == 3 && !g.bcz) rz = min_image_d(rz, g.nz);
+      const double sx = s[x], sy = s[g.N + x];
+      if (D == 2) {
+        acc[0] -= sx;
+        acc[1] -= sy;
+        acc[2] -= rx * sy - ry * sx;
+      } else {
+        const double sz = s[2 * g.N + x];
+        acc[0] -= sx;
+        acc[1] -= sy;
+        acc[2] -= sz;
+        acc[3] -= ry * sz - rz * sy;
+        acc[4] -= rz * sx - rx * sz;
+        acc[5] -= rx * sy - ry * sx;
+      }
+    }
+  }
+#pragma unroll
+  for (int v = 0; v < NV; ++v)
+    for (int o = 16; o > 0; o >>= 1) acc[v] += __shfl_down_sync(0xffffffffu, acc[v], o);
+  if ((gl & 31) == 0)
+    for (int v = 0; v < NV; ++v) sh[grp][gl >> 5][v] = acc[v];
+  __syncthreads();
+  if (gl == 0 && p < P) {
+    double tot[NV];
+    for (int v = 0; v < NV; ++v) {
+      tot[v] = 0.0;
+      for (int w = 0; w < G / 32; ++w) tot[v] += sh[grp][w][v];
+    }
+    for (int c = 0; c < D; ++c) force[(int64_t)c * P + p] = tot[c];
+    if (D == 2) {
+      torque[p] = tot[2];
+    } else {
+      for (int c = 0; c < 3; ++c) torque[(int64_t)c * P + p] = tot[3 + c];
+    }
+  }
+}
+
+lbmimb_status launch_reduce(lbmimb_lattice *h) {
+  if (h->g.dim == 2)
+    reduce_forces_kernel<2, 32><<<blocks_for(h->P, 4), 128, 0, h->stream>>>(h->g, h->P, h->pos, h->radius, h->pid,
+                                                                           h->s, h->force, h->torque);
+  else
+    reduce_forces_kernel<3, 128><<<blocks_for(h->P, 1), 128, 0, h->stream>>>(h->g, h->P, h->pos, h->radius, h->pid,
+                                                                            h->s, h->force, h->torque);
+  LBMIMB_LAUNCH_CHECK(h, "reduce_forces_kernel");
+  return LBMIMB_OK;
+}
+
+// ---------------------------------------------------------------------------
+// a4: DEM, eq. (4)-(5) with the readings R8-R11.
+// ---------------------------------------------------------------------------
+struct DemArgs {
+  Geom g;
+  CellGeom cg;
+  int64_t P;
+  double *pos, *vel, *omega;
+  const double *radius, *mass, *force, *torque;
+  double *fc;
+  const int32_t *start, *items;
+  double kn, ce;  // eta = ce * sqrt(kn * m_eff), ce = -2 ln e / sqrt(pi^2 + ln^2 e)
+  double gp[3];
+  double dt;
+};
+
+template <int D>
+__global__ void dem_contact_kernel(const DemArgs a) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= a.P) return;
+  const int n[3] = {a.g.nx, a.g.ny, a.g.nz};
+  double xi[3], vi[3], F[3] = {0.0, 0.0, 0.0};
+  for (int c = 0; c < D; ++c) {
+    xi[c] = a.pos[(int64_t)c * a.P + i];
+    vi[c] = a.vel[(int64_t)c * a.P + i];
+  }
+  const double Ri = a.radius[i], mi = a.mass[i];
+  int cc[3] = {0, 0, 0};
+  for (int c = 0; c < D; ++c) cc[c] = cell_coord(xi[c], a.cg, c);
+  const int nc0 = a.cg.nc[0], nc1 = a.cg.nc[1], nc2 = D == 3 ? a.cg.nc[2] : 1;
+  for (int oz = D == 3 ? off_lo(nc2, a.cg.periodic[2]) : 0; oz <= (D == 3 ? off_hi(nc2, a.cg.periodic[2]) : 0); ++oz)
+    for (int oy = off_lo(nc1, a.cg.periodic[1]); oy <= off_hi(nc1, a.cg.periodic[1]); ++oy)
+      for (int ox = off_lo(nc0, a.cg.periodic[0]); ox <= off_hi(nc0, a.cg.periodic[0]); ++ox) {
+        int ex = cc[0] + ox, ey = cc[1] + oy, ez = cc[2] + oz;
+        if (a.cg.periodic[0]) ex = wrap_i(ex, nc0);
+        else if (ex < 0 || ex >= nc0) continue;
+        if (a.cg.periodic[1]) ey = wrap_i(ey, nc1);
+        else if (ey < 0 || ey >= nc1) continue;
+        if (D == 3) {
+          if (a.cg.periodic[2]) ez = wrap_i(ez, nc2);
+          else if (ez < 0 || ez >= nc2) continue;
+        }
+        const int c = (ez * nc1 + ey) * nc0 + ex;
+        for (int it = a.start[c]; it < a.start[c + 1]; ++it) {
+          const int j = a.items[it];
+          if (j == (int)i) continue;
+          double d[3] = {0.0, 0.0, 0.0}, dist2 = 0.0;
+          for (int q = 0; q < D; ++q) {
+            d[q] = xi[q] - a.pos[(int64_t)q * a.P + j];
+            const bool per = q == 0 ? !a.g.bcx : (q == 1 ? !a.g.bcy : !a.g.bcz);
+            if (per) d[q] = min_image_d(d[q], n[q]);
+            dist2 += d[q] * d[q];
+          }
+          const double Rs = Ri + a.radius[j];
+          if (dist2 >= Rs * Rs) continue;
+          const double dist = sqrt(dist2);
+          const double delta = Rs - dist;
+          if (!(delta > 0.0)) continue;
+          const double mj = a.mass[j];
+          const double meff = mi * mj / (mi + mj);
+          const double eta = a.ce * sqrt(a.kn * meff);
+          double nrm[3], vn = 0.0;
+          for (int q = 0; q < D; ++q) {
+            nrm[q] = d[q] / dist;
+            vn += (vi[q] - a.vel[(int64_t)q * a.P + j]) * nrm[q];
+          }
+          const double mag = a.kn * delta - eta * vn;
+          for (int q = 0; q < D; ++q) F[q] += mag * nrm[q];
+        }
+      }
+  // walls: planes at -1/2 and n-1/2 of a wall axis, m_eff = m_i (R10)
+  for (int q = 0; q < D; ++q) {
+    const bool wall = q == 0 ? a.g.bcx : (q == 1 ? a.g.bcy : a.g.bcz);
+    if (!wall) continue;
+    const double eta = a.ce * sqrt(a.kn * mi);
+    double delta = Ri - (xi[q] + 0.5);
+    if (delta > 0.0) F[q] += a.kn * delta - eta * vi[q];
+    delta = Ri - (((double)n[q] - 0.5) - xi[q]);
+    if (delta > 0.0) F[q] += -a.kn * delta - eta * vi[q];
+  }
+  for (int q = 0; q < D; ++q) a.fc[(int64_t)q * a.P + i] = F[q];
+}
+
+// first half: v += dt/2 a0; x += dt v (wrapped into [0,n) on periodic axes)
+template <int D>
+__global__ void dem_kick_drift_kernel(const DemArgs a) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= a.P) return;
+  const int n[3] = {a.g.nx, a.g.ny, a.g.nz};
+  const double m = a.mass[p];
+  for (int q = 0; q < D; ++q) {
+    const int64_t id = (int64_t)q * a.P + p;
+    const double a0 = (a.force[id] + a.fc[id]) / m + a.gp[q];
+    const double v = a.vel[id] + 0.5 * a.dt * a0;
+    a.vel[id] = v;
+    double x = a.pos[id] + a.dt * v;
+    const bool per = q == 0 ? !a.g.bcx : (q == 1 ? !a.g.bcy : !a.g.bcz);
+    if (per) {
+      if (x >= (double)n[q]) x -= (double)n[q];
+      if (x < 0.0) x += (double)n[q];
+    }
+    a.pos[id] = x;
+  }
+}
+
+// second half: v += dt/2 a1; omega += dt T_h / I
+template <int D>
+__global__ void dem_kick_kernel(const DemArgs a) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= a.P) return;
+  const double m = a.mass[p], R = a.radius[p];
+  for (int q = 0; q < D; ++q) {
+    const int64_t id = (int64_t)q * a.P + p;
+    const double a1 = (a.force[id] + a.fc[id]) / m + a.gp[q];
+    a.vel[id] = a.vel[id] + 0.5 * a.dt * a1;
+  }
+  const double I = (D == 3 ? 0.4 : 0.5) * m * R * R;
+  constexpr int nt = D == 2 ? 1 : 3;
+  for (int q = 0; q < nt; ++q) {
+    const int64_t id = (int64_t)q * a.P + p;
+    a.omega[id] = a.omega[id] + a.dt * a.torque[id] / I;
+  }
+}
+
+template <int D>
+static lbmimb_status dem_impl(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
+  lbmimb_status st;
+  if (!h->cl_valid && (st = build_cell_list(h)) != LBMIMB_OK) return st;
+  DemArgs a;
+  a.g = h->g;
+  a.P = h->P;
+  a.pos = h->pos;
+  a.vel = h->vel;
+  a.omega = h->omega;
+  a.radius = h->radius;
+  a.mass = h->mass;
+  a.force = h->force;
+  a.torque = h->torque;
+  a.fc = h->fc;
+  a.start = h->cl.start;
+  a.items = h->cl.items;
+  a.kn = dem->kn;
+  const double le = log(dem->restitution);
+  a.ce = -2.0 * le / sqrt(M_PI * M_PI + le * le);
+  for (int c = 0; c < 3; ++c) a.gp[c] = dem->g_particle[c];
+  a.dt = dem->dt;
+  const int nb = blocks_for(h->P, 128);
+  a.cg = cell_geom(h);
+  dem_contact_kernel<D><<<nb, 128, 0, h->stream>>>(a);
+  LBMIMB_LAUNCH_CHECK(h, "dem_contact_kernel");
+  dem_kick_drift_kernel<D><<<nb, 128, 0, h->stream>>>(a);
+  LBMIMB_LAUNCH_CHECK(h, "dem_kick_drift_kernel");
+  if ((st = build_cell_list(h)) != LBMIMB_OK) return st;
+  a.cg = cell_geom(h);
+  dem_contact_kernel<D><<<nb, 128, 0, h->stream>>>(a);
+  LBMIMB_LAUNCH_CHECK(h, "dem_contact_kernel");
+  dem_kick_kernel<D><<<nb, 128, 0, h->stream>>>(a);
+  LBMIMB_LAUNCH_CHECK(h, "dem_kick_kernel");
+  return LBMIMB_OK;
+}
+
+lbmimb_status launch_dem(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
+  return h->g.dim == 2 ? dem_impl<2>(h, dem) : dem_impl<3>(h, dem);
+}
+
+}  // namespace lbmimb
