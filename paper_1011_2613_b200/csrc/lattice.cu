@@ -7,6 +7,9 @@
 // collides with eq. (1) of the paper and writes f*(x,t) to the other
 // buffer at its own node: every store is aligned and coalesced, the x-shifted loads
 // are misaligned by one element and served from L1/L2 sectors.
+#include <cstdlib>
+
+#include "collide.cuh"
 #include "lbmimb_internal.cuh"
 
 namespace lbmimb {
@@ -23,155 +26,81 @@ struct StepArgs {
   int nx, ny, nz;
   int bcx, bcy, bcz;
   unsigned tiles;      // blocks per lattice row
-  double omega;        // 1/tau
-  double gx, gy, gz;   // g_fluid
+  CollideParams cp;
 };
 
 constexpr int kStepThreads = 128;
 
-template <int D>
-__device__ __forceinline__ double min_image(double d, int n) {
-  double hn = 0.5 * (double)n;
-  if (d > hn) return d - (double)n;
-  if (d < -hn) return d + (double)n;
-  return d;
-}
-
 // ---------------------------------------------------------------------------
-// a2: fused collide-and-stream.  IMB = particles present, EMIT = also store the
-// exchange vector s = beta*rho*(V_S - u) (= beta sum_i Omega_i c_i, P6).
+// a2: fused collide-and-stream, one thread per node, one block per row segment.
+// IMB = particles present, EMIT = also store the exchange vector s.
+// The y/z part of every source address is block-uniform; per thread only the three
+// x indices i-1, i, i+1 (wrapped) differ.  A warp takes the IMB path as a whole when
+// any of its nodes is covered (beta = 0 on the others), else the cheaper LBGK path.
 // ---------------------------------------------------------------------------
-template <int D, bool IMB, bool EMIT>
-__global__ void __launch_bounds__(kStepThreads) collide_stream_kernel(const StepArgs a) {
+template <int D, bool IMB, bool EMIT, int MINB>
+__global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(const StepArgs a) {
   using L = Lat<D>;
   constexpr int Q = L::Q;
   const unsigned row = blockIdx.x / a.tiles;
   const unsigned tile = blockIdx.x - row * a.tiles;
-  const int i = (int)(tile * kStepThreads + threadIdx.x);
-  if (i >= a.nx) return;
+  const int i0 = (int)(tile * kStepThreads + threadIdx.x);
+  const bool live = i0 < a.nx;
+  const int i = live ? i0 : a.nx - 1;
   const int k = D == 3 ? (int)(row / (unsigned)a.ny) : 0;
   const int j = (int)(row - (unsigned)k * (unsigned)a.ny);
-  const int64_t x = ((int64_t)k * a.ny + j) * a.nx + i;
+  const int64_t rowoff = ((int64_t)k * a.ny + j) * a.nx;
+  const int64_t x = rowoff + i;
+  const int im = i == 0 ? a.nx - 1 : i - 1;
+  const int ip = i == a.nx - 1 ? 0 : i + 1;
 
   // ---- gather (streaming) ----
   double f[Q];
 #pragma unroll
   for (int q = 0; q < Q; ++q) {
-    constexpr int dummy = 0;
-    (void)dummy;
     const int cx = L::cx(q), cy = L::cy(q), cz = L::cz(q);
     bool bounce = false;
-    int is = i - cx, js = j - cy, ks = k - cz;
-    if (cx != 0) {
-      if (is < 0 || is >= a.nx) {
-        if (a.bcx) bounce = true;
-        else is = is < 0 ? is + a.nx : is - a.nx;
-      }
+    int js = j - cy, ks = k - cz;
+    if (cy != 0 && (js < 0 || js >= a.ny)) {
+      if (a.bcy) bounce = true;
+      else js = js < 0 ? js + a.ny : js - a.ny;
     }
-    if (cy != 0) {
-      if (js < 0 || js >= a.ny) {
-        if (a.bcy) bounce = true;
-        else js = js < 0 ? js + a.ny : js - a.ny;
-      }
+    if (D == 3 && cz != 0 && (ks < 0 || ks >= a.nz)) {
+      if (a.bcz) bounce = true;
+      else ks = ks < 0 ? ks + a.nz : ks - a.nz;
     }
-    if (D == 3 && cz != 0) {
-      if (ks < 0 || ks >= a.nz) {
-        if (a.bcz) bounce = true;
-        else ks = ks < 0 ? ks + a.nz : ks - a.nz;
-      }
+    const double *base = bounce ? a.fin + ((int64_t)opposite(q) * a.N + rowoff)
+                                : a.fin + ((int64_t)q * a.N + ((int64_t)ks * a.ny + js) * a.nx);
+    const int xs = (bounce || cx == 0) ? i : (cx == 1 ? im : ip);
+    f[q] = base[xs];
+  }
+  if (a.bcx && (i == 0 || i == a.nx - 1)) {
+    // x walls: the end nodes of a row bounce their own opposite population back (R15)
+#pragma unroll
+    for (int q = 1; q < Q; ++q) {
+      const int cx = L::cx(q);
+      if ((cx == 1 && i == 0) || (cx == -1 && i == a.nx - 1)) f[q] = a.fin[(int64_t)opposite(q) * a.N + x];
     }
-    const int64_t src = bounce ? (int64_t)opposite(q) * a.N + x
-                               : (int64_t)q * a.N + ((int64_t)ks * a.ny + js) * a.nx + is;
-    f[q] = a.fin[src];
   }
 
   int cnt = 0;
   if (IMB) cnt = a.eps_cnt[x];
 
-  // ---- moments ----
-  double rho = 0.0, mx = 0.0, my = 0.0, mz = 0.0;
-#pragma unroll
-  for (int q = 0; q < Q; ++q) {
-    rho += f[q];
-    if (L::cx(q) == 1) mx += f[q];
-    if (L::cx(q) == -1) mx -= f[q];
-    if (L::cy(q) == 1) my += f[q];
-    if (L::cy(q) == -1) my -= f[q];
-    if (D == 3) {
-      if (L::cz(q) == 1) mz += f[q];
-      if (L::cz(q) == -1) mz -= f[q];
-    }
-  }
-  const double inv = 1.0 / rho;
-  const double ux = mx * inv, uy = my * inv, uz = D == 3 ? mz * inv : 0.0;
-  const double om = a.omega;
-  const double uu15 = 1.5 * (ux * ux + uy * uy + uz * uz);
+  double rho, ux, uy, uz;
+  moments<D>(f, rho, ux, uy, uz);
 
-  double fs[Q];
-  if (!IMB || cnt == 0) {
-    // pure LBGK + body force:  f* = f - (f - feq)/tau + F_i,  F_i = 3 w rho c.g  (R3)
-    const double ev0 = rho * (1.0 - uu15);
-    fs[0] = f[0] - om * (f[0] - L::w(0) * ev0);
-#pragma unroll
-    for (int q = 1; q < Q; q += 2) {
-      const int cx = L::cx(q), cy = L::cy(q), cz = L::cz(q);
-      const double cu = cx * ux + cy * uy + (D == 3 ? cz * uz : 0.0);
-      const double cg = cx * a.gx + cy * a.gy + (D == 3 ? cz * a.gz : 0.0);
-      const double wr = L::w(q) * rho;
-      const double e = wr * (1.0 - uu15 + 4.5 * cu * cu);   // even part of feq
-      const double o = wr * 3.0 * cu;                        // odd part of feq
-      const double Fo = 3.0 * wr * cg;
-      fs[q] = f[q] - om * (f[q] - (e + o)) + Fo;
-      fs[q + 1] = f[q + 1] - om * (f[q + 1] - (e - o)) - Fo;
-    }
+  if (!IMB || !__any_sync(0xffffffffu, cnt > 0)) {
+    collide_fluid<D>(f, a.cp, rho, ux, uy, uz);
   } else {
-    // immersed moving boundary node, eq. (1)-(2)
-    const int p = a.pid[x];
-    const double beta = __ldg(a.beta_tab + cnt);
-    const double *pr = a.prec + (int64_t)p * prec_stride(D);
-    double vx, vy, vz = 0.0;
-    if (D == 2) {
-      double rx = (double)i - __ldg(pr + 0), ry = (double)j - __ldg(pr + 1);
-      if (!a.bcx) rx = min_image<D>(rx, a.nx);
-      if (!a.bcy) ry = min_image<D>(ry, a.ny);
-      const double w = __ldg(pr + 4);
-      vx = __ldg(pr + 2) - w * ry;
-      vy = __ldg(pr + 3) + w * rx;
-    } else {
-      double rx = (double)i - __ldg(pr + 0), ry = (double)j - __ldg(pr + 1), rz = (double)k - __ldg(pr + 2);
-      if (!a.bcx) rx = min_image<D>(rx, a.nx);
-      if (!a.bcy) ry = min_image<D>(ry, a.ny);
-      if (!a.bcz) rz = min_image<D>(rz, a.nz);
-      const double wx = __ldg(pr + 6), wy = __ldg(pr + 7), wz = __ldg(pr + 8);
-      vx = __ldg(pr + 3) + (wy * rz - wz * ry);
-      vy = __ldg(pr + 4) + (wz * rx - wx * rz);
-      vz = __ldg(pr + 5) + (wx * ry - wy * rx);
+    double beta = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
+    if (cnt > 0) {
+      const int p = a.pid[x];
+      beta = __ldg(a.beta_tab + cnt);
+      solid_velocity<D>(a.prec + (int64_t)p * prec_stride(D), i, j, k, a.nx, a.ny, a.nz, a.bcx, a.bcy, a.bcz, vx, vy,
+                        vz);
     }
-    const double vv15 = 1.5 * (vx * vx + vy * vy + vz * vz);
-    const double omb = (1.0 - beta) * om;
-    {
-      const double eu = L::w(0) * rho * (1.0 - uu15);
-      const double ev = L::w(0) * rho * (1.0 - vv15);
-      fs[0] = f[0] - omb * (f[0] - eu) + beta * (ev - eu);
-    }
-#pragma unroll
-    for (int q = 1; q < Q; q += 2) {
-      const int cx = L::cx(q), cy = L::cy(q), cz = L::cz(q);
-      const double cu = cx * ux + cy * uy + (D == 3 ? cz * uz : 0.0);
-      const double cv = cx * vx + cy * vy + (D == 3 ? cz * vz : 0.0);
-      const double cg = cx * a.gx + cy * a.gy + (D == 3 ? cz * a.gz : 0.0);
-      const double wr = L::w(q) * rho;
-      const double eu = wr * (1.0 - uu15 + 4.5 * cu * cu), ou = wr * 3.0 * cu;
-      const double ev = wr * (1.0 - vv15 + 4.5 * cv * cv), ov = wr * 3.0 * cv;
-      const double Fo = 3.0 * wr * cg;
-      // Omega_q = f_-q - f_q + feq_q(V) - feq_-q(u);  Omega_-q = f_q - f_-q + feq_-q(V) - feq_q(u)
-      const double df = f[q + 1] - f[q];
-      const double Op = df + (ev + ov) - (eu - ou);
-      const double Om = -df + (ev - ov) - (eu + ou);
-      fs[q] = f[q] - omb * (f[q] - (eu + ou)) + beta * Op + Fo;
-      fs[q + 1] = f[q + 1] - omb * (f[q + 1] - (eu - ou)) + beta * Om - Fo;
-    }
-    if (EMIT) {
+    collide_imb<D>(f, a.cp, rho, ux, uy, uz, beta, vx, vy, vz);
+    if (EMIT && cnt > 0 && live) {
       const double br = beta * rho;
       a.s[x] = br * (vx - ux);
       a.s[a.N + x] = br * (vy - uy);
@@ -179,8 +108,10 @@ __global__ void __launch_bounds__(kStepThreads) collide_stream_kernel(const Step
     }
   }
 
+  if (live) {
 #pragma unroll
-  for (int q = 0; q < Q; ++q) a.fout[(int64_t)q * a.N + x] = fs[q];
+    for (int q = 0; q < Q; ++q) a.fout[(int64_t)q * a.N + x] = f[q];
+  }
 }
 
 // ---------------------------------------------------------------------------
@@ -332,14 +263,45 @@ lbmimb_status launch_init_rest(lbmimb_lattice *h) {
   return LBMIMB_OK;
 }
 
+template <int D, int MINB>
+static void launch_cs2(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, bool imb, bool emit) {
+  if (!imb)
+    collide_stream_kernel<D, false, false, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
+  else if (!emit)
+    collide_stream_kernel<D, true, false, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
+  else
+    collide_stream_kernel<D, true, true, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
+}
+
+// Experiment switch (environment LBMIMB_STEP_VARIANT): 0-9 plain kernel with different
+// occupancy targets, >= 10 the TMA-staged kernel of lattice_tma.cu.
+int step_variant() {
+  static int v = -1;
+  if (v < 0) {
+    const char *e = getenv("LBMIMB_STEP_VARIANT");
+    v = e ? atoi(e) : 0;
+  }
+  return v;
+}
+
 template <int D>
 static void launch_cs(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, bool imb, bool emit) {
-  if (!imb)
-    collide_stream_kernel<D, false, false><<<blocks, kStepThreads, 0, h->stream>>>(a);
-  else if (!emit)
-    collide_stream_kernel<D, true, false><<<blocks, kStepThreads, 0, h->stream>>>(a);
-  else
-    collide_stream_kernel<D, true, true><<<blocks, kStepThreads, 0, h->stream>>>(a);
+  if (D == 3) {
+    switch (step_variant()) {
+      case 1: launch_cs2<D, 5>(h, a, blocks, imb, emit); break;
+      case 2: launch_cs2<D, 6>(h, a, blocks, imb, emit); break;
+      case 3: launch_cs2<D, 8>(h, a, blocks, imb, emit); break;
+      default: launch_cs2<D, 7>(h, a, blocks, imb, emit); break;
+    }
+  } else {
+    switch (step_variant()) {
+      case 1: launch_cs2<D, 8>(h, a, blocks, imb, emit); break;
+      case 2: launch_cs2<D, 10>(h, a, blocks, imb, emit); break;
+      case 3: launch_cs2<D, 12>(h, a, blocks, imb, emit); break;
+      case 4: launch_cs2<D, 16>(h, a, blocks, imb, emit); break;
+      default: launch_cs2<D, 9>(h, a, blocks, imb, emit); break;
+    }
+  }
 }
 
 lbmimb_status launch_collide_stream(lbmimb_lattice *h, bool emit) {
@@ -359,13 +321,15 @@ lbmimb_status launch_collide_stream(lbmimb_lattice *h, bool emit) {
   a.bcy = h->g.bcy;
   a.bcz = h->g.bcz;
   a.tiles = (unsigned)((h->g.nx + kStepThreads - 1) / kStepThreads);
-  a.omega = 1.0 / h->prm.tau;
-  a.gx = h->prm.g_fluid[0];
-  a.gy = h->prm.g_fluid[1];
-  a.gz = h->g.dim == 3 ? h->prm.g_fluid[2] : 0.0;
+  a.cp = make_collide_params(h);
   const int64_t blocks = (int64_t)a.tiles * h->g.ny * h->g.nz;
   if (blocks > 0x7fffffff) return fail(LBMIMB_EINVAL, "lattice needs more than 2^31 thread blocks");
   const bool imb = h->P > 0;
+  if (step_variant() >= 10) {
+    bool done = false;
+    lbmimb_status st = launch_collide_stream_tma(h, emit, step_variant(), &done);
+    if (st != LBMIMB_OK || done) return st;
+  }
   if (h->g.dim == 2)
     launch_cs<2>(h, a, (unsigned)blocks, imb, emit);
   else

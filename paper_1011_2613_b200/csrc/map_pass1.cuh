@@ -1,0 +1,212 @@
+// a1, pass 1 of the particle -> lattice mapping (included by particles.cu).
+//
+// One group of G threads per particle walks the particle's bounding box.
+//   phase A: every node is classified by the distance of its centre to the particle centre:
+//            surely full (count = S^D), surely empty, or a boundary cell that must be sampled;
+//   phase B: one THREAD per boundary cell counts the inside samples.  The squared distance is
+//            separable, d2 = (dx^2 + dy^2) + dz^2 with dx depending on (i, ax) only, so the S
+//            values per axis are formed once (S*D subtract/multiply) and the S^D samples cost one
+//            or two additions and a compare each.  Every operation is the same IEEE operation on
+//            the same operands as in the definition (include/lbmimb.h a1), so the counts are
+//            bit-exact; only the order in which samples are visited differs.
+// Nodes reached by more than one particle are detected with an atomic exchange on pid and
+// queued for pass 2 (map_contested_kernel), which recomputes them from the definition.
+#pragma once
+// (included inside namespace lbmimb, after MapArgs / bbox_axis / min_image_d / wrap_i / sub_offset)
+
+constexpr int kMapChunk = 1024;
+
+// exact b / d and b % d for 0 <= b < 2^24, d >= 1, without the integer-division sequence
+__device__ __forceinline__ void fast_divmod(int b, int d, float inv_d, int &q, int &r) {
+  q = __float2int_rz((float)b * inv_d);
+  r = b - q * d;
+  if (r < 0) {
+    --q;
+    r += d;
+  } else if (r >= d) {
+    ++q;
+    r -= d;
+  }
+}
+
+// inside-sample count of one node, compile-time S (register arrays)
+template <int D, int S>
+__device__ __forceinline__ int thread_count_fixed(const Geom &g, const double *__restrict__ sub, int i, int j, int k,
+                                                  double cx, double cy, double cz, double R2, bool wx, bool wy,
+                                                  bool wz) {
+  double dx2[S], dy2[S], dz2[S];
+  const double di = (double)i, dj = (double)j, dk = (double)k;
+#pragma unroll
+  for (int a = 0; a < S; ++a) {
+    const double so = sub[a];
+    double dx = __dsub_rn(__dadd_rn(di, so), cx);
+    double dy = __dsub_rn(__dadd_rn(dj, so), cy);
+    if (wx) dx = min_image_d(dx, g.nx);
+    if (wy) dy = min_image_d(dy, g.ny);
+    dx2[a] = __dmul_rn(dx, dx);
+    dy2[a] = __dmul_rn(dy, dy);
+    if (D == 3) {
+      double dz = __dsub_rn(__dadd_rn(dk, so), cz);
+      if (wz) dz = min_image_d(dz, g.nz);
+      dz2[a] = __dmul_rn(dz, dz);
+    } else {
+      dz2[a] = 0.0;
+    }
+  }
+  int cnt = 0;
+#pragma unroll
+  for (int ay = 0; ay < S; ++ay) {
+#pragma unroll
+    for (int ax = 0; ax < S; ++ax) {
+      const double s2 = __dadd_rn(dx2[ax], dy2[ay]);
+      if (D == 2) {
+        cnt += s2 <= R2 ? 1 : 0;
+      } else {
+#pragma unroll
+        for (int az = 0; az < S; ++az) cnt += __dadd_rn(s2, dz2[az]) <= R2 ? 1 : 0;
+      }
+    }
+  }
+  return cnt;
+}
+
+// inside-sample count of one node, run-time S
+template <int D>
+__device__ __forceinline__ int thread_count_generic(const Geom &g, int S, const double *__restrict__ sub, int i, int j,
+                                                    int k, double cx, double cy, double cz, double R2, bool wx, bool wy,
+                                                    bool wz) {
+  const double di = (double)i, dj = (double)j, dk = (double)k;
+  int cnt = 0;
+  for (int az = 0; az < (D == 3 ? S : 1); ++az) {
+    double dz2 = 0.0;
+    if (D == 3) {
+      double dz = __dsub_rn(__dadd_rn(dk, sub[az]), cz);
+      if (wz) dz = min_image_d(dz, g.nz);
+      dz2 = __dmul_rn(dz, dz);
+    }
+    for (int ay = 0; ay < S; ++ay) {
+      double dy = __dsub_rn(__dadd_rn(dj, sub[ay]), cy);
+      if (wy) dy = min_image_d(dy, g.ny);
+      const double dy2 = __dmul_rn(dy, dy);
+      for (int ax = 0; ax < S; ++ax) {
+        double dx = __dsub_rn(__dadd_rn(di, sub[ax]), cx);
+        if (wx) dx = min_image_d(dx, g.nx);
+        double d2 = __dadd_rn(__dmul_rn(dx, dx), dy2);
+        if (D == 3) d2 = __dadd_rn(d2, dz2);
+        cnt += d2 <= R2 ? 1 : 0;
+      }
+    }
+  }
+  return cnt;
+}
+
+// does the bounding box of this particle touch the periodic seam of an axis (or cover it whole)?
+__device__ __forceinline__ bool crosses_seam(double c, double R, int n, int bc) {
+  if (bc) return false;
+  const int l = (int)floor(c - R) - 1;
+  const int h = (int)ceil(c + R) + 1;
+  return l < 0 || h > n - 1;
+}
+
+template <int D, int G, int SFIX>
+__global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
+  constexpr int groups = 128 / G;
+  __shared__ double sub[256];
+  __shared__ int list[groups][kMapChunk];
+  __shared__ int nlist[groups];
+  __shared__ int smax;
+  for (int t = threadIdx.x; t < a.S; t += blockDim.x) sub[t] = sub_offset(t, a.S);
+  if (threadIdx.x == 0) smax = 0;
+  const int grp = threadIdx.x / G, gl = threadIdx.x % G;
+  const int64_t p = (int64_t)blockIdx.x * groups + grp;
+  const bool active = p < a.P;
+  double cx = 0, cy = 0, cz = 0, R = 1;
+  int lo[3] = {0, 0, 0}, ext[3] = {1, 1, 1};
+  bool wx = false, wy = false, wz = false;
+  if (active) {
+    cx = a.pos[p];
+    cy = a.pos[a.P + p];
+    cz = D == 3 ? a.pos[2 * a.P + p] : 0.0;
+    R = a.radius[p];
+    bbox_axis(cx, R, a.g.nx, a.g.bcx, lo[0], ext[0]);
+    bbox_axis(cy, R, a.g.ny, a.g.bcy, lo[1], ext[1]);
+    if (D == 3) bbox_axis(cz, R, a.g.nz, a.g.bcz, lo[2], ext[2]);
+    wx = crosses_seam(cx, R, a.g.nx, a.g.bcx);
+    wy = crosses_seam(cy, R, a.g.ny, a.g.bcy);
+    wz = D == 3 && crosses_seam(cz, R, a.g.nz, a.g.bcz);
+  }
+  const int64_t nbox64 = active ? (int64_t)ext[0] * ext[1] * ext[2] : 0;
+  const int nbox = nbox64 > 0x7fffffff ? 0x7fffffff : (int)nbox64;
+  const bool fast = nbox < (1 << 24);
+  const float inv0 = 1.0f / (float)ext[0], inv1 = 1.0f / (float)ext[1];
+  const double R2 = __dmul_rn(R, R);
+  const double rin = R - a.h_in, rout = R + a.h_out;
+  const double rin2 = rin > 0.0 ? rin * rin : -1.0, rout2 = rout * rout;
+  __syncthreads();
+  atomicMax(&smax, nbox);
+  __syncthreads();
+  const int maxbox = smax;
+
+  auto node_of = [&](int b, int &i, int &j, int &k) {
+    int bi, bj, bk, t;
+    if (fast) {
+      fast_divmod(b, ext[0], inv0, t, bi);
+      fast_divmod(t, ext[1], inv1, bk, bj);
+    } else {
+      bi = b % ext[0];
+      t = b / ext[0];
+      bj = t % ext[1];
+      bk = t / ext[1];
+    }
+    i = lo[0] + bi;
+    j = lo[1] + bj;
+    k = lo[2] + bk;
+    if (wx) i = wrap_i(i, a.g.nx);
+    if (wy) j = wrap_i(j, a.g.ny);
+    if (D == 3 && wz) k = wrap_i(k, a.g.nz);
+  };
+  auto commit = [&](int i, int j, int k, int cnt) {
+    const int64_t x = ((int64_t)k * a.g.ny + j) * a.g.nx + i;
+    const int32_t old = atomicExch(a.pid + x, (int32_t)p);
+    a.eps_cnt[x] = (uint8_t)cnt;
+    if (old != -1 && old != (int32_t)p) {
+      const int slot = atomicAdd(a.counters, 1);
+      if (slot < a.contested_cap) a.contested[slot] = x;
+      else a.counters[1] = 1;
+    }
+  };
+
+  for (int base = 0; base < maxbox; base += kMapChunk) {
+    if (gl == 0) nlist[grp] = 0;
+    __syncthreads();
+    // phase A: classify nodes by the distance of the node centre
+    for (int b = base + gl; b < nbox && b < base + kMapChunk; b += G) {
+      int i, j, k;
+      node_of(b, i, j, k);
+      double dx = (double)i - cx, dy = (double)j - cy, dz = D == 3 ? (double)k - cz : 0.0;
+      if (wx) dx = min_image_d(dx, a.g.nx);
+      if (wy) dy = min_image_d(dy, a.g.ny);
+      if (D == 3 && wz) dz = min_image_d(dz, a.g.nz);
+      const double d2 = dx * dx + dy * dy + dz * dz;
+      if (d2 <= rin2) {
+        commit(i, j, k, a.SD);          // every sample is inside (triangle inequality + margin)
+      } else if (d2 <= rout2) {
+        const int slot = atomicAdd(&nlist[grp], 1);
+        list[grp][slot] = b;            // boundary cell: sample it
+      }
+    }
+    __syncthreads();
+    // phase B: one thread per boundary cell
+    const int nl = nlist[grp];
+    for (int e = gl; e < nl; e += G) {
+      int i, j, k;
+      node_of(list[grp][e], i, j, k);
+      int cnt;
+      if (SFIX > 0) cnt = thread_count_fixed<D, (SFIX > 0 ? SFIX : 1)>(a.g, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
+      else cnt = thread_count_generic<D>(a.g, a.S, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
+      if (cnt > 0) commit(i, j, k, cnt);
+    }
+    __syncthreads();
+  }
+}
+

@@ -275,16 +275,31 @@ __device__ __forceinline__ double sub_offset(int a, int S) {
   return __dsub_rn(__ddiv_rn(__dadd_rn((double)a, 0.5), (double)S), 0.5);
 }
 
+// Per-CTA table of the sample offsets: sample b = (az*S + ay)*S + ax -> (sub[ax], sub[ay], sub[az]).
+struct SampleTable {
+  double sx[256], sy[256], sz[256];
+};
+
+__device__ __forceinline__ void fill_sample_table(SampleTable &t, int S, int SD, int dim) {
+  for (int b = threadIdx.x; b < SD; b += blockDim.x) {
+    const int ax = b % S, r = b / S;
+    const int ay = r % S, az = r / S;
+    t.sx[b] = sub_offset(ax, S);
+    t.sy[b] = sub_offset(ay, S);
+    t.sz[b] = dim == 3 ? sub_offset(az, S) : 0.0;
+  }
+}
+
 template <int D>
-__device__ __forceinline__ bool sample_inside(const Geom &g, int i, int j, int k, double sx, double sy, double sz,
-                                              double cx, double cy, double cz, double R2) {
-  double dx = __dsub_rn(__dadd_rn((double)i, sx), cx);
-  double dy = __dsub_rn(__dadd_rn((double)j, sy), cy);
+__device__ __forceinline__ bool sample_inside(const Geom &g, double di, double dj, double dk, double sx, double sy,
+                                              double sz, double cx, double cy, double cz, double R2) {
+  double dx = __dsub_rn(__dadd_rn(di, sx), cx);
+  double dy = __dsub_rn(__dadd_rn(dj, sy), cy);
   if (!g.bcx) dx = min_image_d(dx, g.nx);
   if (!g.bcy) dy = min_image_d(dy, g.ny);
   double d2 = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
   if (D == 3) {
-    double dz = __dsub_rn(__dadd_rn((double)k, sz), cz);
+    double dz = __dsub_rn(__dadd_rn(dk, sz), cz);
     if (!g.bcz) dz = min_image_d(dz, g.nz);
     d2 = __dadd_rn(d2, __dmul_rn(dz, dz));
   }
@@ -294,18 +309,15 @@ __device__ __forceinline__ bool sample_inside(const Geom &g, int i, int j, int k
 // number of inside samples of node (i,j,k) for one particle, computed by one warp
 // (lane l tests samples l, l+32, ...); also returns this lane's inside bits in `bits`.
 template <int D>
-__device__ __forceinline__ int warp_count_samples(const Geom &g, int S, int SD, const double *sub, int i, int j, int k,
+__device__ __forceinline__ int warp_count_samples(const Geom &g, int SD, const SampleTable &tab, int i, int j, int k,
                                                   double cx, double cy, double cz, double R2, unsigned &bits) {
   const int lane = threadIdx.x & 31;
+  const double di = (double)i, dj = (double)j, dk = (double)k;
   int cnt = 0;
   bits = 0;
   for (int m = 0, b = lane; m * 32 < SD; ++m, b += 32) {
     bool in = false;
-    if (b < SD) {
-      const int ax = b % S, t = b / S;
-      const int ay = t % S, az = t / S;
-      in = sample_inside<D>(g, i, j, k, sub[ax], sub[ay], D == 3 ? sub[az] : 0.0, cx, cy, cz, R2);
-    }
+    if (b < SD) in = sample_inside<D>(g, di, dj, dk, tab.sx[b], tab.sy[b], tab.sz[b], cx, cy, cz, R2);
     const unsigned bal = __ballot_sync(0xffffffffu, in);
     cnt += __popc(bal);
     if (in) bits |= 1u << m;
@@ -328,97 +340,7 @@ __device__ __forceinline__ void bbox_axis(double c, double R, int n, int bc, int
   if (ext < 0) ext = 0;
 }
 
-constexpr int kMapChunk = 1024;
-
-// pass 1: one group of G threads per particle walks the particle's bounding box.
-template <int D, int G>
-__global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
-  constexpr int groups = 128 / G;
-  __shared__ double sub[256];
-  __shared__ int list[groups][kMapChunk];
-  __shared__ int nlist[groups];
-  for (int t = threadIdx.x; t < a.S; t += blockDim.x) sub[t] = sub_offset(t, a.S);
-  const int grp = threadIdx.x / G, gl = threadIdx.x % G;
-  const int64_t p = (int64_t)blockIdx.x * groups + grp;
-  const bool active = p < a.P;
-  double cx = 0, cy = 0, cz = 0, R = 1;
-  int lo[3] = {0, 0, 0}, ext[3] = {0, 0, 1};
-  if (active) {
-    cx = a.pos[p];
-    cy = a.pos[a.P + p];
-    cz = D == 3 ? a.pos[2 * a.P + p] : 0.0;
-    R = a.radius[p];
-    bbox_axis(cx, R, a.g.nx, a.g.bcx, lo[0], ext[0]);
-    bbox_axis(cy, R, a.g.ny, a.g.bcy, lo[1], ext[1]);
-    if (D == 3) bbox_axis(cz, R, a.g.nz, a.g.bcz, lo[2], ext[2]);
-  }
-  const int nbox = active ? ext[0] * ext[1] * ext[2] : 0;
-  const double R2 = __dmul_rn(R, R);
-  const double rin = R - a.h_in, rout = R + a.h_out;
-  const double rin2 = rin > 0.0 ? rin * rin : -1.0, rout2 = rout * rout;
-  // all groups of the block iterate the same number of chunks (block-wide barriers)
-  int maxbox = nbox;
-  __shared__ int smax;
-  if (threadIdx.x == 0) smax = 0;
-  __syncthreads();
-  atomicMax(&smax, nbox);
-  __syncthreads();
-  maxbox = smax;
-
-  auto node_of = [&](int b, int &i, int &j, int &k) {
-    const int bi = b % ext[0], t = b / ext[0];
-    const int bj = t % ext[1], bk = t / ext[1];
-    i = lo[0] + bi;
-    j = lo[1] + bj;
-    k = lo[2] + bk;
-    if (!a.g.bcx) i = wrap_i(i, a.g.nx);
-    if (!a.g.bcy) j = wrap_i(j, a.g.ny);
-    if (D == 3 && !a.g.bcz) k = wrap_i(k, a.g.nz);
-  };
-  auto commit = [&](int i, int j, int k, int cnt) {
-    const int64_t x = ((int64_t)k * a.g.ny + j) * a.g.nx + i;
-    const int32_t old = atomicExch(a.pid + x, (int32_t)p);
-    a.eps_cnt[x] = (uint8_t)cnt;
-    if (old != -1 && old != (int32_t)p) {
-      const int slot = atomicAdd(a.counters, 1);
-      if (slot < a.contested_cap) a.contested[slot] = x;
-      else a.counters[1] = 1;
-    }
-  };
-
-  for (int base = 0; base < maxbox; base += kMapChunk) {
-    if (gl == 0) nlist[grp] = 0;
-    __syncthreads();
-    // phase A: classify nodes by the distance of the node centre
-    for (int b = base + gl; b < nbox && b < base + kMapChunk; b += G) {
-      int i, j, k;
-      node_of(b, i, j, k);
-      double dx = (double)i - cx, dy = (double)j - cy, dz = D == 3 ? (double)k - cz : 0.0;
-      if (!a.g.bcx) dx = min_image_d(dx, a.g.nx);
-      if (!a.g.bcy) dy = min_image_d(dy, a.g.ny);
-      if (D == 3 && !a.g.bcz) dz = min_image_d(dz, a.g.nz);
-      const double d2 = dx * dx + dy * dy + dz * dz;
-      if (d2 <= rin2) {
-        commit(i, j, k, a.SD);          // every sample is inside (triangle inequality + margin)
-      } else if (d2 <= rout2) {
-        const int slot = atomicAdd(&nlist[grp], 1);
-        list[grp][slot] = b;            // boundary cell: sample it
-      }
-    }
-    __syncthreads();
-    // phase B: one warp per boundary node, lanes over the samples
-    const int nl = nlist[grp];
-    constexpr int wpg = G / 32;
-    for (int e = gl / 32; e < nl; e += wpg) {
-      int i, j, k;
-      node_of(list[grp][e], i, j, k);
-      unsigned bits;
-      const int cnt = warp_count_samples<D>(a.g, a.S, a.SD, sub, i, j, k, cx, cy, cz, R2, bits);
-      if ((threadIdx.x & 31) == 0 && cnt > 0) commit(i, j, k, cnt);
-    }
-    __syncthreads();
-  }
-}
+#include "map_pass1.cuh"
 
 // pass 2: nodes reached by more than one particle are recomputed from the definition:
 // union of the inside samples, covering particle = most samples, ties -> lowest index.
@@ -426,8 +348,8 @@ template <int D>
 __global__ void __launch_bounds__(128) map_contested_kernel(const MapArgs a, const CellGeom cg,
                                                             const int32_t *__restrict__ start,
                                                             const int32_t *__restrict__ items) {
-  __shared__ double sub[256];
-  for (int t = threadIdx.x; t < a.S; t += blockDim.x) sub[t] = sub_offset(t, a.S);
+  __shared__ SampleTable tab;
+  fill_sample_table(tab, a.S, a.SD, D);
   __syncthreads();
   int total = a.counters[0];
   if (total > a.contested_cap) total = (int)a.contested_cap;
@@ -461,7 +383,7 @@ __global__ void __launch_bounds__(128) map_contested_kernel(const MapArgs a, con
             const double pcx = a.pos[p], pcy = a.pos[a.P + p], pcz = D == 3 ? a.pos[2 * a.P + p] : 0.0;
             const double R = a.radius[p];
             unsigned bits;
-            const int cnt = warp_count_samples<D>(a.g, a.S, a.SD, sub, i, j, k, pcx, pcy, pcz, __dmul_rn(R, R), bits);
+            const int cnt = warp_count_samples<D>(a.g, a.SD, tab, i, j, k, pcx, pcy, pcz, __dmul_rn(R, R), bits);
             ubits |= bits;
             if (cnt > best_cnt || (cnt == best_cnt && cnt > 0 && p < best_p)) {
               best_cnt = cnt;
@@ -500,9 +422,11 @@ lbmimb_status launch_map(lbmimb_lattice *h) {
   a.h_in = hs + 1e-6;
   a.h_out = hs + 1e-6;
   if (h->g.dim == 2) {
-    map_particles_kernel<2, 32><<<blocks_for(h->P, 4), 128, 0, h->stream>>>(a);
+    if (a.S == 8) map_particles_kernel<2, 32, 8><<<blocks_for(h->P, 4), 128, 0, h->stream>>>(a);
+    else map_particles_kernel<2, 32, 0><<<blocks_for(h->P, 4), 128, 0, h->stream>>>(a);
   } else {
-    map_particles_kernel<3, 128><<<blocks_for(h->P, 1), 128, 0, h->stream>>>(a);
+    if (a.S == 4) map_particles_kernel<3, 128, 4><<<blocks_for(h->P, 1), 128, 0, h->stream>>>(a);
+    else map_particles_kernel<3, 128, 0><<<blocks_for(h->P, 1), 128, 0, h->stream>>>(a);
   }
   LBMIMB_LAUNCH_CHECK(h, "map_particles_kernel");
   CellGeom cg = cell_geom(h);
