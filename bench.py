@@ -36,6 +36,11 @@ METRIC = "fp64 LBM-IMB MLUPS on 1 B200 and % of HBM roofline (bytes/update count
 UNIT = "MLUPS"
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused kernel from the committed
+# `ncu --set full` capture (profiles/r1_traffic.md); None where no capture exists for the workload.
+NCU_TRAFFIC_BYTES = {"C3": 21427389000}
+
+
 def measured_peak_gbs():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -282,7 +287,7 @@ def main():
     peak, peak_src = measured_peak_gbs()
     achieved = bytes_per_node * N / (kern_ms * 1e-3) / 1e9
     roof = {"bound": "hbm", "kernel": "collide_stream_kernel<%d,IMB,EMIT>" % w.dim, "achieved": achieved,
-            "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+            "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload), "peak_source": peak_src,
             "bytes_per_node": bytes_per_node, "nodes_per_launch": N, "kernel_ms": kern_ms,
             "kernel_mlups": N / (kern_ms * 1e-3) / 1e6, "frac_of_nominal_8TBs": achieved / 8000.0,
             "kernel_share_of_step": kern_ms / (total_ms / args.steps)}

@@ -216,7 +216,7 @@ def sub_box(w, lo, size):
     """Particle set of workload w seen from the all-periodic box [lo, lo+size):
     every particle (and periodic image) whose bounding box touches the box,
     translated by -lo (exact, centres are multiples of 2**-16).  Returns
-    (pos, vel, omega, radius, mass) for a lattice of `size` nodes."""
+    (pos, vel, omega, radius, mass, idx) for a lattice of `size` nodes; idx = original particle indices."""
     dim = w.dim
     lo = np.asarray(lo, dtype=np.float64)
     size = np.asarray(size, dtype=np.float64)
@@ -233,4 +233,4 @@ def sub_box(w, lo, size):
         keep_idx.append(idx)
     idx = np.concatenate(keep_idx)
     pos = np.concatenate(keep_pos, axis=1)
-    return pos, w.vel[:, idx].copy(), w.omega[:, idx].copy(), w.radius[idx].copy(), w.mass[idx].copy()
+    return pos, w.vel[:, idx].copy(), w.omega[:, idx].copy(), w.radius[idx].copy(), w.mass[idx].copy(), idx

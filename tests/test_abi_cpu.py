@@ -142,7 +142,7 @@ def test_sub_box_translation_is_exact():
     from paper_1011_2613_b200 import inputs
     w = inputs.reduced("C3")
     lo, size = (60, 10, 30), (24, 24, 24)
-    pos, vel, om, rad, mass = inputs.sub_box(w, lo, size)
+    pos, vel, om, rad, mass, idx = inputs.sub_box(w, lo, size)
     assert pos.shape[1] > 0 and np.array_equal(pos * 65536, np.round(pos * 65536))
     # every kept particle is an exact integer translate of an original one
     for p in range(pos.shape[1]):

@@ -1,0 +1,127 @@
+"""Full-size parity (`-m gpu`): C3 and C4 at BASELINE.json's sizes, in the launch configuration
+bench.py times, checked on sampled outputs the oracle can compute one by one.
+
+After n steps the state inside a box depends only on the initial state within n nodes of it, so the
+oracle runs the SAME particles (exact integer translates, paper_1011_2613_b200.inputs.sub_box) on a
+small lattice = box + halo; everything further than n + (2R + 3) nodes from the small lattice's edges
+is untouched by its artificial boundary and must match the full-size CUDA run to the usual tolerances.
+Plus invariants that hold at any size (mass conservation, total force vs momentum change).
+"""
+import numpy as np
+import pytest
+
+from paper_1011_2613_b200 import inputs
+from parity_util import F_TOL, assert_forces_close, force_floor
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lb():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1011_2613_b200 import binding
+    binding.load()
+    return binding
+
+
+def _fetch_wrapped(lat, lb, what, lo, size, n, bc):
+    """fetch_fields of a box that may cross the periodic seam in x (and z): assembled from pieces."""
+    dim = len(lo)
+    pieces = [[(lo[a], size[a], 0)] for a in range(dim)]
+    for a in range(dim):
+        l, s = lo[a], size[a]
+        if not bc[a] and (l < 0 or l + s > n[a]):
+            l0 = l % n[a]
+            first = min(s, n[a] - l0)
+            pieces[a] = [(l0, first, 0), (0, s - first, first)]
+    comps = {lb.FIELD_F: lat.Q, lb.FIELD_S: dim, lb.FIELD_U: dim}.get(what, 0)
+    dt = {lb.FIELD_EPS_CNT: np.uint8, lb.FIELD_PID: np.int32}.get(what, np.float64)
+    ext = tuple(reversed(list(size) + [1] * (3 - dim)))
+    out = np.empty(((comps,) if comps else ()) + ext, dtype=dt)
+    pz = pieces[2] if dim == 3 else [(0, 1, 0)]
+    for (z0, zs, zo) in pz:
+        for (y0, ys, yo) in pieces[1]:
+            for (x0, xs, xo) in pieces[0]:
+                if xs <= 0 or ys <= 0 or zs <= 0:
+                    continue
+                part = lat.fetch_fields(what, (x0, y0, z0), (x0 + xs, y0 + ys, z0 + zs))
+                out[..., zo:zo + zs, yo:yo + ys, xo:xo + xs] = part
+    return out
+
+
+def _check_boxes(orc, lb, w, nsteps, boxes):
+    R = float(w.radius.max())
+    rim = nsteps + int(2 * R) + 3
+    lat = lb.from_workload(w)
+    lat.map_particles()
+    lat.step(nsteps)
+    gF, gT = lat.reduce_particle_forces()
+    worst = 0.0
+    for lo, size, sub_bc in boxes:
+        pos, vel, om, rad, mass, idx = inputs.sub_box(w, lo, size)
+        assert pos.shape[1] > 3
+        eps, pid = orc.map_particles(w.dim, size, sub_bc, w.subsamples, pos, rad)
+        f = orc.init(w.dim, size)
+        for it in range(nsteps):
+            last = it == nsteps - 1
+            res = orc.step(w.dim, size, sub_bc, w.tau, w.g_fluid, w.subsamples, f, eps_cnt=eps, pid=pid, pos=pos,
+                           vel=vel, omega=om, want_s=last)
+            f, s = res if last else (res, None)
+        # inner region: `rim` nodes away from every artificial edge of the small lattice
+        inner = []
+        for a in range(w.dim):
+            lo_a = 0 if (sub_bc[a] and lo[a] == 0) else rim
+            hi_a = size[a] if (sub_bc[a] and lo[a] + size[a] == w.n[a]) else size[a] - rim
+            inner.append(slice(lo_a, hi_a))
+        sl = tuple(reversed(inner)) if w.dim == 3 else (slice(None),) + tuple(reversed(inner))
+        ge = _fetch_wrapped(lat, lb, lb.FIELD_EPS_CNT, lo, size, w.n, w.bc)
+        gp = _fetch_wrapped(lat, lb, lb.FIELD_PID, lo, size, w.n, w.bc)
+        gf = _fetch_wrapped(lat, lb, lb.FIELD_F, lo, size, w.n, w.bc)
+        assert np.array_equal(ge[sl], eps[sl]), "eps_cnt"
+        opid = np.where(pid >= 0, idx[np.maximum(pid, 0)], -1)
+        assert np.array_equal(gp[sl], opid[sl]), "pid"
+        fsl = (slice(None),) + sl
+        err = np.abs(gf[fsl] - f[fsl]).max() / np.abs(f[fsl]).max()
+        assert err <= F_TOL, "f: %.3e" % err
+        worst = max(worst, err)
+        assert np.abs(gf[fsl] - orc.init(w.dim, size)[fsl]).max() > 1e-8      # the flow has developed
+        # forces of the particles that lie wholly inside the inner region
+        F, T, aF, aT = orc.forces(w.dim, size, sub_bc, s, pid, pos)
+        keep = np.ones(pos.shape[1], dtype=bool)
+        for a in range(w.dim):
+            keep &= (pos[a] - rad - 2 >= inner[a].start) & (pos[a] + rad + 2 <= inner[a].stop - 1)
+        assert keep.sum() >= 1
+        ref = dict(force=F[:, keep], torque=T[:, keep], abs_f=aF[keep], abs_t=aT[keep],
+                   floor=force_floor(pid, pos.shape[1])[keep], radius=rad[keep])
+        assert_forces_close(gF[:, idx[keep]], gT[:, idx[keep]], ref)
+    return lat, worst
+
+
+def test_c3_full_size_sampled_boxes_and_mass(orc, lb):
+    w = inputs.c3()
+    n = 6
+    boxes = [((100, 400, 90), (64, 64, 64), (0, 0, 0)),          # interior
+             ((-20, 0, 230), (60, 70, 60), (0, 1, 0)),           # bottom wall, across the x and z seams
+             ((200, 1008 - 66, -10), (70, 66, 56), (0, 1, 0))]   # top wall, across both seams
+    lat, worst = _check_boxes(orc, lb, w, n, boxes)
+    m0 = float(w.nodes)
+    rho = lat.fetch_fields(lb.FIELD_RHO)
+    assert abs(rho.sum() - m0) / m0 < 1e-12                      # mass is conserved (P2) at full size
+    assert lat.time() == n
+    lat.close()
+
+
+def test_c4_full_size_sampled_boxes_and_mass(orc, lb):
+    w = inputs.c4()
+    n = 8
+    boxes = [((4000, 16000), (90, 90), (0, 0)),
+             ((-30, 0), (100, 80), (0, 1)),
+             ((8192 - 50, 32768 - 80), (100, 80), (0, 1))]
+    lat, worst = _check_boxes(orc, lb, w, n, boxes)
+    m0 = float(w.nodes)
+    total = 0.0
+    for j0 in range(0, 32768, 4096):                              # slab-wise: 268 M nodes
+        total += lat.fetch_fields(lb.FIELD_RHO, (0, j0, 0), (8192, j0 + 4096, 1)).sum()
+    assert abs(total - m0) / m0 < 1e-12
+    lat.close()
