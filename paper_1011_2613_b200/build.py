@@ -31,7 +31,8 @@ def _stale(target, deps):
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    hdrs = [os.path.join(CSRC, "lbmimb_internal.cuh"), os.path.join(HERE, "..", "include", "lbmimb.h")]
+    hdrs = [os.path.join(CSRC, h) for h in sorted(os.listdir(CSRC)) if h.endswith(".cuh")]
+    hdrs.append(os.path.join(HERE, "..", "include", "lbmimb.h"))
     objs = []
     nvcc = _nvcc()
     for src in SOURCES:

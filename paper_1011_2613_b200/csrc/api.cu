@@ -78,7 +78,7 @@ static Layout make_layout(const lbmimb_params *p, int64_t maxp) {
   L.off_f[1] = take((uint64_t)Q * L.N * 8);
   L.off_eps = take((uint64_t)L.N);
   L.off_pid = take((uint64_t)L.N * 4);
-  L.off_s = take((uint64_t)p->dim * L.N * 8);
+  L.off_s = take((uint64_t)exchange_stride(p->dim) * L.N * 8);
   L.off_beta = take(256 * 8);
   L.off_contested = take((uint64_t)L.contested_cap * 8);
   L.off_counters = take(64);

@@ -123,6 +123,19 @@ __device__ __forceinline__ void collide_imb(double (&f)[Lat<D>::Q], const Collid
   }
 }
 
+// Exchange vector of a covered node: one aligned record per node (16 B in 2D, 32 B = one DRAM
+// sector in 3D) so that the store and the later gather of a3 move whole sectors.
+template <int D>
+__device__ __forceinline__ void store_exchange(double *__restrict__ s, int64_t x, double sx, double sy, double sz) {
+  if (D == 2) {
+    reinterpret_cast<double2 *>(s)[x] = make_double2(sx, sy);
+  } else {
+    double2 *p = reinterpret_cast<double2 *>(s) + 2 * x;
+    p[0] = make_double2(sx, sy);
+    p[1] = make_double2(sz, 0.0);
+  }
+}
+
 // V_S = v_p + omega_p x (x_node - x_p), minimum image on periodic axes (R5)
 template <int D>
 __device__ __forceinline__ void solid_velocity(const double *__restrict__ pr, int i, int j, int k, int nx, int ny,

@@ -102,9 +102,7 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
     collide_imb<D>(f, a.cp, rho, ux, uy, uz, beta, vx, vy, vz);
     if (EMIT && cnt > 0 && live) {
       const double br = beta * rho;
-      a.s[x] = br * (vx - ux);
-      a.s[a.N + x] = br * (vy - uy);
-      if (D == 3) a.s[2 * a.N + x] = br * (vz - uz);
+      store_exchange<D>(a.s, x, br * (vx - ux), br * (vy - uy), br * (vz - uz));
     }
   }
 
@@ -222,7 +220,7 @@ __global__ void fetch_kernel(const FetchArgs a, const Geom g) {
       ((int32_t *)a.dst)[b] = a.pid[x];
     } else if (a.what == LBMIMB_FIELD_S) {
       const bool cov = a.have_particles && a.eps_cnt[x] > 0;
-      for (int c = 0; c < D; ++c) ((double *)a.dst)[(int64_t)c * a.box + b] = cov ? a.s[(int64_t)c * g.N + x] : 0.0;
+      for (int c = 0; c < D; ++c) ((double *)a.dst)[(int64_t)c * a.box + b] = cov ? a.s[x * exchange_stride(D) + c] : 0.0;
     } else {
       double f[L::Q];
       gather_node<D>(a.fpost, g, i, j, k, f);

@@ -239,9 +239,7 @@ __global__ void __launch_bounds__(TX + 32, MINB) collide_stream_tma_kernel(const
       collide_imb<D>(f, a.cp, rho, ux, uy, uz, beta, vx, vy, vz);
       if (EMIT && cnt > 0) {
         const double br = beta * rho;
-        a.s[x] = br * (vx - ux);
-        a.s[a.N + x] = br * (vy - uy);
-        if (D == 3) a.s[2 * a.N + x] = br * (vz - uz);
+        store_exchange<D>(a.s, x, br * (vx - ux), br * (vy - uy), br * (vz - uz));
       }
     }
     if (live) {

@@ -59,6 +59,9 @@ __host__ __device__ constexpr int opposite(int q) { return q == 0 ? 0 : ((q & 1)
 //   3D: x y z vx vy vz wx wy wz R   (10 doubles)      2D: x y vx vy w R (6 doubles)
 __host__ __device__ constexpr int prec_stride(int dim) { return dim == 3 ? 10 : 6; }
 
+// Exchange vectors s are stored as one record per node: [N][2] in 2D, [N][4] in 3D (4th slot unused).
+__host__ __device__ constexpr int exchange_stride(int dim) { return dim == 3 ? 4 : 2; }
+
 struct Geom {
   int dim;
   int nx, ny, nz;   // nodes per axis (each < 2^31)
@@ -98,7 +101,7 @@ struct lbmimb_lattice {
   int cur;
   uint8_t *eps_cnt;   // [N]
   int32_t *pid;       // [N]
-  double *s;          // [dim][N] exchange vectors of the last step
+  double *s;          // [N][exchange_stride] exchange vectors of the last step
   double *beta_tab;   // [256] beta(n_s / S^D, tau)
   int64_t *contested; // mapping fix-up list
   int64_t contested_cap;

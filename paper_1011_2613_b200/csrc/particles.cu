@@ -382,6 +382,14 @@ __global__ void __launch_bounds__(128) map_contested_kernel(const MapArgs a, con
             const int p = items[it];
             const double pcx = a.pos[p], pcy = a.pos[a.P + p], pcz = D == 3 ? a.pos[2 * a.P + p] : 0.0;
             const double R = a.radius[p];
+            {  // cheap reject: no sample of this node can lie inside a particle that far away
+              double ex = (double)i - pcx, ey = (double)j - pcy, ez = D == 3 ? (double)k - pcz : 0.0;
+              if (!a.g.bcx) ex = min_image_d(ex, a.g.nx);
+              if (!a.g.bcy) ey = min_image_d(ey, a.g.ny);
+              if (D == 3 && !a.g.bcz) ez = min_image_d(ez, a.g.nz);
+              const double ro = R + a.h_out;
+              if (ex * ex + ey * ey + ez * ez > ro * ro) continue;
+            }
             unsigned bits;
             const int cnt = warp_count_samples<D>(a.g, a.SD, tab, i, j, k, pcx, pcy, pcz, __dmul_rn(R, R), bits);
             ubits |= bits;
@@ -440,11 +448,82 @@ lbmimb_status launch_map(lbmimb_lattice *h) {
 
 // ---------------------------------------------------------------------------
 // a3: force / torque reduction, eq. (3) with the sign of R6.  One group of G threads per
-// particle gathers the exchange vectors of the nodes it covers inside its bounding box;
-// fixed traversal and tree order => bitwise reproducible.
+// particle walks the rows of the particle's bounding box, W lanes per row.  A node can only
+// belong to the particle if its centre is within R + h_out of the particle centre (the map's
+// own classification), so that test selects the candidates in registers and the pid and
+// exchange-vector loads of a candidate are independent of each other; U row slots are in
+// flight per thread.  Fixed traversal and tree order => bitwise reproducible.
 // ---------------------------------------------------------------------------
+template <int D, int G, int W>
+__device__ __forceinline__ void reduce_gather(const Geom &g, int32_t p, double cx, double cy, double cz, double rout2,
+                                              const int (&lo)[3], const int (&ext)[3], int gl,
+                                              const int32_t *__restrict__ pid, const double *__restrict__ s,
+                                              double *acc) {
+  constexpr int U = 4;
+  constexpr int RPI = G / W;  // row slots per iteration of the group
+  const int bi0 = gl % W, rs = gl / W;
+  const int nchunks = (ext[0] + W - 1) / W;
+  const int nslots = ext[1] * ext[2] * nchunks;
+  for (int s0 = rs; s0 < nslots; s0 += U * RPI) {
+    bool cand[U];
+    int32_t owner[U];
+    double2 s01[U], s23[U];
+    double rx[U], ry[U], rz[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int slot = s0 + u * RPI;
+      int row = slot, bi = bi0;
+      if (nchunks > 1) {
+        row = slot / nchunks;
+        bi += (slot - row * nchunks) * W;
+      }
+      const int bk = D == 3 ? row / ext[1] : 0;
+      const int bj = row - bk * ext[1];
+      int i = lo[0] + bi, j = lo[1] + bj, k = lo[2] + bk;
+      if (!g.bcx) i = wrap_i(i, g.nx);
+      if (!g.bcy) j = wrap_i(j, g.ny);
+      if (D == 3 && !g.bcz) k = wrap_i(k, g.nz);
+      rx[u] = (double)i - cx;
+      ry[u] = (double)j - cy;
+      rz[u] = D == 3 ? (double)k - cz : 0.0;
+      if (!g.bcx) rx[u] = min_image_d(rx[u], g.nx);
+      if (!g.bcy) ry[u] = min_image_d(ry[u], g.ny);
+      if (D == 3 && !g.bcz) rz[u] = min_image_d(rz[u], g.nz);
+      cand[u] = slot < nslots && bi < ext[0] && rx[u] * rx[u] + ry[u] * ry[u] + rz[u] * rz[u] <= rout2;
+      owner[u] = -1;
+      s01[u] = s23[u] = make_double2(0.0, 0.0);
+      if (cand[u]) {
+        const int64_t x = ((int64_t)k * g.ny + j) * g.nx + i;
+        const double2 *sr = reinterpret_cast<const double2 *>(s) + x * (exchange_stride(D) / 2);
+        owner[u] = __ldg(pid + x);
+        s01[u] = __ldg(sr);
+        if (D == 3) s23[u] = __ldg(sr + 1);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      if (owner[u] != p) continue;  // fixed order: u ascending (s of a node p does not own is never used)
+      const double sx = s01[u].x, sy = s01[u].y;
+      if (D == 2) {
+        acc[0] -= sx;
+        acc[1] -= sy;
+        acc[2] -= rx[u] * sy - ry[u] * sx;
+      } else {
+        const double sz = s23[u].x;
+        acc[0] -= sx;
+        acc[1] -= sy;
+        acc[2] -= sz;
+        acc[3] -= ry[u] * sz - rz[u] * sy;
+        acc[4] -= rz[u] * sx - rx[u] * sz;
+        acc[5] -= rx[u] * sy - ry[u] * sx;
+      }
+    }
+  }
+}
+
 template <int D, int G>
-__global__ void __launch_bounds__(128) reduce_forces_kernel(Geom g, int64_t P, const double *__restrict__ pos,
+__global__ void __launch_bounds__(128) reduce_forces_kernel(Geom g, int64_t P, double h_out,
+                                                            const double *__restrict__ pos,
                                                             const double *__restrict__ radius,
                                                             const int32_t *__restrict__ pid,
                                                             const double *__restrict__ s, double *__restrict__ force,
@@ -463,35 +542,11 @@ __global__ void __launch_bounds__(128) reduce_forces_kernel(Geom g, int64_t P, c
     bbox_axis(cx, R, g.nx, g.bcx, lo[0], ext[0]);
     bbox_axis(cy, R, g.ny, g.bcy, lo[1], ext[1]);
     if (D == 3) bbox_axis(cz, R, g.nz, g.bcz, lo[2], ext[2]);
-    const int nbox = ext[0] * ext[1] * ext[2];
-    for (int b = gl; b < nbox; b += G) {
-      const int bi = b % ext[0], t = b / ext[0];
-      const int bj = t % ext[1], bk = t / ext[1];
-      int i = lo[0] + bi, j = lo[1] + bj, k = lo[2] + bk;
-      if (!g.bcx) i = wrap_i(i, g.nx);
-      if (!g.bcy) j = wrap_i(j, g.ny);
-      if (D == 3 && !g.bcz) k = wrap_i(k, g.nz);
-      const int64_t x = ((int64_t)k * g.ny + j) * g.nx + i;
-      if (pid[x] != (int32_t)p) continue;
-      double rx = (double)i - cx, ry = (double)j - cy, rz = D == 3 ? (double)k - cz : 0.0;
-      if (!g.bcx) rx = min_image_d(rx, g.nx);
-      if (!g.bcy) ry = min_image_d(ry, g.ny);
-      if (D == 3 && !g.bcz) rz = min_image_d(rz, g.nz);
-      const double sx = s[x], sy = s[g.N + x];
-      if (D == 2) {
-        acc[0] -= sx;
-        acc[1] -= sy;
-        acc[2] -= rx * sy - ry * sx;
-      } else {
-        const double sz = s[2 * g.N + x];
-        acc[0] -= sx;
-        acc[1] -= sy;
-        acc[2] -= sz;
-        acc[3] -= ry * sz - rz * sy;
-        acc[4] -= rz * sx - rx * sz;
-        acc[5] -= rx * sy - ry * sx;
-      }
-    }
+    const double rout = R + h_out;
+    if (ext[0] <= 16)
+      reduce_gather<D, G, 16>(g, (int32_t)p, cx, cy, cz, rout * rout, lo, ext, gl, pid, s, acc);
+    else
+      reduce_gather<D, G, 32>(g, (int32_t)p, cx, cy, cz, rout * rout, lo, ext, gl, pid, s, acc);
   }
 #pragma unroll
   for (int v = 0; v < NV; ++v)
@@ -514,13 +569,20 @@ __global__ void __launch_bounds__(128) reduce_forces_kernel(Geom g, int64_t P, c
   }
 }
 
+// half extent of a node's sample cloud plus a safety margin: a node whose centre is farther than
+// R + h from a particle centre has no sample inside that particle
+static double sample_cloud_radius(const lbmimb_lattice *h) {
+  return sqrt((double)h->g.dim) * (0.5 - 0.5 / (double)h->prm.subsamples) + 1e-6;
+}
+
 lbmimb_status launch_reduce(lbmimb_lattice *h) {
+  const double ho = sample_cloud_radius(h);
   if (h->g.dim == 2)
-    reduce_forces_kernel<2, 32><<<blocks_for(h->P, 4), 128, 0, h->stream>>>(h->g, h->P, h->pos, h->radius, h->pid,
-                                                                           h->s, h->force, h->torque);
+    reduce_forces_kernel<2, 32><<<blocks_for(h->P, 4), 128, 0, h->stream>>>(h->g, h->P, ho, h->pos, h->radius,
+                                                                           h->pid, h->s, h->force, h->torque);
   else
-    reduce_forces_kernel<3, 128><<<blocks_for(h->P, 1), 128, 0, h->stream>>>(h->g, h->P, h->pos, h->radius, h->pid,
-                                                                            h->s, h->force, h->torque);
+    reduce_forces_kernel<3, 128><<<blocks_for(h->P, 1), 128, 0, h->stream>>>(h->g, h->P, ho, h->pos, h->radius,
+                                                                            h->pid, h->s, h->force, h->torque);
   LBMIMB_LAUNCH_CHECK(h, "reduce_forces_kernel");
   return LBMIMB_OK;
 }
