@@ -344,61 +344,111 @@ __device__ __forceinline__ void bbox_axis(double c, double R, int n, int bc, int
 
 // pass 2: nodes reached by more than one particle are recomputed from the definition:
 // union of the inside samples, covering particle = most samples, ties -> lowest index.
+// One warp per node.  The 3^D neighbour cells are read by one lane each, their particles are
+// gathered into a per-warp candidate list, the candidates are distance-tested one per lane,
+// and only the survivors are sampled (by the whole warp, lane l tests samples l, l+32, ...).
+constexpr int kContestedCand = 64;  // candidates staged per round
+
 template <int D>
 __global__ void __launch_bounds__(128) map_contested_kernel(const MapArgs a, const CellGeom cg,
                                                             const int32_t *__restrict__ start,
                                                             const int32_t *__restrict__ items) {
   __shared__ SampleTable tab;
+  __shared__ int32_t cand[4][kContestedCand];
   fill_sample_table(tab, a.S, a.SD, D);
   __syncthreads();
   int total = a.counters[0];
   if (total > a.contested_cap) total = (int)a.contested_cap;
   const int warps = (gridDim.x * blockDim.x) >> 5;
   const int wid = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int lane = threadIdx.x & 31;
+  const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
+  // this lane's neighbour-cell offset (lanes beyond the 3^D offsets idle)
+  const int lo0 = off_lo(cg.nc[0], cg.periodic[0]), n0 = off_hi(cg.nc[0], cg.periodic[0]) - lo0 + 1;
+  const int lo1 = off_lo(cg.nc[1], cg.periodic[1]), n1 = off_hi(cg.nc[1], cg.periodic[1]) - lo1 + 1;
+  const int lo2 = D == 3 ? off_lo(cg.nc[2], cg.periodic[2]) : 0;
+  const int n2 = D == 3 ? off_hi(cg.nc[2], cg.periodic[2]) - lo2 + 1 : 1;
+  const bool cell_lane = lane < n0 * n1 * n2;
+  const int ox = lo0 + lane % n0, oy = lo1 + (lane / n0) % n1, oz = lo2 + lane / (n0 * n1);
+  const double ro_h = a.h_out;
   for (int e = wid; e < total; e += warps) {
     const int64_t x = a.contested[e];
     const int i = (int)(x % a.g.nx);
     const int64_t r = x / a.g.nx;
     const int j = (int)(r % a.g.ny), k = (int)(r / a.g.ny);
-    const int ccx = cell_coord((double)i, cg, 0), ccy = cell_coord((double)j, cg, 1);
-    const int ccz = D == 3 ? cell_coord((double)k, cg, 2) : 0;
+    int b = 0, en = 0;
+    if (cell_lane) {
+      int cx_ = cell_coord((double)i, cg, 0) + ox, cy_ = cell_coord((double)j, cg, 1) + oy;
+      int cz_ = D == 3 ? cell_coord((double)k, cg, 2) + oz : 0;
+      bool ok = true;
+      if (cg.periodic[0]) cx_ = wrap_i(cx_, cg.nc[0]);
+      else ok = ok && cx_ >= 0 && cx_ < cg.nc[0];
+      if (cg.periodic[1]) cy_ = wrap_i(cy_, cg.nc[1]);
+      else ok = ok && cy_ >= 0 && cy_ < cg.nc[1];
+      if (D == 3) {
+        if (cg.periodic[2]) cz_ = wrap_i(cz_, cg.nc[2]);
+        else ok = ok && cz_ >= 0 && cz_ < cg.nc[2];
+      }
+      if (ok) {
+        const int c = (cz_ * cg.nc[1] + cy_) * cg.nc[0] + cx_;
+        b = __ldg(start + c);
+        en = __ldg(start + c + 1);
+      }
+    }
     unsigned ubits = 0;
     int best_cnt = 0, best_p = -1;
-    for (int oz = D == 3 ? off_lo(cg.nc[2], cg.periodic[2]) : 0; oz <= (D == 3 ? off_hi(cg.nc[2], cg.periodic[2]) : 0); ++oz)
-      for (int oy = off_lo(cg.nc[1], cg.periodic[1]); oy <= off_hi(cg.nc[1], cg.periodic[1]); ++oy)
-        for (int ox = off_lo(cg.nc[0], cg.periodic[0]); ox <= off_hi(cg.nc[0], cg.periodic[0]); ++ox) {
-          int nx_ = ccx + ox, ny_ = ccy + oy, nz_ = ccz + oz;
-          if (cg.periodic[0]) nx_ = wrap_i(nx_, cg.nc[0]);
-          else if (nx_ < 0 || nx_ >= cg.nc[0]) continue;
-          if (cg.periodic[1]) ny_ = wrap_i(ny_, cg.nc[1]);
-          else if (ny_ < 0 || ny_ >= cg.nc[1]) continue;
-          if (D == 3) {
-            if (cg.periodic[2]) nz_ = wrap_i(nz_, cg.nc[2]);
-            else if (nz_ < 0 || nz_ >= cg.nc[2]) continue;
-          }
-          const int c = (nz_ * cg.nc[1] + ny_) * cg.nc[0] + nx_;
-          for (int it = start[c]; it < start[c + 1]; ++it) {
-            const int p = items[it];
-            const double pcx = a.pos[p], pcy = a.pos[a.P + p], pcz = D == 3 ? a.pos[2 * a.P + p] : 0.0;
-            const double R = a.radius[p];
-            {  // cheap reject: no sample of this node can lie inside a particle that far away
-              double ex = (double)i - pcx, ey = (double)j - pcy, ez = D == 3 ? (double)k - pcz : 0.0;
-              if (!a.g.bcx) ex = min_image_d(ex, a.g.nx);
-              if (!a.g.bcy) ey = min_image_d(ey, a.g.ny);
-              if (D == 3 && !a.g.bcz) ez = min_image_d(ez, a.g.nz);
-              const double ro = R + a.h_out;
-              if (ex * ex + ey * ey + ez * ez > ro * ro) continue;
-            }
-            unsigned bits;
-            const int cnt = warp_count_samples<D>(a.g, a.SD, tab, i, j, k, pcx, pcy, pcz, __dmul_rn(R, R), bits);
-            ubits |= bits;
-            if (cnt > best_cnt || (cnt == best_cnt && cnt > 0 && p < best_p)) {
-              best_cnt = cnt;
-              best_p = p;
-            }
+    // rounds of at most kContestedCand candidates (one round unless cells are crowded)
+    while (__any_sync(0xffffffffu, b < en)) {
+      int mine = en - b;
+      int incl = mine;
+      for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+      }
+      int excl = incl - mine;
+      int take = mine;
+      if (excl >= kContestedCand) take = 0;
+      else if (excl + take > kContestedCand) take = kContestedCand - excl;
+      for (int m = 0; m < take; ++m) cand[wl][excl + m] = __ldg(items + b + m);
+      b += take;
+      int T = __shfl_sync(0xffffffffu, incl, 31);
+      if (T > kContestedCand) T = kContestedCand;
+      __syncwarp();
+      for (int t0 = 0; t0 < T; t0 += 32) {
+        // one candidate per lane: cheap reject (no sample of this node can lie inside a particle that far away)
+        int p = -1;
+        double pcx = 0.0, pcy = 0.0, pcz = 0.0, R = 0.0;
+        bool near = false;
+        if (t0 + lane < T) {
+          p = cand[wl][t0 + lane];
+          pcx = a.pos[p];
+          pcy = a.pos[a.P + p];
+          pcz = D == 3 ? a.pos[2 * a.P + p] : 0.0;
+          R = a.radius[p];
+          double ex = (double)i - pcx, ey = (double)j - pcy, ez = D == 3 ? (double)k - pcz : 0.0;
+          if (!a.g.bcx) ex = min_image_d(ex, a.g.nx);
+          if (!a.g.bcy) ey = min_image_d(ey, a.g.ny);
+          if (D == 3 && !a.g.bcz) ez = min_image_d(ez, a.g.nz);
+          const double ro = R + ro_h;
+          near = ex * ex + ey * ey + ez * ez <= ro * ro;
+        }
+        unsigned live = __ballot_sync(0xffffffffu, near);
+        while (live) {
+          const int src = __ffs(live) - 1;
+          live &= live - 1;
+          const int sp = __shfl_sync(0xffffffffu, p, src);
+          const double sx = __shfl_sync(0xffffffffu, pcx, src), sy = __shfl_sync(0xffffffffu, pcy, src);
+          const double sz = __shfl_sync(0xffffffffu, pcz, src), sR = __shfl_sync(0xffffffffu, R, src);
+          unsigned bits;
+          const int cnt = warp_count_samples<D>(a.g, a.SD, tab, i, j, k, sx, sy, sz, __dmul_rn(sR, sR), bits);
+          ubits |= bits;
+          if (cnt > best_cnt || (cnt == best_cnt && cnt > 0 && sp < best_p)) {
+            best_cnt = cnt;
+            best_p = sp;
           }
         }
+      }
+      __syncwarp();
+    }
     int ucnt = 0;
     for (int m = 0; m * 32 < a.SD; ++m) ucnt += __popc(__ballot_sync(0xffffffffu, (ubits >> m) & 1u));
     if (lane == 0) {
@@ -456,14 +506,17 @@ lbmimb_status launch_map(lbmimb_lattice *h) {
 // ---------------------------------------------------------------------------
 template <int D, int G, int W>
 __device__ __forceinline__ void reduce_gather(const Geom &g, int32_t p, double cx, double cy, double cz, double rout2,
-                                              const int (&lo)[3], const int (&ext)[3], int gl,
-                                              const int32_t *__restrict__ pid, const double *__restrict__ s,
+                                              const int (&lo)[3], const int (&ext)[3], bool wx, bool wy, bool wz,
+                                              int gl, const int32_t *__restrict__ pid, const double *__restrict__ s,
                                               double *acc) {
   constexpr int U = 4;
   constexpr int RPI = G / W;  // row slots per iteration of the group
   const int bi0 = gl % W, rs = gl / W;
   const int nchunks = (ext[0] + W - 1) / W;
   const int nslots = ext[1] * ext[2] * nchunks;
+  const float inv_nch = 1.0f / (float)nchunks, inv_e1 = 1.0f / (float)ext[1];
+  // a bounding box reaches at most one period beyond either end of a periodic axis
+  auto wrap1 = [](int v, int n) { return v < 0 ? v + n : (v >= n ? v - n : v); };
   for (int s0 = rs; s0 < nslots; s0 += U * RPI) {
     bool cand[U];
     int32_t owner[U];
@@ -474,21 +527,22 @@ __device__ __forceinline__ void reduce_gather(const Geom &g, int32_t p, double c
       const int slot = s0 + u * RPI;
       int row = slot, bi = bi0;
       if (nchunks > 1) {
-        row = slot / nchunks;
-        bi += (slot - row * nchunks) * W;
+        int ch;
+        fast_divmod(slot, nchunks, inv_nch, row, ch);
+        bi += ch * W;
       }
-      const int bk = D == 3 ? row / ext[1] : 0;
-      const int bj = row - bk * ext[1];
+      int bk = 0, bj = row;
+      if (D == 3) fast_divmod(row, ext[1], inv_e1, bk, bj);
       int i = lo[0] + bi, j = lo[1] + bj, k = lo[2] + bk;
-      if (!g.bcx) i = wrap_i(i, g.nx);
-      if (!g.bcy) j = wrap_i(j, g.ny);
-      if (D == 3 && !g.bcz) k = wrap_i(k, g.nz);
+      if (wx) i = wrap1(i, g.nx);
+      if (wy) j = wrap1(j, g.ny);
+      if (D == 3 && wz) k = wrap1(k, g.nz);
       rx[u] = (double)i - cx;
       ry[u] = (double)j - cy;
       rz[u] = D == 3 ? (double)k - cz : 0.0;
-      if (!g.bcx) rx[u] = min_image_d(rx[u], g.nx);
-      if (!g.bcy) ry[u] = min_image_d(ry[u], g.ny);
-      if (D == 3 && !g.bcz) rz[u] = min_image_d(rz[u], g.nz);
+      if (wx) rx[u] = min_image_d(rx[u], g.nx);
+      if (wy) ry[u] = min_image_d(ry[u], g.ny);
+      if (D == 3 && wz) rz[u] = min_image_d(rz[u], g.nz);
       cand[u] = slot < nslots && bi < ext[0] && rx[u] * rx[u] + ry[u] * ry[u] + rz[u] * rz[u] <= rout2;
       owner[u] = -1;
       s01[u] = s23[u] = make_double2(0.0, 0.0);
@@ -543,10 +597,12 @@ __global__ void __launch_bounds__(128) reduce_forces_kernel(Geom g, int64_t P, d
     bbox_axis(cy, R, g.ny, g.bcy, lo[1], ext[1]);
     if (D == 3) bbox_axis(cz, R, g.nz, g.bcz, lo[2], ext[2]);
     const double rout = R + h_out;
+    const bool wx = crosses_seam(cx, R, g.nx, g.bcx), wy = crosses_seam(cy, R, g.ny, g.bcy);
+    const bool wz = D == 3 && crosses_seam(cz, R, g.nz, g.bcz);
     if (ext[0] <= 16)
-      reduce_gather<D, G, 16>(g, (int32_t)p, cx, cy, cz, rout * rout, lo, ext, gl, pid, s, acc);
+      reduce_gather<D, G, 16>(g, (int32_t)p, cx, cy, cz, rout * rout, lo, ext, wx, wy, wz, gl, pid, s, acc);
     else
-      reduce_gather<D, G, 32>(g, (int32_t)p, cx, cy, cz, rout * rout, lo, ext, gl, pid, s, acc);
+      reduce_gather<D, G, 32>(g, (int32_t)p, cx, cy, cz, rout * rout, lo, ext, wx, wy, wz, gl, pid, s, acc);
   }
 #pragma unroll
   for (int v = 0; v < NV; ++v)
