@@ -38,7 +38,7 @@ constexpr int kStepThreads = 128;
 // x indices i-1, i, i+1 (wrapped) differ.  A warp takes the IMB path as a whole when
 // any of its nodes is covered (beta = 0 on the others), else the cheaper LBGK path.
 // ---------------------------------------------------------------------------
-template <int D, bool IMB, bool EMIT, int MINB>
+template <int D, bool IMB, bool EMIT, int MINB, bool EARLY = false>
 __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(const StepArgs a) {
   using L = Lat<D>;
   constexpr int Q = L::Q;
@@ -53,6 +53,14 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
   const int64_t x = rowoff + i;
   const int im = i == 0 ? a.nx - 1 : i - 1;
   const int ip = i == a.nx - 1 ? 0 : i + 1;
+
+  // EARLY: the node tag (sample count, covering particle) is requested before the populations
+  // so that the dependent gather of the particle record overlaps the population loads.
+  int cnt = 0, pe = 0;
+  if (IMB && EARLY) {
+    cnt = a.eps_cnt[x];
+    pe = a.pid[x];
+  }
 
   // ---- gather (streaming) ----
   double f[Q];
@@ -83,8 +91,13 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
     }
   }
 
-  int cnt = 0;
-  if (IMB) cnt = a.eps_cnt[x];
+  if (IMB && !EARLY) cnt = a.eps_cnt[x];
+  double beta = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
+  if (IMB && EARLY && cnt > 0) {
+    beta = __ldg(a.beta_tab + cnt);
+    solid_velocity<D>(a.prec + (int64_t)pe * prec_stride(D), i, j, k, a.nx, a.ny, a.nz, a.bcx, a.bcy, a.bcz, vx, vy,
+                      vz);
+  }
 
   double rho, ux, uy, uz;
   moments<D>(f, rho, ux, uy, uz);
@@ -92,8 +105,7 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
   if (!IMB || !__any_sync(0xffffffffu, cnt > 0)) {
     collide_fluid<D>(f, a.cp, rho, ux, uy, uz);
   } else {
-    double beta = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
-    if (cnt > 0) {
+    if (!EARLY && cnt > 0) {
       const int p = a.pid[x];
       beta = __ldg(a.beta_tab + cnt);
       solid_velocity<D>(a.prec + (int64_t)p * prec_stride(D), i, j, k, a.nx, a.ny, a.nz, a.bcx, a.bcy, a.bcz, vx, vy,
@@ -261,14 +273,14 @@ lbmimb_status launch_init_rest(lbmimb_lattice *h) {
   return LBMIMB_OK;
 }
 
-template <int D, int MINB>
+template <int D, int MINB, bool EARLY = false>
 static void launch_cs2(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, bool imb, bool emit) {
   if (!imb)
     collide_stream_kernel<D, false, false, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
   else if (!emit)
-    collide_stream_kernel<D, true, false, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
+    collide_stream_kernel<D, true, false, MINB, EARLY><<<blocks, kStepThreads, 0, h->stream>>>(a);
   else
-    collide_stream_kernel<D, true, true, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
+    collide_stream_kernel<D, true, true, MINB, EARLY><<<blocks, kStepThreads, 0, h->stream>>>(a);
 }
 
 // Experiment switch (environment LBMIMB_STEP_VARIANT): 0-9 plain kernel with different
@@ -284,12 +296,15 @@ int step_variant() {
 
 template <int D>
 static void launch_cs(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, bool imb, bool emit) {
-  if (D == 3) {
+  if constexpr (D == 3) {
     switch (step_variant()) {
       case 1: launch_cs2<D, 5>(h, a, blocks, imb, emit); break;
       case 2: launch_cs2<D, 6>(h, a, blocks, imb, emit); break;
       case 3: launch_cs2<D, 8>(h, a, blocks, imb, emit); break;
-      default: launch_cs2<D, 7>(h, a, blocks, imb, emit); break;
+      case 4: launch_cs2<D, 7>(h, a, blocks, imb, emit); break;
+      case 5: launch_cs2<D, 7, true>(h, a, blocks, imb, emit); break;
+      case 7: launch_cs2<D, 5, true>(h, a, blocks, imb, emit); break;
+      default: launch_cs2<D, 6, true>(h, a, blocks, imb, emit); break;
     }
   } else {
     switch (step_variant()) {
@@ -297,7 +312,10 @@ static void launch_cs(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, boo
       case 2: launch_cs2<D, 10>(h, a, blocks, imb, emit); break;
       case 3: launch_cs2<D, 12>(h, a, blocks, imb, emit); break;
       case 4: launch_cs2<D, 16>(h, a, blocks, imb, emit); break;
-      default: launch_cs2<D, 9>(h, a, blocks, imb, emit); break;
+      case 5: launch_cs2<D, 9>(h, a, blocks, imb, emit); break;
+      case 6: launch_cs2<D, 8, true>(h, a, blocks, imb, emit); break;
+      case 7: launch_cs2<D, 10, true>(h, a, blocks, imb, emit); break;
+      default: launch_cs2<D, 9, true>(h, a, blocks, imb, emit); break;
     }
   }
 }

@@ -108,11 +108,20 @@ __device__ __forceinline__ bool crosses_seam(double c, double R, int n, int bc) 
   return l < 0 || h > n - 1;
 }
 
+// Group barrier: a warp (or part of one) synchronises with __syncwarp, larger groups with the block barrier
+// (all groups of a block run the same number of chunk iterations: the count is the block maximum).
+template <int G>
+__device__ __forceinline__ void group_sync() {
+  if (G <= 32) __syncwarp();
+  else __syncthreads();
+}
+
 template <int D, int G, int SFIX>
 __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
   constexpr int groups = 128 / G;
+  constexpr int CH = G >= 64 ? kMapChunk : 8 * G;   // bounding-box nodes per pass of a group
   __shared__ double sub[256];
-  __shared__ int list[groups][kMapChunk];
+  __shared__ int list[groups][CH];
   __shared__ int nlist[groups];
   __shared__ int smax;
   for (int t = threadIdx.x; t < a.S; t += blockDim.x) sub[t] = sub_offset(t, a.S);
@@ -140,8 +149,11 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
   const bool fast = nbox < (1 << 24);
   const float inv0 = 1.0f / (float)ext[0], inv1 = 1.0f / (float)ext[1];
   const double R2 = __dmul_rn(R, R);
-  const double rin = R - a.h_in, rout = R + a.h_out;
-  const double rin2 = rin > 0.0 ? rin * rin : -1.0, rout2 = rout * rout;
+  // Classification of a node by the box [|d| - hs, |d| + hs] per axis that holds its sample cloud
+  // (hs = 1/2 - 1/(2S)): its farthest corner inside the particle => every sample is inside, its nearest
+  // point outside => none is.  The margin (relative 1e-9) dwarfs the rounding of either test.
+  const double hs = a.hs;
+  const double r2_full = R2 - 1e-9 * (R2 + 1.0), r2_none = R2 + 1e-9 * (R2 + 1.0);
   __syncthreads();
   atomicMax(&smax, nbox);
   __syncthreads();
@@ -165,37 +177,50 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
     if (wy) j = wrap_i(j, a.g.ny);
     if (D == 3 && wz) k = wrap_i(k, a.g.nz);
   };
-  auto commit = [&](int i, int j, int k, int cnt) {
-    const int64_t x = ((int64_t)k * a.g.ny + j) * a.g.nx + i;
-    const int32_t old = atomicExch(a.pid + x, (int32_t)p);
-    a.eps_cnt[x] = (uint8_t)cnt;
-    if (old != -1 && old != (int32_t)p) {
+  // The exchange on pid tells whether another particle reached the node first.  Its result is looked at
+  // one commit later (or at the end), so that the round trip of the atomic is off the critical path.
+  int64_t pend_x = -1;
+  int32_t pend_old = -1;
+  auto settle = [&]() {
+    if (pend_x >= 0 && pend_old != -1 && pend_old != (int32_t)p) {
       const int slot = atomicAdd(a.counters, 1);
-      if (slot < a.contested_cap) a.contested[slot] = x;
+      if (slot < a.contested_cap) a.contested[slot] = pend_x;
       else a.counters[1] = 1;
     }
+    pend_x = -1;
+  };
+  auto commit = [&](int i, int j, int k, int cnt) {
+    const int64_t x = ((int64_t)k * a.g.ny + j) * a.g.nx + i;
+    settle();
+    pend_old = atomicExch(a.pid + x, (int32_t)p);
+    pend_x = x;
+    a.eps_cnt[x] = (uint8_t)cnt;
   };
 
-  for (int base = 0; base < maxbox; base += kMapChunk) {
+  for (int base = 0; base < maxbox; base += CH) {
     if (gl == 0) nlist[grp] = 0;
-    __syncthreads();
-    // phase A: classify nodes by the distance of the node centre
-    for (int b = base + gl; b < nbox && b < base + kMapChunk; b += G) {
+    group_sync<G>();
+    // phase A: classify nodes
+    for (int b = base + gl; b < nbox && b < base + CH; b += G) {
       int i, j, k;
       node_of(b, i, j, k);
       double dx = (double)i - cx, dy = (double)j - cy, dz = D == 3 ? (double)k - cz : 0.0;
       if (wx) dx = min_image_d(dx, a.g.nx);
       if (wy) dy = min_image_d(dy, a.g.ny);
       if (D == 3 && wz) dz = min_image_d(dz, a.g.nz);
-      const double d2 = dx * dx + dy * dy + dz * dz;
-      if (d2 <= rin2) {
-        commit(i, j, k, a.SD);          // every sample is inside (triangle inequality + margin)
-      } else if (d2 <= rout2) {
+      dx = fabs(dx);
+      dy = fabs(dy);
+      dz = fabs(dz);
+      const double fx = dx + hs, fy = dy + hs, fz = D == 3 ? dz + hs : 0.0;
+      const double nx_ = fmax(dx - hs, 0.0), ny_ = fmax(dy - hs, 0.0), nz_ = D == 3 ? fmax(dz - hs, 0.0) : 0.0;
+      if (fx * fx + fy * fy + fz * fz <= r2_full) {
+        commit(i, j, k, a.SD);
+      } else if (nx_ * nx_ + ny_ * ny_ + nz_ * nz_ <= r2_none) {
         const int slot = atomicAdd(&nlist[grp], 1);
         list[grp][slot] = b;            // boundary cell: sample it
       }
     }
-    __syncthreads();
+    group_sync<G>();
     // phase B: one thread per boundary cell
     const int nl = nlist[grp];
     for (int e = gl; e < nl; e += G) {
@@ -206,7 +231,8 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
       else cnt = thread_count_generic<D>(a.g, a.S, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
       if (cnt > 0) commit(i, j, k, cnt);
     }
-    __syncthreads();
+    group_sync<G>();
   }
+  settle();
 }
 

@@ -268,7 +268,8 @@ struct MapArgs {
   int64_t *contested;
   int64_t contested_cap;
   int32_t *counters;
-  double h_in, h_out;  // half extent of the sample cloud -/+ safety margin
+  double h_in, h_out;  // radius of a node's sample cloud + safety margin
+  double hs;           // half edge of the sample cloud, 1/2 - 1/(2S)
 };
 
 __device__ __forceinline__ double sub_offset(int a, int S) {
@@ -479,8 +480,13 @@ lbmimb_status launch_map(lbmimb_lattice *h) {
   const double hs = sqrt((double)h->g.dim) * (0.5 - 0.5 / (double)a.S);
   a.h_in = hs + 1e-6;
   a.h_out = hs + 1e-6;
+  a.hs = 0.5 - 0.5 / (double)a.S;
+  // threads per particle: enough lanes for the boundary shell without leaving most of them idle
+  const double edge = 2.0 * h->rmax + 3.0;
   if (h->g.dim == 2) {
-    if (a.S == 8) map_particles_kernel<2, 32, 8><<<blocks_for(h->P, 4), 128, 0, h->stream>>>(a);
+    const bool small = edge * edge <= 256.0;
+    if (a.S == 8 && small) map_particles_kernel<2, 16, 8><<<blocks_for(h->P, 8), 128, 0, h->stream>>>(a);
+    else if (a.S == 8) map_particles_kernel<2, 32, 8><<<blocks_for(h->P, 4), 128, 0, h->stream>>>(a);
     else map_particles_kernel<2, 32, 0><<<blocks_for(h->P, 4), 128, 0, h->stream>>>(a);
   } else {
     if (a.S == 4) map_particles_kernel<3, 128, 4><<<blocks_for(h->P, 1), 128, 0, h->stream>>>(a);
