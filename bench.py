@@ -38,7 +38,7 @@ UNIT = "MLUPS"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused kernel from the committed
 # `ncu --set full` capture (profiles/r1_traffic.md); None where no capture exists for the workload.
-NCU_TRAFFIC_BYTES = {"C3": 21427389000}
+NCU_TRAFFIC_BYTES = {"C3": 20849638000, "C4": 41870191000}
 
 
 def measured_peak_gbs():
@@ -60,6 +60,13 @@ class ClockSampler:
         self.index = index
         self.rows = []
         self.proc = None
+        self.t0 = self.t1 = None
+
+    def mark_begin(self):
+        self.t0 = time.time()
+
+    def mark_end(self):
+        self.t1 = time.time()
 
     def start(self):
         try:
@@ -75,7 +82,7 @@ class ClockSampler:
         for line in self.proc.stdout:
             parts = [p.strip() for p in line.split(",")]
             if len(parts) >= 7:
-                self.rows.append(parts)
+                self.rows.append((time.time(), parts))
 
     def stop(self):
         if self.proc is None:
@@ -87,7 +94,10 @@ class ClockSampler:
         except Exception:
             self.proc.kill()
         sm, mx, reasons = [], [], set()
-        for r in self.rows:
+        inside = [r for (t, r) in self.rows if self.t0 is None or (self.t0 <= t <= (self.t1 or t) + 0.1)]
+        if not inside:          # region shorter than one sampling period: the sample nearest to it
+            inside = [r for (t, r) in self.rows[-1:]]
+        for r in inside:
             try:
                 sm.append(float(r[0]))
                 mx.append(float(r[1]))
@@ -174,8 +184,8 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--workload", default="C3", choices=["C2", "C3", "C4", "C5"])
     ap.add_argument("--impl", default="lbmimb", choices=["lbmimb", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -206,17 +216,18 @@ def main():
         if dem:
             lat.dem_step(dem["kn"], dem["restitution"], dem["g_particle"], dem["dt"])
 
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()          # nvidia-smi needs a few hundred ms to deliver its first sample
     for _ in range(args.warmup):
         whole_step()
     lat.synchronize()
 
     # ---- timed region: device-resident inputs -------------------------------------------------
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(args.steps)]
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
     replicas.barrier()
     torch.cuda.synchronize()
+    sampler.mark_begin()
     launches0 = lat.launch_count()
     for k in range(args.steps):
         ev[k][0].record()
@@ -230,6 +241,7 @@ def main():
             lat.dem_step(dem["kn"], dem["restitution"], dem["g_particle"], dem["dt"])
         ev[k][4].record()
     torch.cuda.synchronize()
+    sampler.mark_end()
     replicas.barrier()
     launches = lat.launch_count() - launches0
     clocks = sampler.stop() if rank == 0 else None
