@@ -30,6 +30,8 @@ def lib():
         _lib.orc_damping.restype = C.c_double
         _lib.orc_damping.argtypes = [C.c_double] * 3
         _lib.orc_map.restype = C.c_int
+        _lib.orc_eps_table.restype = C.c_int
+        _lib.orc_map_table.restype = C.c_int
         _lib.orc_dem_step.restype = C.c_int
         _lib.orc_num_threads.restype = C.c_int
     return _lib
@@ -136,10 +138,54 @@ def map_particles(dim, n, bc, S, pos, radius):
     return eps, pid
 
 
+# discretisation of the eps table (R17): (Nd, Nt, St) per dimension; part of the ABI text
+TABLE_DIMS = {2: (128, 32, 256), 3: (128, 16, 64)}
+TABLE_DEN = 255
+
+
+_tables = {}
+
+
+def eps_table(dim, R, dims=None):
+    """The paper's pre-calculated table gamma = phi(d, theta) as uint8 codes,
+    shape [Nd, Nt] (2D) or [Nd, Nt, Nt] (3D); gamma = code / 255.  Computed once per (dim, R, dims)."""
+    Nd, Nt, St = dims or TABLE_DIMS[dim]
+    key = (dim, float(R), Nd, Nt, St)
+    if key not in _tables:
+        tab = np.zeros((Nd, Nt) if dim == 2 else (Nd, Nt, Nt), dtype=np.uint8)
+        rc = lib().orc_eps_table(C.c_int(dim), C.c_double(R), C.c_int(Nd), C.c_int(Nt), C.c_int(St), _p(tab))
+        if rc != 0:
+            raise RuntimeError("orc_eps_table failed (R < 1 or bad sizes)")
+        tab.setflags(write=False)
+        _tables[key] = tab
+    return _tables[key]
+
+
+def map_particles_table(dim, n, bc, pos, radius, dims=None):
+    """Table-mode map -> eps_code uint8[nz,ny,nx] (eps = code/255), pid int32[nz,ny,nx]."""
+    Nd, Nt, St = dims or TABLE_DIMS[dim]
+    n3, bc3 = _n3(n), _bc3(bc)
+    pos = _f64(pos).reshape(dim, -1)
+    radius = _f64(radius)
+    P = pos.shape[1]
+    shp = (int(n3[2]), int(n3[1]), int(n3[0]))
+    eps = np.zeros(shp, dtype=np.uint8)
+    pid = np.empty(shp, dtype=np.int32)
+    tab = eps_table(dim, radius[0], (Nd, Nt, St)) if P else np.zeros(1, dtype=np.uint8)
+    rc = lib().orc_map_table(C.c_int(dim), _p(n3), _p(bc3), C.c_int(Nd), C.c_int(Nt), _p(tab),
+                             C.c_int64(P), _p(pos), _p(radius), _p(eps), _p(pid))
+    if rc != 0:
+        raise RuntimeError("orc_map_table failed (%d: -2 = radii differ)" % rc)
+    return eps, pid
+
+
 def step(dim, n, bc, tau, g, S, f, eps_cnt=None, pid=None, pos=None, vel=None,
-         omega=None, want_s=False):
-    """One step of eq. (1): returns f(t+1) (and s[dim,nz,ny,nx] if want_s)."""
+         omega=None, want_s=False, eps_den=None):
+    """One step of eq. (1): returns f(t+1) (and s[dim,nz,ny,nx] if want_s).
+    eps = eps_cnt / eps_den, eps_den = S^dim unless given (255 for the table map)."""
     n3, bc3, g3 = _n3(n), _bc3(bc), _g3(g)
+    if eps_den is None:
+        eps_den = S ** dim
     f = _f64(f)
     out = np.empty_like(f)
     shp = f.shape[1:]
@@ -156,7 +202,7 @@ def step(dim, n, bc, tau, g, S, f, eps_cnt=None, pid=None, pos=None, vel=None,
         pid = np.ascontiguousarray(pid, dtype=np.int32)
         args = [_p(eps_cnt), _p(pid), _p(pos), _p(vel), _p(omega)]
     lib().orc_step(C.c_int(dim), _p(n3), _p(bc3), C.c_double(tau), _p(g3),
-                   C.c_int(S), _p(f), _p(out), args[0], args[1], C.c_int64(P),
+                   C.c_int(eps_den), _p(f), _p(out), args[0], args[1], C.c_int64(P),
                    args[2], args[3], args[4], _p(s) if want_s else None)
     return (out, s) if want_s else out
 

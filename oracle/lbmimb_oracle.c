@@ -271,6 +271,171 @@ int orc_map(int dim, const int64_t *n, const int32_t *bc, int S, int64_t P,
   return 0;
 }
 
+/* ------------------------------------------------------------------------ */
+/* NEXT-1: the paper's own eps method, table look-up gamma = phi(d, theta)    */
+/* (eq. (6); Fig. 1 is missing, so the discretisation is the  */
+/* reading R17 of DESIGN.md).  "For a lattice and a solid particle with a     */
+/* given radius, gamma can be determined by two factors: the distance between */
+/* the lattice and the origin of the solid particle d, and the orientation of */
+/* the lattice to the solid particle theta"; gamma "is pre-calculated".       */
+/*                                                                            */
+/* R17.  w = sqrt(D)/2 (half diagonal of a cell), d0 = R - w, dd = sqrt(D)/Nd.*/
+/* The orientation is kept as the ratios of the sorted absolute components of */
+/* the displacement, a >= b >= c: t1 = b/a (= tan theta in 2D), t2 = c/a, so  */
+/* that no transcendental function enters an index.  Entry (k, m1[, m2]):     */
+/*   d_k = d0 + (k + 1/2) dd,  t1 = (m1 + 1/2)/Nt,  t2 = (m2 + 1/2)/Nt,       */
+/*   r = d_k (1, t1, t2)/sqrt(1 + t1^2 + t2^2)  (cell centre relative to the  */
+/*   particle centre), n = number of the St^D sub-cell points of that cell    */
+/*   inside the particle (same point set and inside test as R4),              */
+/*   code = (255 n + St^D/2) / St^D  (integer; gamma = code/255).             */
+/* Returns 0, -1 on bad arguments (R < 1, sizes).                             */
+/* ------------------------------------------------------------------------ */
+int orc_eps_table(int dim, double R, int Nd, int Nt, int St,
+                  uint8_t *table /*[Nd][Nt] (2D) or [Nd][Nt][Nt] (3D)*/) {
+  if (!(R >= 1.0) || Nd < 1 || Nt < 1 || St < 1 || (dim != 2 && dim != 3))
+    return -1;
+  double sqD = sqrt((double)dim);
+  double d0 = R - 0.5 * sqD;
+  double dd = sqD / (double)Nd;
+  int64_t total = dim == 2 ? (int64_t)St * St : (int64_t)St * St * St;
+  int Nt2 = dim == 3 ? Nt : 1;
+#pragma omp parallel for
+  for (int k = 0; k < Nd; ++k)
+    for (int m1 = 0; m1 < Nt; ++m1)
+      for (int m2 = 0; m2 < Nt2; ++m2) {
+        double dk = d0 + ((double)k + 0.5) * dd;
+        double t1 = ((double)m1 + 0.5) / (double)Nt;
+        double t2 = dim == 3 ? ((double)m2 + 0.5) / (double)Nt : 0.0;
+        double nrm = dim == 3 ? sqrt((1.0 + t1 * t1) + t2 * t2) : sqrt(1.0 + t1 * t1);
+        double rx = dk / nrm;
+        double ry = rx * t1;
+        double rz = rx * t2;
+        int64_t n = 0;
+        int Sz = dim == 3 ? St : 1;
+        for (int az = 0; az < Sz; ++az)
+          for (int ay = 0; ay < St; ++ay)
+            for (int ax = 0; ax < St; ++ax) {
+              double px = rx + (((double)ax + 0.5) / (double)St - 0.5);
+              double py = ry + (((double)ay + 0.5) / (double)St - 0.5);
+              double d2 = px * px + py * py;
+              if (dim == 3) {
+                double pz = rz + (((double)az + 0.5) / (double)St - 0.5);
+                d2 = d2 + pz * pz;
+              }
+              if (d2 <= R * R) ++n;
+            }
+        table[((int64_t)k * Nt + m1) * Nt2 + m2] =
+            (uint8_t)((255 * n + total / 2) / total);
+      }
+  return 0;
+}
+
+/* Look-up of one node: displacement delta = x_node - c (already reduced by
+ * minimum image).  d = sqrt(dx*dx + dy*dy (+ dz*dz)) left to right;
+ * d < d0 -> 255; k = (int)((d - d0) * (Nd / sqrt(D))), k >= Nd -> 0;
+ * m = min((int)(t * Nt), Nt - 1) with t1 = b/a, t2 = c/a of the sorted
+ * absolute components a >= b >= c. */
+static int table_lookup(int dim, double R, int Nd, int Nt, const uint8_t *table,
+                        const double *delta) {
+  double sqD = sqrt((double)dim);
+  double d0 = R - 0.5 * sqD;
+  double inv_dd = (double)Nd / sqD;
+  double d2 = delta[0] * delta[0] + delta[1] * delta[1];
+  if (dim == 3) d2 = d2 + delta[2] * delta[2];
+  double d = sqrt(d2);
+  if (d < d0) return 255;
+  double u = (d - d0) * inv_dd;
+  if (u >= (double)Nd) return 0;
+  int k = (int)u;
+  double a = fabs(delta[0]), b = fabs(delta[1]), c = dim == 3 ? fabs(delta[2]) : 0.0;
+  double t;
+  if (a < b) { t = a; a = b; b = t; }
+  if (dim == 3) {
+    if (b < c) { t = b; b = c; c = t; }
+    if (a < b) { t = a; a = b; b = t; }
+  }
+  int m1 = (int)((b / a) * (double)Nt);
+  if (m1 > Nt - 1) m1 = Nt - 1;
+  int m2 = 0, Nt2 = 1;
+  if (dim == 3) {
+    Nt2 = Nt;
+    m2 = (int)((c / a) * (double)Nt);
+    if (m2 > Nt - 1) m2 = Nt - 1;
+  }
+  return table[((int64_t)k * Nt + m1) * Nt2 + m2];
+}
+
+/*
+ * a1 in table mode: for every particle, every node of its bounding box (same
+ * box as orc_map), code_p = look-up of the node's displacement.  Node result:
+ * eps_code = min(255, sum_p code_p) (non-overlapping particles cover disjoint
+ * parts of a cell, so their fractions add), pid = particle with the largest
+ * code, ties -> lowest index (R5), -1 if the sum is 0.  All particles must
+ * have the same radius ("a solid particle with a given radius").
+ * Returns 0, -1 bad arguments / out of memory, -2 radii differ.
+ */
+int orc_map_table(int dim, const int64_t *n, const int32_t *bc, int Nd, int Nt,
+                  const uint8_t *table /* orc_eps_table(dim, radius[0], Nd, Nt, .) */,
+                  int64_t P, const double *pos, const double *radius,
+                  uint8_t *eps_code /*[N]*/, int32_t *pid /*[N]*/) {
+  int64_t nx = n[0], ny = n[1], nz = dim == 3 ? n[2] : 1;
+  int64_t N = nx * ny * nz;
+  for (int64_t x = 0; x < N; ++x) {
+    eps_code[x] = 0;
+    pid[x] = -1;
+  }
+  if (P == 0) return 0;
+  double R = radius[0];
+  for (int64_t p = 1; p < P; ++p)
+    if (radius[p] != R) return -2;
+  uint8_t *best = (uint8_t *)calloc((size_t)N, 1);
+  int32_t *sum = (int32_t *)calloc((size_t)N, sizeof(int32_t));
+  if (!best || !sum || !(R >= 1.0)) {
+    free(best);
+    free(sum);
+    return -1;
+  }
+  for (int64_t p = 0; p < P; ++p) {
+    double c[3] = {pos[p], pos[P + p], dim == 3 ? pos[2 * P + p] : 0.0};
+    int64_t lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
+    for (int a = 0; a < dim; ++a) {
+      lo[a] = (int64_t)floor(c[a] - R) - 1;
+      hi[a] = (int64_t)ceil(c[a] + R) + 1;
+      if (bc[a] != 0) {
+        if (lo[a] < 0) lo[a] = 0;
+        if (hi[a] > n[a] - 1) hi[a] = n[a] - 1;
+      } else if (hi[a] - lo[a] + 1 > n[a]) { /* box wider than the axis: every node once */
+        lo[a] = 0;
+        hi[a] = n[a] - 1;
+      }
+    }
+    for (int64_t kk = lo[2]; kk <= hi[2]; ++kk)
+      for (int64_t jj = lo[1]; jj <= hi[1]; ++jj)
+        for (int64_t ii = lo[0]; ii <= hi[0]; ++ii) {
+          int64_t i = bc[0] == 0 ? wrap(ii, nx) : ii;
+          int64_t j = bc[1] == 0 ? wrap(jj, ny) : jj;
+          int64_t k = dim == 3 ? (bc[2] == 0 ? wrap(kk, nz) : kk) : 0;
+          int64_t node = (k * ny + j) * nx + i;
+          double delta[3] = {(double)i - c[0], (double)j - c[1],
+                             dim == 3 ? (double)k - c[2] : 0.0};
+          for (int a = 0; a < dim; ++a)
+            if (bc[a] == 0) delta[a] = min_image(delta[a], n[a]);
+          int code = table_lookup(dim, R, Nd, Nt, table, delta);
+          if (code > 0) {
+            sum[node] += code;
+            if (code > best[node]) { /* strict: ties keep the lower index */
+              best[node] = (uint8_t)code;
+              pid[node] = (int32_t)p;
+            }
+          }
+        }
+  }
+  for (int64_t x = 0; x < N; ++x) eps_code[x] = (uint8_t)(sum[x] > 255 ? 255 : sum[x]);
+  free(best);
+  free(sum);
+  return 0;
+}
+
 /*
  * a2: one time step of eq. (1) on the whole lattice, f_in (time t) ->
  * f_out (time t+1).  Collision per node (orc_collide_node), then streaming:
@@ -278,17 +443,19 @@ int orc_map(int dim, const int64_t *n, const int32_t *bc, int S, int64_t P,
  * wall axis, half-way bounce-back: f_out[x][-i] = f*_i(x) (R15), else
  * f_out[y][i] = f*_i(x).  On eps>0 nodes V_S = v_p + omega_p x (x - x_p)
  * (minimum image; R5) with p = pid[x]; the node's exchange vector s is stored
- * to s_out[dim][N] when s_out != NULL (zero on eps = 0 nodes).
+ * to s_out[dim][N] when s_out != NULL (zero on eps = 0 nodes).  eps =
+ * eps_cnt[x] / eps_den with eps_den = S^D for the sampled map (orc_map) and
+ * 255 for the table map (orc_map_table).
  */
 void orc_step(int dim, const int64_t *n, const int32_t *bc, double tau,
-              const double *g, int S, const double *f_in, double *f_out,
+              const double *g, int eps_den, const double *f_in, double *f_out,
               const uint8_t *eps_cnt, const int32_t *pid, int64_t P,
               const double *pos, const double *vel, const double *omega,
               double *s_out) {
   int Q = nq(dim);
   int64_t nx = n[0], ny = n[1], nz = dim == 3 ? n[2] : 1;
   int64_t N = nx * ny * nz;
-  double SD = dim == 2 ? (double)(S * S) : (double)(S * S * S);
+  double SD = (double)eps_den; /* eps = eps_cnt / eps_den: S^D (sampling, R4) or 255 (table, R17) */
 #pragma omp parallel for
   for (int64_t k = 0; k < nz; ++k)
     for (int64_t j = 0; j < ny; ++j)
