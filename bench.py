@@ -188,6 +188,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--workload", default="C3", choices=["C2", "C3", "C4", "C5"])
     ap.add_argument("--impl", default="lbmimb", choices=["lbmimb", "reference"])
+    ap.add_argument("--map-mode", default="sampling", choices=["sampling", "table"],
+                    help="a1 variant: sub-cell sampling (BASELINE.json configs) or the paper's table look-up")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -203,7 +205,7 @@ def main():
         raise SystemExit("bench.py needs a CUDA device: the lbmimb path has no CPU fallback")
     torch.cuda.set_device(local)
     w = get_workload(args.workload)
-    lat = lb.from_workload(w, device=local)
+    lat = lb.from_workload(w, device=local, map_mode=lb.MAP_TABLE if args.map_mode == "table" else lb.MAP_SAMPLING)
     dem = w.dem
     Q = w.Q
     bytes_per_node = 2 * Q * 8 + 1 + 4
@@ -311,7 +313,8 @@ def main():
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.workload, "lattice": list(w.n), "Q": Q, "particles": w.P, "tau": w.tau,
-                       "bc": list(w.bc), "step": "map_particles + step(1) + reduce_particle_forces" +
+                       "bc": list(w.bc), "map_mode": args.map_mode,
+                       "step": "map_particles + step(1) + reduce_particle_forces" +
                        (" + dem_step" if dem else ""), "parallelism": "replicas x%d" % world,
                        "l2": "inputs (%.1f GB of distributions) exceed the 126 MB L2; no flush needed" %
                        (2 * Q * N * 8 / 1e9)},

@@ -86,6 +86,34 @@ enum {
   LBMIMB_FIELD_S = 5        /* double [D][box]  exchange vector s of the last step (0 where eps = 0) */
 };
 
+/*
+ * Mapping modes of a1 (lbmimb_set_mapping_mode).
+ * SAMPLING (default): the S^D sub-cell points of lbmimb_map_particles below; eps = n_s / S^D.
+ * TABLE: the paper's own method (eq. (6)): gamma = phi(d, theta) is pre-calculated for
+ *   "a solid particle with a given radius" and looked up per node from the distance d between the cell
+ *   centre and the particle centre and the orientation of the displacement.  Fig. 1 is not available, so
+ *   the discretisation is DESIGN.md R17:  sqD = sqrt(D), d0 = R - sqD/2, dd = sqD/Nd;
+ *     entry (k, m1[, m2]): d_k = d0 + (k+1/2) dd, t1 = (m1+1/2)/Nt, t2 = (m2+1/2)/Nt, cell centre
+ *       r = d_k (1, t1, t2)/sqrt(1 + t1^2 + t2^2), n = number of the St^D sub-cell points
+ *       r + ((a+1/2)/St - 1/2) inside the particle (|p|^2 <= R^2, fp64, no FMA, left to right),
+ *       code = (255 n + St^D/2) / St^D (integer division), gamma = code/255;
+ *     look-up of a node with displacement delta (minimum image): d = sqrt(dx^2 + dy^2 (+ dz^2));
+ *       d < d0 -> 255;  k = (int)((d - d0) * (Nd/sqD)), k >= Nd -> 0;  a >= b >= c the sorted |delta|,
+ *       m1 = min((int)((b/a) Nt), Nt-1), m2 = min((int)((c/a) Nt), Nt-1);
+ *     a node reached by several particles: code = min(255, sum of their codes), covering particle =
+ *       largest code, ties -> lowest index.
+ *   eps_cnt then holds the code and eps = code/255.  All particles must have one radius >= 1 (else
+ *   map_particles returns ESTATE).  Integer results, bit-exact against this definition.
+ */
+enum { LBMIMB_MAP_SAMPLING = 0, LBMIMB_MAP_TABLE = 1 };
+#define LBMIMB_TABLE_ND_2D 128
+#define LBMIMB_TABLE_NT_2D 32
+#define LBMIMB_TABLE_ST_2D 256
+#define LBMIMB_TABLE_ND_3D 128
+#define LBMIMB_TABLE_NT_3D 16
+#define LBMIMB_TABLE_ST_3D 64
+#define LBMIMB_TABLE_DEN 255
+
 /* Bytes of device memory a lattice of these parameters needs (0 on invalid parameters). */
 uint64_t lbmimb_workspace_bytes(const lbmimb_params *params, int64_t max_particles);
 
@@ -122,6 +150,15 @@ int64_t lbmimb_num_particles(const lbmimb_lattice *h);
  * the definition.  Uses a cell list over the particles.  Asynchronous.
  */
 lbmimb_status lbmimb_map_particles(lbmimb_lattice *h);
+
+/* Selects the mapping mode (see above).  Invalidates the particle map.  EINVAL on an unknown mode. */
+lbmimb_status lbmimb_set_mapping_mode(lbmimb_lattice *h, int32_t mode);
+/*
+ * Copies the look-up table of TABLE mode for the current particle radius into dst (uint8
+ * [Nd][Nt] in 2D, [Nd][Nt][Nt] in 3D; capacity = bytes available at dst).  Synchronous.
+ * ESTATE unless TABLE mode is selected and particles with one radius >= 1 are set.
+ */
+lbmimb_status lbmimb_fetch_eps_table(lbmimb_lattice *h, uint8_t *dst, int64_t capacity);
 
 /*
  * a2. nsteps fused collide-and-stream steps of eq. (1) with beta,

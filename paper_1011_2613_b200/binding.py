@@ -16,6 +16,9 @@ LIB_PATH = os.path.join(HERE, "liblbmimb.so")
 
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = range(5)
 FIELD_F, FIELD_RHO, FIELD_U, FIELD_EPS_CNT, FIELD_PID, FIELD_S = range(6)
+MAP_SAMPLING, MAP_TABLE = 0, 1
+TABLE_DEN = 255
+TABLE_SHAPE = {2: (128, 32), 3: (128, 16, 16)}      # LBMIMB_TABLE_ND/NT_* of include/lbmimb.h
 
 EXPORTS = [
     "lbmimb_workspace_bytes", "lbmimb_create_lattice", "lbmimb_destroy_lattice", "lbmimb_set_particles",
@@ -23,6 +26,7 @@ EXPORTS = [
     "lbmimb_step", "lbmimb_reduce_particle_forces", "lbmimb_dem_step", "lbmimb_fetch_fields",
     "lbmimb_set_distributions", "lbmimb_set_particles_dev", "lbmimb_reduce_particle_forces_dev",
     "lbmimb_synchronize", "lbmimb_time", "lbmimb_launch_count", "lbmimb_last_error", "lbmimb_version",
+    "lbmimb_set_mapping_mode", "lbmimb_fetch_eps_table",
 ]
 
 
@@ -67,6 +71,8 @@ def load():
     lib.lbmimb_num_particles.restype = i64
     lib.lbmimb_num_particles.argtypes = [vp]
     lib.lbmimb_map_particles.argtypes = [vp]
+    lib.lbmimb_set_mapping_mode.argtypes = [vp, i32]
+    lib.lbmimb_fetch_eps_table.argtypes = [vp, vp, i64]
     lib.lbmimb_step.argtypes = [vp, i32]
     lib.lbmimb_reduce_particle_forces.argtypes = [vp, vp, vp]
     lib.lbmimb_reduce_particle_forces_dev.argtypes = [vp, vp, vp]
@@ -204,6 +210,14 @@ class Lattice:
         return pos, vel, om
 
     # -- the path -----------------------------------------------------------
+    def set_mapping_mode(self, mode):
+        _check(self.lib.lbmimb_set_mapping_mode(self.h, mode))
+
+    def fetch_eps_table(self):
+        out = np.empty(TABLE_SHAPE[self.dim], dtype=np.uint8)
+        _check(self.lib.lbmimb_fetch_eps_table(self.h, _hp(out), out.nbytes))
+        return out
+
     def map_particles(self):
         _check(self.lib.lbmimb_map_particles(self.h))
 
@@ -259,10 +273,12 @@ class Lattice:
         return int(self.lib.lbmimb_launch_count(self.h))
 
 
-def from_workload(w, device=0, max_particles=None):
+def from_workload(w, device=0, max_particles=None, map_mode=MAP_SAMPLING):
     """Lattice for a paper_1011_2613_b200.inputs.Workload with its particles set (not yet mapped)."""
     lat = Lattice(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples,
                   max_particles=w.P if max_particles is None else max_particles, device=device)
+    if map_mode != MAP_SAMPLING:
+        lat.set_mapping_mode(map_mode)
     if w.P:
         lat.set_particles(w.pos, w.vel, w.omega, w.radius, w.mass)
     return lat

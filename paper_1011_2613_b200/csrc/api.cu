@@ -52,7 +52,7 @@ static bool valid_params(const lbmimb_params *p, int64_t maxp) {
 
 // One place that decides the device memory layout; used for sizing and for carving.
 struct Layout {
-  uint64_t off_f[2], off_eps, off_pid, off_s, off_beta, off_contested, off_counters;
+  uint64_t off_f[2], off_eps, off_pid, off_s, off_beta, off_contested, off_counters, off_table;
   uint64_t off_pos, off_vel, off_omega, off_radius, off_mass, off_force, off_torque, off_fc, off_prec;
   uint64_t off_count, off_start, off_fill, off_items, off_cell_of, off_bsums;
   uint64_t total;
@@ -82,6 +82,7 @@ static Layout make_layout(const lbmimb_params *p, int64_t maxp) {
   L.off_beta = take(256 * 8);
   L.off_contested = take((uint64_t)L.contested_cap * 8);
   L.off_counters = take(64);
+  L.off_table = take((uint64_t)eps_table_entries(p->dim));
   L.off_pos = take((uint64_t)3 * pm * 8);
   L.off_vel = take((uint64_t)3 * pm * 8);
   L.off_omega = take((uint64_t)3 * pm * 8);
@@ -193,6 +194,9 @@ lbmimb_status lbmimb_create_lattice(const lbmimb_params *params, int64_t max_par
   h->contested = (int64_t *)(h->ws + L.off_contested);
   h->contested_cap = L.contested_cap;
   h->counters = (int32_t *)(h->ws + L.off_counters);
+  h->eps_table = (uint8_t *)(h->ws + L.off_table);
+  h->map_mode = LBMIMB_MAP_SAMPLING;
+  h->table_R = -1.0;
   h->pos = (double *)(h->ws + L.off_pos);
   h->vel = (double *)(h->ws + L.off_vel);
   h->omega = (double *)(h->ws + L.off_omega);
@@ -268,8 +272,9 @@ lbmimb_status lbmimb_set_particles(lbmimb_lattice *h, int64_t P, const double *p
                                         (long long)h->Pmax);
   if (P > 0 && (!pos || !vel || !radius || !mass)) return fail(LBMIMB_EINVAL, "NULL particle array");
   int D = h->g.dim, nt = D == 2 ? 1 : 3;
-  double rmax = 0.0;
+  double rmax = 0.0, rmin = INFINITY;
   for (int64_t p = 0; p < P; ++p) {
+    if (radius[p] < rmin) rmin = radius[p];
     if (!(radius[p] > 0.0) || !(mass[p] > 0.0) || !std::isfinite(radius[p]) || !std::isfinite(mass[p]))
       return fail(LBMIMB_EINVAL, "particle %lld: radius and mass must be positive and finite", (long long)p);
     for (int a = 0; a < D; ++a) {
@@ -296,6 +301,7 @@ lbmimb_status lbmimb_set_particles(lbmimb_lattice *h, int64_t P, const double *p
   }
   h->P = P;
   h->rmax = rmax;
+  h->rmin = P > 0 ? rmin : 0.0;
   if (P == 0) {
     LBMIMB_CUDA(cudaMemsetAsync(h->eps_cnt, 0, (size_t)h->g.N, h->stream));
     LBMIMB_CUDA(cudaMemsetAsync(h->pid, 0xFF, (size_t)h->g.N * 4, h->stream));
@@ -314,7 +320,7 @@ lbmimb_status lbmimb_set_particles_dev(lbmimb_lattice *h, int64_t P, const doubl
   lbmimb_status st = use_device(h);
   if (st != LBMIMB_OK) return st;
   int D = h->g.dim, nt = D == 2 ? 1 : 3;
-  double rmax = 0.0;
+  double rmax = 0.0, rmin = INFINITY;
   if (P > 0) {
     auto d2d = [&](void *dst, const void *src, uint64_t bytes) -> lbmimb_status {
       LBMIMB_CUDA(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, h->stream));
@@ -338,10 +344,12 @@ lbmimb_status lbmimb_set_particles_dev(lbmimb_lattice *h, int64_t P, const doubl
     for (int64_t p = 0; p < P; ++p) {
       if (!(r[p] > 0.0) || !std::isfinite(r[p])) return fail(LBMIMB_EINVAL, "particle %lld: bad radius", (long long)p);
       if (r[p] > rmax) rmax = r[p];
+      if (r[p] < rmin) rmin = r[p];
     }
   }
   h->P = P;
   h->rmax = rmax;
+  h->rmin = P > 0 ? rmin : 0.0;
   if (P == 0) {
     LBMIMB_CUDA(cudaMemsetAsync(h->eps_cnt, 0, (size_t)h->g.N, h->stream));
     LBMIMB_CUDA(cudaMemsetAsync(h->pid, 0xFF, (size_t)h->g.N * 4, h->stream));
@@ -403,6 +411,39 @@ lbmimb_status lbmimb_map_particles(lbmimb_lattice *h) {
   h->map_valid = true;
   h->s_valid = false;
   h->forces_valid = false;
+  return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_set_mapping_mode(lbmimb_lattice *h, int32_t mode) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (mode != LBMIMB_MAP_SAMPLING && mode != LBMIMB_MAP_TABLE) return fail(LBMIMB_EINVAL, "unknown mapping mode %d", mode);
+  if (mode == h->map_mode) return LBMIMB_OK;
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  // eps = eps_cnt / S^D (sampling) or code / 255 (table): refresh beta(eps, tau)
+  double tab[256];
+  fill_beta_table(h->prm.tau, mode == LBMIMB_MAP_TABLE ? LBMIMB_TABLE_DEN : h->SD, tab);
+  LBMIMB_CUDA(cudaMemcpyAsync(h->beta_tab, tab, sizeof(tab), cudaMemcpyHostToDevice, h->stream));
+  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));  // tab lives on this stack frame
+  h->map_mode = mode;
+  h->map_valid = (h->P == 0);
+  h->s_valid = false;
+  h->forces_valid = false;
+  return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_fetch_eps_table(lbmimb_lattice *h, uint8_t *dst, int64_t capacity) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (!dst) return fail(LBMIMB_EINVAL, "dst is NULL");
+  if (h->map_mode != LBMIMB_MAP_TABLE) return fail(LBMIMB_ESTATE, "table mapping mode is not selected");
+  if (h->P == 0) return fail(LBMIMB_ESTATE, "no particles: the table is built for the particles' radius");
+  const int64_t bytes = eps_table_entries(h->g.dim);
+  if (capacity < bytes) return fail(LBMIMB_EINVAL, "dst holds %lld bytes, the table has %lld", (long long)capacity, (long long)bytes);
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  if ((st = ensure_eps_table(h)) != LBMIMB_OK) return st;
+  LBMIMB_CUDA(cudaMemcpyAsync(dst, h->eps_table, (size_t)bytes, cudaMemcpyDeviceToHost, h->stream));
+  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
   return LBMIMB_OK;
 }
 

@@ -110,7 +110,10 @@ struct lbmimb_lattice {
   // particles (SoA, device)
   int64_t Pmax, P;
   double *pos, *vel, *omega, *radius, *mass, *force, *torque, *fc, *prec;
-  double rmax;        // max radius of the current set
+  double rmax, rmin;  // largest / smallest radius of the current set
+  int map_mode;       // LBMIMB_MAP_SAMPLING or LBMIMB_MAP_TABLE
+  uint8_t *eps_table; // table of map mode TABLE (R17), built for radius table_R
+  double table_R;
   lbmimb::CellList cl;
   bool cl_valid;
 
@@ -148,6 +151,8 @@ lbmimb_status launch_fetch(lbmimb_lattice *h, int what, const int64_t lo[3], con
 lbmimb_status launch_pack_records(lbmimb_lattice *h);
 lbmimb_status build_cell_list(lbmimb_lattice *h);
 lbmimb_status launch_map(lbmimb_lattice *h);
+lbmimb_status ensure_eps_table(lbmimb_lattice *h);
+int64_t eps_table_entries(int dim);
 lbmimb_status launch_reduce(lbmimb_lattice *h);
 lbmimb_status launch_dem(lbmimb_lattice *h, const lbmimb_dem_params *dem);
 

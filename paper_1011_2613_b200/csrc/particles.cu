@@ -459,6 +459,67 @@ __global__ void __launch_bounds__(128) map_contested_kernel(const MapArgs a, con
   }
 }
 
+#include "map_table.cuh"
+
+// table geometry of DESIGN.md R17 for the handle's (single) particle radius
+static TableGeom table_geom(const lbmimb_lattice *h) {
+  TableGeom t;
+  const int D = h->g.dim;
+  t.Nd = D == 2 ? LBMIMB_TABLE_ND_2D : LBMIMB_TABLE_ND_3D;
+  t.Nt = D == 2 ? LBMIMB_TABLE_NT_2D : LBMIMB_TABLE_NT_3D;
+  t.St = D == 2 ? LBMIMB_TABLE_ST_2D : LBMIMB_TABLE_ST_3D;
+  const double sqD = sqrt((double)D);
+  t.R = h->rmax;
+  t.d0 = h->rmax - 0.5 * sqD;
+  t.inv_dd = (double)t.Nd / sqD;
+  t.dd = sqD / (double)t.Nd;
+  t.full2 = t.d0 > 1e-9 ? (t.d0 - 1e-9) * (t.d0 - 1e-9) : 0.0;
+  t.none2 = (t.d0 + sqD + 1e-9) * (t.d0 + sqD + 1e-9);
+  t.tab = h->eps_table;
+  return t;
+}
+
+int64_t eps_table_entries(int dim) {
+  return dim == 2 ? (int64_t)LBMIMB_TABLE_ND_2D * LBMIMB_TABLE_NT_2D
+                  : (int64_t)LBMIMB_TABLE_ND_3D * LBMIMB_TABLE_NT_3D * LBMIMB_TABLE_NT_3D;
+}
+
+// (re)builds the table when the radius changed since the last build
+lbmimb_status ensure_eps_table(lbmimb_lattice *h) {
+  if (h->P > 0 && h->rmin != h->rmax)
+    return fail(LBMIMB_ESTATE, "table mapping needs one particle radius (PAPER.md:73), got %g .. %g", h->rmin, h->rmax);
+  if (!(h->rmax >= 1.0)) return fail(LBMIMB_ESTATE, "table mapping needs a radius >= 1 lattice spacing");
+  if (h->table_R == h->rmax) return LBMIMB_OK;
+  const TableGeom t = table_geom(h);
+  const int entries = (int)eps_table_entries(h->g.dim);
+  if (h->g.dim == 2) build_eps_table_kernel<2><<<entries, 256, 0, h->stream>>>(t, h->eps_table);
+  else build_eps_table_kernel<3><<<entries, 256, 0, h->stream>>>(t, h->eps_table);
+  LBMIMB_LAUNCH_CHECK(h, "build_eps_table_kernel");
+  h->table_R = h->rmax;
+  return LBMIMB_OK;
+}
+
+static lbmimb_status launch_map_table(lbmimb_lattice *h, const MapArgs &a) {
+  lbmimb_status st = ensure_eps_table(h);
+  if (st != LBMIMB_OK) return st;
+  const TableGeom t = table_geom(h);
+  const double edge = 2.0 * h->rmax + 3.0;
+  if (h->g.dim == 2) {
+    if (edge * edge <= 256.0) map_table_kernel<2, 16><<<blocks_for(h->P, 8), 128, 0, h->stream>>>(a, t);
+    else map_table_kernel<2, 32><<<blocks_for(h->P, 4), 128, 0, h->stream>>>(a, t);
+  } else {
+    map_table_kernel<3, 128><<<blocks_for(h->P, 1), 128, 0, h->stream>>>(a, t);
+  }
+  LBMIMB_LAUNCH_CHECK(h, "map_table_kernel");
+  CellGeom cg = cell_geom(h);
+  if (h->g.dim == 2)
+    map_table_contested_kernel<2><<<148 * 4, 128, 0, h->stream>>>(a, t, cg, h->cl.start, h->cl.items);
+  else
+    map_table_contested_kernel<3><<<148 * 4, 128, 0, h->stream>>>(a, t, cg, h->cl.start, h->cl.items);
+  LBMIMB_LAUNCH_CHECK(h, "map_table_contested_kernel");
+  return LBMIMB_OK;
+}
+
 lbmimb_status launch_map(lbmimb_lattice *h) {
   lbmimb_status st;
   if (!h->cl_valid && (st = build_cell_list(h)) != LBMIMB_OK) return st;
@@ -481,6 +542,7 @@ lbmimb_status launch_map(lbmimb_lattice *h) {
   a.h_in = hs + 1e-6;
   a.h_out = hs + 1e-6;
   a.hs = 0.5 - 0.5 / (double)a.S;
+  if (h->map_mode == LBMIMB_MAP_TABLE) return launch_map_table(h, a);
   // threads per particle: enough lanes for the boundary shell without leaving most of them idle
   const double edge = 2.0 * h->rmax + 3.0;
   if (h->g.dim == 2) {
@@ -634,6 +696,7 @@ __global__ void __launch_bounds__(128) reduce_forces_kernel(Geom g, int64_t P, d
 // half extent of a node's sample cloud plus a safety margin: a node whose centre is farther than
 // R + h from a particle centre has no sample inside that particle
 static double sample_cloud_radius(const lbmimb_lattice *h) {
+  if (h->map_mode == LBMIMB_MAP_TABLE) return 0.5 * sqrt((double)h->g.dim) + 1e-6;  // whole cell (R17)
   return sqrt((double)h->g.dim) * (0.5 - 0.5 / (double)h->prm.subsamples) + 1e-6;
 }
 
