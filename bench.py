@@ -190,6 +190,8 @@ def main():
     ap.add_argument("--impl", default="lbmimb", choices=["lbmimb", "reference"])
     ap.add_argument("--map-mode", default="sampling", choices=["sampling", "table"],
                     help="a1 variant: sub-cell sampling (BASELINE.json configs) or the paper's table look-up")
+    ap.add_argument("--streaming", default="ab", choices=["ab", "aa"],
+                    help="a2 variant: pull with two arrays (A-B) or in-place AA-pattern on one array")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -205,7 +207,8 @@ def main():
         raise SystemExit("bench.py needs a CUDA device: the lbmimb path has no CPU fallback")
     torch.cuda.set_device(local)
     w = get_workload(args.workload)
-    lat = lb.from_workload(w, device=local, map_mode=lb.MAP_TABLE if args.map_mode == "table" else lb.MAP_SAMPLING)
+    lat = lb.from_workload(w, device=local, map_mode=lb.MAP_TABLE if args.map_mode == "table" else lb.MAP_SAMPLING,
+                           streaming=lb.STREAM_AA if args.streaming == "aa" else lb.STREAM_AB)
     dem = w.dem
     Q = w.Q
     bytes_per_node = 2 * Q * 8 + 1 + 4
@@ -300,8 +303,9 @@ def main():
 
     peak, peak_src = measured_peak_gbs()
     achieved = bytes_per_node * N / (kern_ms * 1e-3) / 1e9
-    roof = {"bound": "hbm", "kernel": "collide_stream_kernel<%d,IMB,EMIT>" % w.dim, "achieved": achieved,
-            "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload), "peak_source": peak_src,
+    roof = {"bound": "hbm", "kernel": ("collide_stream_aa_kernel<%d,IMB,EMIT,even|odd>" if args.streaming == "aa"
+                                       else "collide_stream_kernel<%d,IMB,EMIT>") % w.dim, "achieved": achieved,
+            "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload) if args.streaming == "ab" else None, "peak_source": peak_src,
             "bytes_per_node": bytes_per_node, "nodes_per_launch": N, "kernel_ms": kern_ms,
             "kernel_mlups": N / (kern_ms * 1e-3) / 1e6, "frac_of_nominal_8TBs": achieved / 8000.0,
             "kernel_share_of_step": kern_ms / (total_ms / args.steps)}
@@ -313,11 +317,11 @@ def main():
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.workload, "lattice": list(w.n), "Q": Q, "particles": w.P, "tau": w.tau,
-                       "bc": list(w.bc), "map_mode": args.map_mode,
+                       "bc": list(w.bc), "map_mode": args.map_mode, "streaming": args.streaming,
                        "step": "map_particles + step(1) + reduce_particle_forces" +
                        (" + dem_step" if dem else ""), "parallelism": "replicas x%d" % world,
                        "l2": "inputs (%.1f GB of distributions) exceed the 126 MB L2; no flush needed" %
-                       (2 * Q * N * 8 / 1e9)},
+                       ((1 if args.streaming == "aa" else 2) * Q * N * 8 / 1e9)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
             "breakdown_ms": {"map_particles": float(seg[:, 0].mean()), "step": kern_ms,
                              "reduce_particle_forces": float(seg[:, 2].mean()),

@@ -67,7 +67,20 @@ typedef struct {
   void *stream;       /* cudaStream_t to run on (e.g. torch.cuda.current_stream().cuda_stream), NULL = default */
   void *workspace_dev;      /* optional caller-owned device buffer, 256-byte aligned; NULL = library allocates */
   uint64_t workspace_bytes; /* size of workspace_dev; must be >= lbmimb_workspace_bytes() */
+  int32_t streaming;  /* LBMIMB_STREAM_AB (0, default) or LBMIMB_STREAM_AA: how step() propagates, see below */
+  int32_t reserved;   /* must be 0 */
 } lbmimb_params;
+
+/*
+ * Streaming schemes of a2 (same results up to rounding order; both are fused collide-and-stream kernels):
+ *   AB: "pull" with two distribution arrays (2 x Q x N doubles); a step reads one and writes the other.
+ *   AA: in-place AA-pattern on ONE array (Q x N doubles): even steps touch only the own node, odd steps
+ *       gather from and scatter to the neighbours.  Halves the footprint, which is what lets the paper's
+ *       512 x 2016 x 512 D3Q19 lattice (80.3 GB of distributions) fit one 180 GB B200.
+ *       In AA mode fetch_fields stages through a temporary device buffer of the box's size (ENOMEM if
+ *       that cannot be allocated: fetch sub-boxes of a large lattice).
+ */
+enum { LBMIMB_STREAM_AB = 0, LBMIMB_STREAM_AA = 1 };
 
 typedef struct {
   double kn;            /* stiffness k_n of eq. (4) */

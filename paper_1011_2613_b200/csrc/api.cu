@@ -44,6 +44,9 @@ static bool valid_params(const lbmimb_params *p, int64_t maxp) {
   if (p->subsamples < 1) return fail(LBMIMB_EINVAL, "subsamples must be >= 1"), false;
   for (int a = 0; a < p->dim; ++a) sd *= p->subsamples;
   if (sd > 255) return fail(LBMIMB_EINVAL, "subsamples^dim must be <= 255"), false;
+  if (p->streaming != LBMIMB_STREAM_AB && p->streaming != LBMIMB_STREAM_AA)
+    return fail(LBMIMB_EINVAL, "streaming must be LBMIMB_STREAM_AB or LBMIMB_STREAM_AA"), false;
+  if (p->reserved != 0) return fail(LBMIMB_EINVAL, "reserved must be 0"), false;
   if (maxp < 0 || maxp > 0x7fffffff) return fail(LBMIMB_EINVAL, "max_particles out of range"), false;
   double nn = (double)p->n[0] * (double)p->n[1] * (double)p->n[2];
   if (nn > 4.0e12) return fail(LBMIMB_EINVAL, "lattice too large"), false;
@@ -75,7 +78,7 @@ static Layout make_layout(const lbmimb_params *p, int64_t maxp) {
     return r;
   };
   L.off_f[0] = take((uint64_t)Q * L.N * 8);
-  L.off_f[1] = take((uint64_t)Q * L.N * 8);
+  L.off_f[1] = p->streaming == LBMIMB_STREAM_AA ? L.off_f[0] : take((uint64_t)Q * L.N * 8);
   L.off_eps = take((uint64_t)L.N);
   L.off_pid = take((uint64_t)L.N * 4);
   L.off_s = take((uint64_t)exchange_stride(p->dim) * L.N * 8);
@@ -128,7 +131,7 @@ using namespace lbmimb;
 extern "C" {
 
 const char *lbmimb_last_error(void) { return g_err; }
-const char *lbmimb_version(void) { return "lbmimb 0.1 (sm_100a, pull AB fused collide-stream)"; }
+const char *lbmimb_version(void) { return "lbmimb 0.2 (sm_100a, fused collide-stream: pull A-B and in-place AA)"; }
 
 uint64_t lbmimb_workspace_bytes(const lbmimb_params *params, int64_t max_particles) {
   if (!valid_params(params, max_particles)) return 0;
@@ -236,6 +239,8 @@ lbmimb_status lbmimb_create_lattice(const lbmimb_params *params, int64_t max_par
     return st;
   }
   h->cur = 0;
+  h->aa = params->streaming == LBMIMB_STREAM_AA;
+  h->aa_swapped = false;
   h->P = 0;
   h->map_valid = true;  // no particles: the all-zero map is the map
   h->s_valid = false;
@@ -456,7 +461,10 @@ lbmimb_status lbmimb_step(lbmimb_lattice *h, int32_t nsteps) {
   for (int32_t it = 0; it < nsteps; ++it) {
     bool emit = (h->P > 0) && (it == nsteps - 1);
     if ((st = launch_collide_stream(h, emit)) != LBMIMB_OK) return st;
-    h->cur ^= 1;
+    if (h->aa)
+      h->aa_swapped = !h->aa_swapped;
+    else
+      h->cur ^= 1;
     h->t += 1;
     if (emit) h->s_valid = true;
     h->forces_valid = false;
@@ -544,12 +552,25 @@ lbmimb_status lbmimb_fetch_fields(lbmimb_lattice *h, int32_t what, const int64_t
   if (what == LBMIMB_FIELD_S && h->P > 0 && !h->s_valid) return fail(LBMIMB_ESTATE, "no exchange vectors yet");
   lbmimb_status st = use_device(h);
   if (st != LBMIMB_OK) return st;
-  // the idle distribution buffer is the staging area: every field of a sub-box fits in Q*N doubles
+  // A-B: the idle distribution buffer is the staging area (every field of a sub-box fits in Q*N
+  // doubles).  AA has no idle buffer: a temporary one of the box's size.
   void *stage = h->f[h->cur ^ 1];
-  if ((st = launch_fetch(h, what, lo, hi, stage)) != LBMIMB_OK) return st;
-  LBMIMB_CUDA(cudaMemcpyAsync(dst, stage, (size_t)comps * box * esz, cudaMemcpyDeviceToHost, h->stream));
-  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
-  return LBMIMB_OK;
+  void *tmp = nullptr;
+  if (h->aa) {
+    cudaError_t e = cudaMalloc(&tmp, (size_t)comps * box * esz);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc(fetch staging, AA mode)");
+    stage = tmp;
+  }
+  auto body = [&]() -> lbmimb_status {
+    lbmimb_status s2 = launch_fetch(h, what, lo, hi, stage);
+    if (s2 != LBMIMB_OK) return s2;
+    LBMIMB_CUDA(cudaMemcpyAsync(dst, stage, (size_t)comps * box * esz, cudaMemcpyDeviceToHost, h->stream));
+    LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+    return LBMIMB_OK;
+  };
+  st = body();
+  if (tmp) cudaFree(tmp);
+  return st;
 }
 
 lbmimb_status lbmimb_set_distributions(lbmimb_lattice *h, const double *f) {
@@ -557,9 +578,14 @@ lbmimb_status lbmimb_set_distributions(lbmimb_lattice *h, const double *f) {
   if (!f) return fail(LBMIMB_EINVAL, "f is NULL");
   lbmimb_status st = use_device(h);
   if (st != LBMIMB_OK) return st;
-  double *stage = h->f[h->cur ^ 1];
-  LBMIMB_CUDA(cudaMemcpyAsync(stage, f, (size_t)h->Q * h->g.N * 8, cudaMemcpyHostToDevice, h->stream));
-  if ((st = launch_unstream(h, stage, h->f[h->cur])) != LBMIMB_OK) return st;
+  if (h->aa) {   // the AA natural layout IS f_i(x,t)
+    LBMIMB_CUDA(cudaMemcpyAsync(h->f[0], f, (size_t)h->Q * h->g.N * 8, cudaMemcpyHostToDevice, h->stream));
+    h->aa_swapped = false;
+  } else {
+    double *stage = h->f[h->cur ^ 1];
+    LBMIMB_CUDA(cudaMemcpyAsync(stage, f, (size_t)h->Q * h->g.N * 8, cudaMemcpyHostToDevice, h->stream));
+    if ((st = launch_unstream(h, stage, h->f[h->cur])) != LBMIMB_OK) return st;
+  }
   LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
   h->t = 0;
   h->s_valid = false;

@@ -30,6 +30,7 @@ struct StepArgs {
 };
 
 constexpr int kStepThreads = 128;
+enum { kLayoutPull = 0, kLayoutNatural = 1, kLayoutSwapped = 2 };
 
 // ---------------------------------------------------------------------------
 // a2: fused collide-and-stream, one thread per node, one block per row segment.
@@ -125,6 +126,114 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
 }
 
 // ---------------------------------------------------------------------------
+// a2, in-place variant: AA-pattern streaming on ONE distribution array (BASELINE.json north_star:
+// "either a pull-scheme double buffer or AA-pattern in-place streaming").  The array alternates
+// between two layouts:
+//   natural (after an ODD step, or after init / set_distributions): slot q of node x holds f_q(x,t);
+//   swapped (after an EVEN step): slot -q of node x holds f*_q(x,t-1), so that
+//       f_q(x,t) = slot -q of node x - c_q, or slot q of node x itself when x - c_q lies behind a wall.
+// EVEN step: read the own node's slots, collide, write f*_q to slot -q of the own node (no neighbour
+// access, every load and store aligned).  ODD step: gather as above, collide, write f*_q to slot q of
+// node x + c_q (or slot -q of x through a wall): a node reads and writes exactly the same set of
+// locations and no two nodes share one, so the update is race-free in place.
+// ---------------------------------------------------------------------------
+template <int D, bool IMB, bool EMIT, bool ODD, int MINB>
+__global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_aa_kernel(const StepArgs a) {
+  using L = Lat<D>;
+  constexpr int Q = L::Q;
+  const unsigned row = blockIdx.x / a.tiles;
+  const unsigned tile = blockIdx.x - row * a.tiles;
+  const int i0 = (int)(tile * kStepThreads + threadIdx.x);
+  const bool live = i0 < a.nx;
+  const int i = live ? i0 : a.nx - 1;
+  const int k = D == 3 ? (int)(row / (unsigned)a.ny) : 0;
+  const int j = (int)(row - (unsigned)k * (unsigned)a.ny);
+  const int64_t rowoff = ((int64_t)k * a.ny + j) * a.nx;
+  const int64_t x = rowoff + i;
+  const int im = i == 0 ? a.nx - 1 : i - 1;
+  const int ip = i == a.nx - 1 ? 0 : i + 1;
+  double *__restrict__ F = a.fout;   // the one array (fin == fout)
+
+  int cnt = 0, pe = 0;
+  if (IMB) {
+    cnt = a.eps_cnt[x];
+    pe = a.pid[x];
+  }
+
+  double f[Q];
+  if (!ODD) {
+#pragma unroll
+    for (int q = 0; q < Q; ++q) f[q] = F[(int64_t)q * a.N + x];
+  } else {
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      const int cx = L::cx(q), cy = L::cy(q), cz = L::cz(q);
+      bool bounce = false;
+      int js = j - cy, ks = k - cz;
+      if (cy != 0 && (js < 0 || js >= a.ny)) {
+        if (a.bcy) bounce = true;
+        else js = js < 0 ? js + a.ny : js - a.ny;
+      }
+      if (D == 3 && cz != 0 && (ks < 0 || ks >= a.nz)) {
+        if (a.bcz) bounce = true;
+        else ks = ks < 0 ? ks + a.nz : ks - a.nz;
+      }
+      if (cx != 0 && a.bcx && ((cx == 1 && i == 0) || (cx == -1 && i == a.nx - 1))) bounce = true;
+      const double *base = bounce ? F + ((int64_t)q * a.N + rowoff)
+                                  : F + ((int64_t)opposite(q) * a.N + ((int64_t)ks * a.ny + js) * a.nx);
+      const int xs = (bounce || cx == 0) ? i : (cx == 1 ? im : ip);
+      f[q] = base[xs];
+    }
+  }
+
+  double beta = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
+  if (IMB && cnt > 0) {
+    beta = __ldg(a.beta_tab + cnt);
+    solid_velocity<D>(a.prec + (int64_t)pe * prec_stride(D), i, j, k, a.nx, a.ny, a.nz, a.bcx, a.bcy, a.bcz, vx, vy,
+                      vz);
+  }
+
+  double rho, ux, uy, uz;
+  moments<D>(f, rho, ux, uy, uz);
+
+  if (!IMB || !__any_sync(0xffffffffu, cnt > 0)) {
+    collide_fluid<D>(f, a.cp, rho, ux, uy, uz);
+  } else {
+    collide_imb<D>(f, a.cp, rho, ux, uy, uz, beta, vx, vy, vz);
+    if (EMIT && cnt > 0 && live) {
+      const double br = beta * rho;
+      store_exchange<D>(a.s, x, br * (vx - ux), br * (vy - uy), br * (vz - uz));
+    }
+  }
+
+  if (!live) return;
+  if (!ODD) {
+#pragma unroll
+    for (int q = 0; q < Q; ++q) F[(int64_t)opposite(q) * a.N + x] = f[q];
+  } else {
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      const int cx = L::cx(q), cy = L::cy(q), cz = L::cz(q);
+      bool bounce = false;
+      int jt = j + cy, kt = k + cz;
+      if (cy != 0 && (jt < 0 || jt >= a.ny)) {
+        if (a.bcy) bounce = true;
+        else jt = jt < 0 ? jt + a.ny : jt - a.ny;
+      }
+      if (D == 3 && cz != 0 && (kt < 0 || kt >= a.nz)) {
+        if (a.bcz) bounce = true;
+        else kt = kt < 0 ? kt + a.nz : kt - a.nz;
+      }
+      if (cx != 0 && a.bcx && ((cx == 1 && i == a.nx - 1) || (cx == -1 && i == 0))) bounce = true;
+      double *base = bounce ? F + ((int64_t)opposite(q) * a.N + rowoff)
+                            : F + ((int64_t)q * a.N + ((int64_t)kt * a.ny + jt) * a.nx);
+      const int xt = (bounce || cx == 0) ? i : (cx == 1 ? ip : im);
+      base[xt] = f[q];
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------
 // a0: f = w_i (rest state, rho = 1, u = 0)
 // ---------------------------------------------------------------------------
 template <int D>
@@ -138,14 +247,20 @@ __global__ void init_rest_kernel(double *__restrict__ f, int64_t N) {
 }
 
 // ---------------------------------------------------------------------------
-// Gather of the pre-collision state f_i(x,t) from the stored post-collision array
-// (the same permutation the step kernel applies), for one node.
+// Gather of the pre-collision state f_i(x,t) of one node from the stored array, whose layout is
+// pull (post-collision, A-B scheme), AA natural or AA swapped.
 // ---------------------------------------------------------------------------
 template <int D>
-__device__ __forceinline__ void gather_node(const double *__restrict__ fpost, const Geom &g, int i, int j, int k,
-                                            double *f) {
+__device__ __forceinline__ void gather_node(const double *__restrict__ fst, const Geom &g, int layout, int i, int j,
+                                            int k, double *f) {
   using L = Lat<D>;
   const int64_t x = ((int64_t)k * g.ny + j) * g.nx + i;
+  if (layout == kLayoutNatural) {
+#pragma unroll
+    for (int q = 0; q < L::Q; ++q) f[q] = fst[(int64_t)q * g.N + x];
+    return;
+  }
+  const bool swapped = layout == kLayoutSwapped;
 #pragma unroll
   for (int q = 0; q < L::Q; ++q) {
     const int cx = L::cx(q), cy = L::cy(q), cz = L::cz(q);
@@ -163,9 +278,11 @@ __device__ __forceinline__ void gather_node(const double *__restrict__ fpost, co
       if (g.bcz) bounce = true;
       else ks = ks < 0 ? ks + g.nz : ks - g.nz;
     }
-    const int64_t src = bounce ? (int64_t)opposite(q) * g.N + x
-                               : (int64_t)q * g.N + ((int64_t)ks * g.ny + js) * g.nx + is;
-    f[q] = fpost[src];
+    // pull (A-B): slot q of the source node, slot -q of the own node through a wall;
+    // AA swapped: the two slots exchanged (see collide_stream_aa_kernel)
+    const int slot = (bounce != swapped) ? opposite(q) : q;
+    const int64_t src = bounce ? (int64_t)slot * g.N + x : (int64_t)slot * g.N + ((int64_t)ks * g.ny + js) * g.nx + is;
+    f[q] = fst[src];
   }
 }
 
@@ -213,6 +330,7 @@ struct FetchArgs {
   int64_t box;
   int what;
   int have_particles;
+  int layout;
 };
 
 template <int D>
@@ -235,7 +353,7 @@ __global__ void fetch_kernel(const FetchArgs a, const Geom g) {
       for (int c = 0; c < D; ++c) ((double *)a.dst)[(int64_t)c * a.box + b] = cov ? a.s[x * exchange_stride(D) + c] : 0.0;
     } else {
       double f[L::Q];
-      gather_node<D>(a.fpost, g, i, j, k, f);
+      gather_node<D>(a.fpost, g, a.layout, i, j, k, f);
       if (a.what == LBMIMB_FIELD_F) {
 #pragma unroll
         for (int q = 0; q < L::Q; ++q) ((double *)a.dst)[(int64_t)q * a.box + b] = f[q];
@@ -320,6 +438,19 @@ static void launch_cs(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, boo
   }
 }
 
+template <int D, int MINB>
+static void launch_aa(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, bool imb, bool emit, bool odd) {
+#define LBMIMB_AA(I, E, O) collide_stream_aa_kernel<D, I, E, O, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a)
+  if (!imb) {
+    if (odd) LBMIMB_AA(false, false, true); else LBMIMB_AA(false, false, false);
+  } else if (!emit) {
+    if (odd) LBMIMB_AA(true, false, true); else LBMIMB_AA(true, false, false);
+  } else {
+    if (odd) LBMIMB_AA(true, true, true); else LBMIMB_AA(true, true, false);
+  }
+#undef LBMIMB_AA
+}
+
 lbmimb_status launch_collide_stream(lbmimb_lattice *h, bool emit) {
   StepArgs a;
   a.fin = h->f[h->cur];
@@ -341,6 +472,15 @@ lbmimb_status launch_collide_stream(lbmimb_lattice *h, bool emit) {
   const int64_t blocks = (int64_t)a.tiles * h->g.ny * h->g.nz;
   if (blocks > 0x7fffffff) return fail(LBMIMB_EINVAL, "lattice needs more than 2^31 thread blocks");
   const bool imb = h->P > 0;
+  if (h->aa) {
+    a.fin = a.fout = h->f[0];
+    if (h->g.dim == 2)
+      launch_aa<2, 9>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
+    else
+      launch_aa<3, 6>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
+    LBMIMB_LAUNCH_CHECK(h, "collide_stream_aa_kernel");
+    return LBMIMB_OK;
+  }
   if (step_variant() >= 10) {
     bool done = false;
     lbmimb_status st = launch_collide_stream_tma(h, emit, step_variant(), &done);
@@ -378,6 +518,7 @@ lbmimb_status launch_fetch(lbmimb_lattice *h, int what, const int64_t lo[3], con
   }
   a.what = what;
   a.have_particles = h->P > 0;
+  a.layout = h->aa ? (h->aa_swapped ? kLayoutSwapped : kLayoutNatural) : kLayoutPull;
   if (h->g.dim == 2)
     fetch_kernel<2><<<grid_for(a.box, 256), 256, 0, h->stream>>>(a, h->g);
   else

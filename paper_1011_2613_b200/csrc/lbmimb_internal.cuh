@@ -97,8 +97,11 @@ struct lbmimb_lattice {
 
   // lattice state.  f[cur] holds the POST-COLLISION distributions f*(x, t-1) of the last step
   // ("pull" representation): f_i(x,t) = f*_i(x - c_i) or, through a wall, f*_{-i}(x).
+  // In AA mode (prm.streaming == LBMIMB_STREAM_AA) there is one array f[0]; aa_swapped tells which of
+  // the two AA layouts it is in (lattice.cu: collide_stream_aa_kernel).
   double *f[2];
   int cur;
+  bool aa, aa_swapped;
   uint8_t *eps_cnt;   // [N]
   int32_t *pid;       // [N]
   double *s;          // [N][exchange_stride] exchange vectors of the last step

@@ -72,9 +72,10 @@ def assert_forces_close(gF, gT, ref, tol=FORCE_TOL):
     return float((dF / (lim + 1e-300)).max()), float((dT / (limT + 1e-300)).max())
 
 
-def gpu_run(lb, w, steps, f0=None):
-    """Fixed-particle CUDA run through the C-ABI binding; returns (lattice, dict)."""
-    lat = lb.from_workload(w)
+def gpu_run(lb, w, steps, f0=None, streaming=0):
+    """Fixed-particle CUDA run through the C-ABI binding; returns (lattice, dict).
+    streaming: lb.STREAM_AB (0) or lb.STREAM_AA (1)."""
+    lat = lb.from_workload(w, streaming=streaming)
     if f0 is not None:
         lat.set_distributions(f0)
     if w.P:
