@@ -27,6 +27,9 @@ struct StepArgs {
   int bcx, bcy, bcz;
   unsigned tiles;      // blocks per lattice row
   CollideParams cp;
+  // AA odd step, rows away from walls and seams: f_q(x) lives koff[q] bytes behind element x - cx_q
+  // of the array (koff[q] = 8 (opposite(q) * N - cy_q * nx - cz_q * nx * ny))
+  int64_t koff[19];
 };
 
 constexpr int kStepThreads = 128;
@@ -137,7 +140,11 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
 // node x + c_q (or slot -q of x through a wall): a node reads and writes exactly the same set of
 // locations and no two nodes share one, so the update is race-free in place.
 // ---------------------------------------------------------------------------
-template <int D, bool IMB, bool EMIT, bool ODD, int MINB>
+// In the ODD step the location node x reads f_q from is the one it writes f*_{-q} to, so there is ONE
+// address per direction: a block-uniform 64-bit offset (slot and row, looked up in a table of the 9
+// neighbouring rows (dy,dz) with their wall flags) plus one of the three wrapped x indices.
+// XW = walls in x, where the end nodes of a row bounce per thread.
+template <int D, bool IMB, bool EMIT, bool ODD, bool XW, int MINB>
 __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_aa_kernel(const StepArgs a) {
   using L = Lat<D>;
   constexpr int Q = L::Q;
@@ -150,8 +157,6 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_aa_kernel(c
   const int j = (int)(row - (unsigned)k * (unsigned)a.ny);
   const int64_t rowoff = ((int64_t)k * a.ny + j) * a.nx;
   const int64_t x = rowoff + i;
-  const int im = i == 0 ? a.nx - 1 : i - 1;
-  const int ip = i == a.nx - 1 ? 0 : i + 1;
   double *__restrict__ F = a.fout;   // the one array (fin == fout)
 
   int cnt = 0, pe = 0;
@@ -160,30 +165,45 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_aa_kernel(c
     pe = a.pid[x];
   }
 
+  const int im = i == 0 ? a.nx - 1 : i - 1;
+  const int ip = i == a.nx - 1 ? 0 : i + 1;
+  // Rows with all 9 neighbouring rows inside the lattice (block-uniform): constant offsets per direction.
+  const bool inner = j >= 1 && j <= a.ny - 2 && (D == 2 || (k >= 1 && k <= a.nz - 2));
+  char *const p0 = (char *)(F + x), *const pm = (char *)(F + (rowoff + im)), *const pp = (char *)(F + (rowoff + ip));
+  auto fast_ptr = [&](int q) -> double * {   // koff is in bytes: one 64-bit add per address
+    const int cx = L::cx(q);
+    if (XW && cx != 0 && ((cx == 1 && i == 0) || (cx == -1 && i == a.nx - 1))) return (double *)p0 + (int64_t)q * a.N;
+    return (double *)((cx == 0 ? p0 : (cx == 1 ? pm : pp)) + a.koff[q]);
+  };
+  // General rows: element offset of row (j+dy, k+dz), or -1 when that row lies behind a wall.
+  auto slow_ptr = [&](int q) -> double * {
+    const int cx = L::cx(q), cy = L::cy(q), cz = L::cz(q);
+    int jj = j - cy, kk = k - cz;
+    bool bounce = false;
+    if (cy != 0 && (jj < 0 || jj >= a.ny)) {
+      if (a.bcy) bounce = true;
+      else jj = jj < 0 ? jj + a.ny : jj - a.ny;
+    }
+    if (D == 3 && cz != 0 && (kk < 0 || kk >= a.nz)) {
+      if (a.bcz) bounce = true;
+      else kk = kk < 0 ? kk + a.nz : kk - a.nz;
+    }
+    if (XW && cx != 0 && ((cx == 1 && i == 0) || (cx == -1 && i == a.nx - 1))) bounce = true;
+    const int64_t uo = bounce ? (int64_t)q * a.N + rowoff : (int64_t)opposite(q) * a.N + ((int64_t)kk * a.ny + jj) * a.nx;
+    const int xs = (bounce || cx == 0) ? i : (cx == 1 ? im : ip);
+    return F + (uo + xs);
+  };
+
   double f[Q];
   if (!ODD) {
 #pragma unroll
     for (int q = 0; q < Q; ++q) f[q] = F[(int64_t)q * a.N + x];
+  } else if (inner) {
+#pragma unroll
+    for (int q = 0; q < Q; ++q) f[q] = *fast_ptr(q);
   } else {
 #pragma unroll
-    for (int q = 0; q < Q; ++q) {
-      const int cx = L::cx(q), cy = L::cy(q), cz = L::cz(q);
-      bool bounce = false;
-      int js = j - cy, ks = k - cz;
-      if (cy != 0 && (js < 0 || js >= a.ny)) {
-        if (a.bcy) bounce = true;
-        else js = js < 0 ? js + a.ny : js - a.ny;
-      }
-      if (D == 3 && cz != 0 && (ks < 0 || ks >= a.nz)) {
-        if (a.bcz) bounce = true;
-        else ks = ks < 0 ? ks + a.nz : ks - a.nz;
-      }
-      if (cx != 0 && a.bcx && ((cx == 1 && i == 0) || (cx == -1 && i == a.nx - 1))) bounce = true;
-      const double *base = bounce ? F + ((int64_t)q * a.N + rowoff)
-                                  : F + ((int64_t)opposite(q) * a.N + ((int64_t)ks * a.ny + js) * a.nx);
-      const int xs = (bounce || cx == 0) ? i : (cx == 1 ? im : ip);
-      f[q] = base[xs];
-    }
+    for (int q = 0; q < Q; ++q) f[q] = *slow_ptr(q);
   }
 
   double beta = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
@@ -210,26 +230,12 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_aa_kernel(c
   if (!ODD) {
 #pragma unroll
     for (int q = 0; q < Q; ++q) F[(int64_t)opposite(q) * a.N + x] = f[q];
+  } else if (inner) {
+#pragma unroll
+    for (int q = 0; q < Q; ++q) *fast_ptr(opposite(q)) = f[q];
   } else {
 #pragma unroll
-    for (int q = 0; q < Q; ++q) {
-      const int cx = L::cx(q), cy = L::cy(q), cz = L::cz(q);
-      bool bounce = false;
-      int jt = j + cy, kt = k + cz;
-      if (cy != 0 && (jt < 0 || jt >= a.ny)) {
-        if (a.bcy) bounce = true;
-        else jt = jt < 0 ? jt + a.ny : jt - a.ny;
-      }
-      if (D == 3 && cz != 0 && (kt < 0 || kt >= a.nz)) {
-        if (a.bcz) bounce = true;
-        else kt = kt < 0 ? kt + a.nz : kt - a.nz;
-      }
-      if (cx != 0 && a.bcx && ((cx == 1 && i == a.nx - 1) || (cx == -1 && i == 0))) bounce = true;
-      double *base = bounce ? F + ((int64_t)opposite(q) * a.N + rowoff)
-                            : F + ((int64_t)q * a.N + ((int64_t)kt * a.ny + jt) * a.nx);
-      const int xt = (bounce || cx == 0) ? i : (cx == 1 ? ip : im);
-      base[xt] = f[q];
-    }
+    for (int q = 0; q < Q; ++q) *slow_ptr(opposite(q)) = f[q];
   }
 }
 
@@ -440,14 +446,22 @@ static void launch_cs(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, boo
 
 template <int D, int MINB>
 static void launch_aa(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, bool imb, bool emit, bool odd) {
-#define LBMIMB_AA(I, E, O) collide_stream_aa_kernel<D, I, E, O, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a)
-  if (!imb) {
-    if (odd) LBMIMB_AA(false, false, true); else LBMIMB_AA(false, false, false);
-  } else if (!emit) {
-    if (odd) LBMIMB_AA(true, false, true); else LBMIMB_AA(true, false, false);
+#define LBMIMB_AA(I, E, O, X) collide_stream_aa_kernel<D, I, E, O, X, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a)
+#define LBMIMB_AA_ODD(I, E)                       \
+  do {                                            \
+    if (a.bcx) LBMIMB_AA(I, E, true, true);       \
+    else LBMIMB_AA(I, E, true, false);            \
+  } while (0)
+  if (!odd) {   // the even step touches the own node only: walls do not matter
+    if (!imb) LBMIMB_AA(false, false, false, false);
+    else if (!emit) LBMIMB_AA(true, false, false, false);
+    else LBMIMB_AA(true, true, false, false);
   } else {
-    if (odd) LBMIMB_AA(true, true, true); else LBMIMB_AA(true, true, false);
+    if (!imb) LBMIMB_AA_ODD(false, false);
+    else if (!emit) LBMIMB_AA_ODD(true, false);
+    else LBMIMB_AA_ODD(true, true);
   }
+#undef LBMIMB_AA_ODD
 #undef LBMIMB_AA
 }
 
@@ -474,10 +488,23 @@ lbmimb_status launch_collide_stream(lbmimb_lattice *h, bool emit) {
   const bool imb = h->P > 0;
   if (h->aa) {
     a.fin = a.fout = h->f[0];
-    if (h->g.dim == 2)
-      launch_aa<2, 9>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
-    else
-      launch_aa<3, 6>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
+    for (int q = 0; q < h->Q; ++q) {
+      const int cy = h->g.dim == 2 ? Lat<2>::cy(q) : Lat<3>::cy(q);
+      const int cz = h->g.dim == 2 ? 0 : Lat<3>::cz(q);
+      a.koff[q] = 8 * ((int64_t)opposite(q) * a.N - (int64_t)cy * a.nx - (int64_t)cz * a.nx * a.ny);
+    }
+    const int v = step_variant();   // experiment switch: occupancy target of the AA kernels
+    if (h->g.dim == 2) {
+      if (v == 1) launch_aa<2, 8>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
+      else if (v == 2) launch_aa<2, 10>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
+      else if (v == 3) launch_aa<2, 12>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
+      else if (v == 4) launch_aa<2, 7>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
+      else launch_aa<2, 9>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
+    } else {
+      if (v == 1) launch_aa<3, 6>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
+      else if (v == 2) launch_aa<3, 7>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
+      else launch_aa<3, 5>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
+    }
     LBMIMB_LAUNCH_CHECK(h, "collide_stream_aa_kernel");
     return LBMIMB_OK;
   }

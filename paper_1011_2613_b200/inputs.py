@@ -191,6 +191,68 @@ def c5(n=(128, 512, 128), P=4096, R=5.0, steps=2000, seed=SEED0 + 5, kn=1e-2):
 FULL = {"C1": c1, "C2": c2, "C3": c3, "C4": c4, "C5": c5}
 
 
+# ---------------------------------------------------------------------------------------------
+# Paper-scale, paper-parameter suspensions (PAPER.md:117 and Table 2).
+# Everything below is a parameter the paper prints (tests/golden/paper_table2.txt) or a placement
+# recipe (R19); none of it is arithmetic of the method.
+# ---------------------------------------------------------------------------------------------
+TABLE2 = {
+    2: dict(nu=0.1231, body_force=8.753e-6, g_s=-1.176e-7, mass=54373.0, kn=2686.0, n=(15360, 61440),
+            grid=(540, 2160)),
+    3: dict(nu=0.2462, body_force=4.04e-5, g_s=-4.704e-7, mass=362491.0, kn=17892.0, n=(512, 2016, 512),
+            grid=(32, 126, 32)),
+}
+PAPER_R, PAPER_E, PAPER_VS0, PAPER_RHO_S = 5.0, 0.9, 5.0e-3, 692.3
+
+
+def balance_body_force(g_s, rho_s, phi, rho_g=1.0):
+    """The body force per unit gas mass that balances the weight of the solids ("A body force
+    F_i is exerted on the gas phase to balance the gravity on solid particles"): the gas occupies the
+    fraction 1 - phi of the domain, the solids phi, so  F rho_g (1 - phi) = |g_s| rho_s phi.
+    Table 2's 2D entry 8.753e-6 follows from it with the actual phi = 0.09707."""
+    return abs(g_s) * rho_s * phi / ((1.0 - phi) * rho_g)
+
+
+def _paper_suspension(name, dim, n, grid, seed, jitter=2.0, steps=1000):
+    t = TABLE2[dim]
+    rng = np.random.default_rng(seed)
+    pitch = [n[a] / grid[a] for a in range(dim)]
+    idx = np.meshgrid(*[np.arange(g) for g in grid], indexing="ij")
+    P = int(np.prod(grid))
+    pos = np.stack([(idx[a].reshape(-1) + 0.5) * pitch[a] + rng.uniform(-jitter, jitter, size=P) for a in range(dim)])
+    pos = _quantise(np.mod(pos, np.array(n, dtype=np.float64)[:, None]))
+    d = rng.standard_normal((dim, P))
+    vel = PAPER_VS0 * d / np.sqrt((d * d).sum(axis=0))          # random direction, magnitude v_s0 (PAPER.md:117)
+    radius = np.full(P, PAPER_R)
+    mass = np.full(P, t["mass"])
+    gf = [0.0] * dim
+    gf[1] = t["body_force"]                                      # on the gas, upwards: balances the solids' weight
+    gp = [0.0] * 3
+    gp[1] = t["g_s"]
+    dem = {"kn": t["kn"], "restitution": PAPER_E, "g_particle": tuple(gp), "dt": 1.0}
+    return Workload(name, dim, tuple(n), (0,) * dim, 3.0 * t["nu"] + 0.5, tuple(gf), 8 if dim == 2 else 4, steps,
+                    pos, vel, np.zeros((1 if dim == 2 else 3, P)), radius, mass, dem=dem,
+                    note="PAPER.md:117 / Table 2 suspension, jittered %s lattice of d = 10 particles" %
+                    "x".join(str(g) for g in grid))
+
+
+def p2d(n=None, grid=None, steps=1000, seed=SEED0 + 12):
+    """The paper's 2D suspension: 15360 x 61440 D2Q9, fully periodic, 1,166,400 disks of d = 10
+    (540 x 2160 jittered lattice, solid fraction 0.0971), Table 2 parameters, coupled LBM-IMB-DEM."""
+    t = TABLE2[2]
+    return _paper_suspension("P2D", 2, n or t["n"], grid or t["grid"], seed, steps=steps)
+
+
+def p3d(n=None, grid=None, steps=1000, seed=SEED0 + 13):
+    """The paper's 3D suspension: 512 x 2016 x 512 D3Q19, fully periodic, 129,024 spheres of d = 10
+    (32 x 126 x 32 jittered lattice, solid fraction 0.128), Table 2 parameters, coupled LBM-IMB-DEM."""
+    t = TABLE2[3]
+    return _paper_suspension("P3D", 3, n or t["n"], grid or t["grid"], seed, steps=steps)
+
+
+FULL.update({"P2D": p2d, "P3D": p3d})
+
+
 def reduced(name):
     """Cuts of C1..C5 the oracle finishes in seconds: same recipe and solid
     fraction, lattice sizes that are NOT multiples of the kernel tiles (ragged
@@ -206,6 +268,10 @@ def reduced(name):
     elif name == "C5":
         w = c5(n=(40, 84, 36), P=58, steps=40, kn=50.0)
         w.extra["note"] = "stiffer k_n so that contacts act within the short run"
+    elif name == "P2D":
+        w = p2d(n=(313, 270), grid=(11, 9), steps=30)            # pitch 28.45 x 30 as in the paper's 28.44
+    elif name == "P3D":
+        w = p3d(n=(70, 96, 52), grid=(4, 6, 3), steps=20)        # pitch 17.5 x 16 x 17.3 (paper: 16)
     else:
         raise KeyError(name)
     w.name = name + "-reduced"
