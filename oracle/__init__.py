@@ -257,3 +257,47 @@ def dem_step(dim, n, bc, pos, vel, omega, radius, mass, fh, th, kn, e, gp, dt=1.
     if rc != 0:
         raise RuntimeError("orc_dem_step failed")
     return pos, vel, omega
+
+
+DIAG_LEN = 20
+
+
+def diagnostics(dim, f, eps_cnt=None, eps_den=1, vel=None, radius=None, mass=None, force=None):
+    """Area/volume-averaged suspension diagnostics of PAPER.md:154 and Figs. 5/7 ("area-averaged inter-phase
+    slip velocity V_ry and drag force F_dy"); the paper prints no formula, the reading is DESIGN.md R18:
+      eps_x = eps_cnt_x / eps_den, u = bare velocity of `macros` (R2),
+      gas area       A_g = sum_x (1 - eps_x)
+      gas velocity   U_g = sum_x (1 - eps_x) u_x / A_g
+      solid velocity V_s = sum_p vol_p v_p / sum_p vol_p,  vol_p = pi R^2 (2D) or 4/3 pi R^3 (3D)
+      slip           V_r = U_g - V_s
+      drag           F_d = sum_p F_p / P        (mean hydrodynamic force per particle, eq. (3))
+    plus the fluid mass sum_x rho, fluid momentum sum_x rho u and solid momentum sum_p m_p v_p.
+    Returns a dict and, under "vector", the 20 doubles in the layout of lbmimb_diagnostics:
+      [0] A_g [1] mass [2:5] U_g [5:8] V_s [8:11] V_r [11:14] F_d [14:17] fluid momentum [17:20] solid momentum
+    (unused z components are 0).  Plain numpy sums in fp64."""
+    rho, u = macros(dim, f)
+    if eps_cnt is None:
+        gas = np.ones(rho.shape)
+    else:
+        gas = 1.0 - np.asarray(eps_cnt, dtype=np.float64).reshape(rho.shape) / float(eps_den)
+    out = np.zeros(DIAG_LEN)
+    A_g = gas.sum()
+    out[0] = A_g
+    out[1] = rho.sum()
+    for a in range(dim):
+        out[2 + a] = (gas * u[a]).sum() / A_g
+        out[14 + a] = (rho * u[a]).sum()
+    P = 0 if radius is None else int(np.asarray(radius).shape[0])
+    if P > 0:
+        radius = _f64(radius)
+        vel = _f64(vel).reshape(dim, P)
+        vol = np.pi * radius ** 2 if dim == 2 else 4.0 / 3.0 * np.pi * radius ** 3
+        for a in range(dim):
+            out[5 + a] = (vol * vel[a]).sum() / vol.sum()
+            out[17 + a] = (_f64(mass) * vel[a]).sum()
+            if force is not None:
+                out[11 + a] = _f64(force).reshape(dim, P)[a].sum() / P
+    out[8:11] = out[2:5] - out[5:8]
+    return {"gas_area": out[0], "mass": out[1], "gas_velocity": out[2:2 + dim], "solid_velocity": out[5:5 + dim],
+            "slip": out[8:8 + dim], "drag": out[11:11 + dim], "fluid_momentum": out[14:14 + dim],
+            "solid_momentum": out[17:17 + dim], "vector": out}
