@@ -210,6 +210,21 @@ lbmimb_status lbmimb_dem_step(lbmimb_lattice *h, const lbmimb_dem_params *dem);
 lbmimb_status lbmimb_fetch_fields(lbmimb_lattice *h, int32_t what, const int64_t lo[3],
                                   const int64_t hi[3], void *dst);
 
+/*
+ * Area/volume-averaged suspension diagnostics: the quantities of PAPER.md:154 and Figs. 5/7 ("area-averaged
+ * inter-phase slip velocity V_ry and drag force F_dy").  The paper prints no formula; R18:
+ *   eps_x = eps_cnt_x / S^D (code/255 in TABLE mode), u = bare velocity (R2) of the current distributions,
+ *   A_g = sum_x (1 - eps_x);  U_g = sum_x (1 - eps_x) u_x / A_g;
+ *   V_s = sum_p vol_p v_p / sum_p vol_p, vol_p = pi R^2 | 4/3 pi R^3;  V_r = U_g - V_s;
+ *   F_d = sum_p F_p / P with F_p of the last reduce_particle_forces (0 if none ran since set_particles).
+ * out[LBMIMB_DIAG_LEN] (host): [0] A_g  [1] sum_x rho  [2:5] U_g  [5:8] V_s  [8:11] V_r  [11:14] F_d
+ *   [14:17] sum_x rho u  [17:20] sum_p m_p v_p   (unused z components and all particle entries with P = 0 are 0).
+ * Two-stage device reduction in a fixed order (deterministic for a given lattice).  Synchronous.
+ * ESTATE if particles are set but not mapped.
+ */
+#define LBMIMB_DIAG_LEN 20
+lbmimb_status lbmimb_diagnostics(lbmimb_lattice *h, double *out);
+
 /* Replaces all distributions: f[Q][nz][ny][nx] = f_i(x, t) as LBMIMB_FIELD_F returns them. */
 lbmimb_status lbmimb_set_distributions(lbmimb_lattice *h, const double *f);
 

@@ -27,8 +27,9 @@ EXPORTS = [
     "lbmimb_step", "lbmimb_reduce_particle_forces", "lbmimb_dem_step", "lbmimb_fetch_fields",
     "lbmimb_set_distributions", "lbmimb_set_particles_dev", "lbmimb_reduce_particle_forces_dev",
     "lbmimb_synchronize", "lbmimb_time", "lbmimb_launch_count", "lbmimb_last_error", "lbmimb_version",
-    "lbmimb_set_mapping_mode", "lbmimb_fetch_eps_table",
+    "lbmimb_set_mapping_mode", "lbmimb_fetch_eps_table", "lbmimb_diagnostics",
 ]
+DIAG_LEN = 20
 
 
 class Params(C.Structure):
@@ -81,6 +82,7 @@ def load():
     lib.lbmimb_dem_step.argtypes = [vp, C.POINTER(DemParams)]
     lib.lbmimb_fetch_fields.argtypes = [vp, i32, C.POINTER(i64), C.POINTER(i64), vp]
     lib.lbmimb_set_distributions.argtypes = [vp, vp]
+    lib.lbmimb_diagnostics.argtypes = [vp, vp]
     lib.lbmimb_synchronize.argtypes = [vp]
     lib.lbmimb_time.restype = i64
     lib.lbmimb_time.argtypes = [vp]
@@ -268,6 +270,15 @@ class Lattice:
         f = _f64(f)
         assert f.size == self.Q * self.n[0] * self.n[1] * self.n[2]
         _check(self.lib.lbmimb_set_distributions(self.h, _hp(f)))
+
+    def diagnostics(self):
+        """The 20 doubles of lbmimb_diagnostics and the same named views as a dict."""
+        out = np.zeros(DIAG_LEN)
+        _check(self.lib.lbmimb_diagnostics(self.h, _hp(out)))
+        D = self.dim
+        return {"gas_area": out[0], "mass": out[1], "gas_velocity": out[2:2 + D], "solid_velocity": out[5:5 + D],
+                "slip": out[8:8 + D], "drag": out[11:11 + D], "fluid_momentum": out[14:14 + D],
+                "solid_momentum": out[17:17 + D], "vector": out}
 
     def synchronize(self):
         _check(self.lib.lbmimb_synchronize(self.h))

@@ -55,7 +55,7 @@ static bool valid_params(const lbmimb_params *p, int64_t maxp) {
 
 // One place that decides the device memory layout; used for sizing and for carving.
 struct Layout {
-  uint64_t off_f[2], off_eps, off_pid, off_s, off_beta, off_contested, off_counters, off_table;
+  uint64_t off_f[2], off_eps, off_pid, off_s, off_beta, off_contested, off_counters, off_table, off_diag;
   uint64_t off_pos, off_vel, off_omega, off_radius, off_mass, off_force, off_torque, off_fc, off_prec;
   uint64_t off_count, off_start, off_fill, off_items, off_cell_of, off_bsums;
   uint64_t total;
@@ -86,6 +86,7 @@ static Layout make_layout(const lbmimb_params *p, int64_t maxp) {
   L.off_contested = take((uint64_t)L.contested_cap * 8);
   L.off_counters = take(64);
   L.off_table = take((uint64_t)eps_table_entries(p->dim));
+  L.off_diag = take((uint64_t)(kDiagBlocksMax * 8 + 32) * 8);
   L.off_pos = take((uint64_t)3 * pm * 8);
   L.off_vel = take((uint64_t)3 * pm * 8);
   L.off_omega = take((uint64_t)3 * pm * 8);
@@ -198,6 +199,8 @@ lbmimb_status lbmimb_create_lattice(const lbmimb_params *params, int64_t max_par
   h->contested_cap = L.contested_cap;
   h->counters = (int32_t *)(h->ws + L.off_counters);
   h->eps_table = (uint8_t *)(h->ws + L.off_table);
+  h->diag_partial = (double *)(h->ws + L.off_diag);
+  h->diag_out = h->diag_partial + (size_t)kDiagBlocksMax * 8;
   h->map_mode = LBMIMB_MAP_SAMPLING;
   h->table_R = -1.0;
   h->pos = (double *)(h->ws + L.off_pos);
@@ -571,6 +574,19 @@ lbmimb_status lbmimb_fetch_fields(lbmimb_lattice *h, int32_t what, const int64_t
   st = body();
   if (tmp) cudaFree(tmp);
   return st;
+}
+
+lbmimb_status lbmimb_diagnostics(lbmimb_lattice *h, double *out) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (!out) return fail(LBMIMB_EINVAL, "out is NULL");
+  if (h->P > 0 && !h->map_valid) return fail(LBMIMB_ESTATE, "particle map is stale: call lbmimb_map_particles first");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  const double den = h->map_mode == LBMIMB_MAP_TABLE ? (double)LBMIMB_TABLE_DEN : (double)h->SD;
+  if ((st = launch_diagnostics(h, den)) != LBMIMB_OK) return st;
+  LBMIMB_CUDA(cudaMemcpyAsync(out, h->diag_out, LBMIMB_DIAG_LEN * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+  return LBMIMB_OK;
 }
 
 lbmimb_status lbmimb_set_distributions(lbmimb_lattice *h, const double *f) {

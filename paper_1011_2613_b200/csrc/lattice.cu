@@ -382,6 +382,125 @@ __global__ void fetch_kernel(const FetchArgs a, const Geom g) {
   }
 }
 
+// ---------------------------------------------------------------------------
+// Suspension diagnostics (Figs. 5/7; R18): deterministic two-stage reduction.
+// Stage 1: every thread sums its grid-stride nodes in a fixed order, the block reduces by a fixed tree
+// and writes 8 partial sums: gas area, mass, (1-eps) u [3], rho u [3].
+// Stage 2 (one block): partials in block order, then the particle sums, then the derived quantities.
+// ---------------------------------------------------------------------------
+constexpr int kDiagThreads = 256;
+constexpr int kDiagK = 8;
+
+__device__ __forceinline__ double diag_block_sum(double v, double *sh) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  __syncthreads();
+  if (l == 0) sh[w] = v;
+  __syncthreads();
+  double r = 0.0;
+  if (threadIdx.x == 0) {
+    for (int k = 0; k < kDiagThreads / 32; ++k) r += sh[k];
+  }
+  return r;   // valid on thread 0
+}
+
+template <int D>
+__global__ void __launch_bounds__(kDiagThreads) diag_nodes_kernel(const double *__restrict__ fst, const uint8_t *__restrict__ eps_cnt,
+                                                                  const Geom g, int layout, int have_particles,
+                                                                  double eps_den, double *__restrict__ partial) {
+  using L = Lat<D>;
+  __shared__ double sh[kDiagThreads / 32];
+  double acc[kDiagK];
+#pragma unroll
+  for (int c = 0; c < kDiagK; ++c) acc[c] = 0.0;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; x < g.N; x += stride) {
+    const int i = (int)(x % g.nx);
+    const int64_t r = x / g.nx;
+    const int j = (int)(r % g.ny);
+    const int k = (int)(r / g.ny);
+    double f[L::Q];
+    gather_node<D>(fst, g, layout, i, j, k, f);
+    double rho = 0.0, m[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+    for (int q = 0; q < L::Q; ++q) {
+      rho += f[q];
+      m[0] += L::cx(q) * f[q];
+      m[1] += L::cy(q) * f[q];
+      m[2] += L::cz(q) * f[q];
+    }
+    const double gas = have_particles ? 1.0 - (double)eps_cnt[x] / eps_den : 1.0;
+    acc[0] += gas;
+    acc[1] += rho;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      acc[2 + c] += gas * (m[c] / rho);
+      acc[5 + c] += m[c];
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < kDiagK; ++c) {
+    const double t = diag_block_sum(acc[c], sh);
+    if (threadIdx.x == 0) partial[(int64_t)blockIdx.x * kDiagK + c] = t;
+  }
+}
+
+// out[20]: [0] A_g [1] mass [2:5] U_g [5:8] V_s [8:11] V_r [11:14] F_d [14:17] fluid momentum [17:20] solid momentum
+template <int D>
+__global__ void __launch_bounds__(kDiagThreads) diag_final_kernel(const double *__restrict__ partial, int nblocks, int64_t P,
+                                                                  const double *__restrict__ vel,
+                                                                  const double *__restrict__ radius,
+                                                                  const double *__restrict__ mass,
+                                                                  const double *__restrict__ force,
+                                                                  double *__restrict__ out) {
+  __shared__ double sh[kDiagThreads / 32];
+  __shared__ double tot[kDiagK + 10];
+  for (int c = 0; c < kDiagK; ++c) {
+    double v = 0.0;
+    for (int b = threadIdx.x; b < nblocks; b += kDiagThreads) v += partial[(int64_t)b * kDiagK + c];
+    const double t = diag_block_sum(v, sh);
+    if (threadIdx.x == 0) tot[c] = t;
+  }
+  // particles: [8] sum vol, [9..11] sum vol v, [12..14] sum m v, [15..17] sum F
+  double pa[10];
+#pragma unroll
+  for (int c = 0; c < 10; ++c) pa[c] = 0.0;
+  const double kPi = 3.14159265358979323846;
+  for (int64_t p = threadIdx.x; p < P; p += kDiagThreads) {
+    const double R = radius[p];
+    const double vol = D == 2 ? kPi * (R * R) : (4.0 / 3.0 * kPi) * (R * R * R);
+    pa[0] += vol;
+#pragma unroll
+    for (int c = 0; c < D; ++c) {
+      const double v = vel[(int64_t)c * P + p];
+      pa[1 + c] += vol * v;
+      pa[4 + c] += mass[p] * v;
+      pa[7 + c] += force[(int64_t)c * P + p];
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < 10; ++c) {
+    const double t = diag_block_sum(pa[c], sh);
+    if (threadIdx.x == 0) tot[kDiagK + c] = t;
+  }
+  if (threadIdx.x == 0) {
+    for (int c = 0; c < 20; ++c) out[c] = 0.0;
+    out[0] = tot[0];
+    out[1] = tot[1];
+    for (int c = 0; c < D; ++c) {
+      out[2 + c] = tot[2 + c] / tot[0];
+      out[14 + c] = tot[5 + c];
+      if (P > 0) {
+        out[5 + c] = tot[9 + c] / tot[8];
+        out[11 + c] = tot[15 + c] / (double)P;
+        out[17 + c] = tot[12 + c];
+      }
+      out[8 + c] = out[2 + c] - out[5 + c];
+    }
+  }
+}
+
 static int grid_for(int64_t n, int threads, int cap = 148 * 16) {
   int64_t b = (n + threads - 1) / threads;
   if (b < 1) b = 1;
@@ -551,6 +670,26 @@ lbmimb_status launch_fetch(lbmimb_lattice *h, int what, const int64_t lo[3], con
   else
     fetch_kernel<3><<<grid_for(a.box, 256), 256, 0, h->stream>>>(a, h->g);
   LBMIMB_LAUNCH_CHECK(h, "fetch_kernel");
+  return LBMIMB_OK;
+}
+
+lbmimb_status launch_diagnostics(lbmimb_lattice *h, double eps_den) {
+  const int layout = h->aa ? (h->aa_swapped ? kLayoutSwapped : kLayoutNatural) : kLayoutPull;
+  const int nb = grid_for(h->g.N, kDiagThreads, kDiagBlocksMax);
+  const double *fst = h->f[h->cur];
+  const int hp = h->P > 0;
+  if (h->g.dim == 2) {
+    diag_nodes_kernel<2><<<nb, kDiagThreads, 0, h->stream>>>(fst, h->eps_cnt, h->g, layout, hp, eps_den, h->diag_partial);
+    LBMIMB_LAUNCH_CHECK(h, "diag_nodes_kernel");
+    diag_final_kernel<2><<<1, kDiagThreads, 0, h->stream>>>(h->diag_partial, nb, h->P, h->vel, h->radius, h->mass,
+                                                           h->force, h->diag_out);
+  } else {
+    diag_nodes_kernel<3><<<nb, kDiagThreads, 0, h->stream>>>(fst, h->eps_cnt, h->g, layout, hp, eps_den, h->diag_partial);
+    LBMIMB_LAUNCH_CHECK(h, "diag_nodes_kernel");
+    diag_final_kernel<3><<<1, kDiagThreads, 0, h->stream>>>(h->diag_partial, nb, h->P, h->vel, h->radius, h->mass,
+                                                           h->force, h->diag_out);
+  }
+  LBMIMB_LAUNCH_CHECK(h, "diag_final_kernel");
   return LBMIMB_OK;
 }
 

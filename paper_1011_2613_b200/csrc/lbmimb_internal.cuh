@@ -109,6 +109,8 @@ struct lbmimb_lattice {
   int64_t *contested; // mapping fix-up list
   int64_t contested_cap;
   int32_t *counters;  // [0] contested count, [1] overflow flag, [2] bad-particle flag
+  double *diag_partial;  // [kDiagBlocksMax][8] stage-1 sums of lbmimb_diagnostics
+  double *diag_out;      // [20]
 
   // particles (SoA, device)
   int64_t Pmax, P;
@@ -158,5 +160,7 @@ lbmimb_status ensure_eps_table(lbmimb_lattice *h);
 int64_t eps_table_entries(int dim);
 lbmimb_status launch_reduce(lbmimb_lattice *h);
 lbmimb_status launch_dem(lbmimb_lattice *h, const lbmimb_dem_params *dem);
+lbmimb_status launch_diagnostics(lbmimb_lattice *h, double eps_den);
+constexpr int kDiagBlocksMax = 148 * 8;
 
 }  // namespace lbmimb
