@@ -128,6 +128,10 @@ def oracle_sample(name, target_s=15.0, max_steps=50):
         w = inputs.c2(n=(1024, 1024), P=3500, steps=1)
     elif name == "C5":
         w = inputs.c5(n=(128, 128, 128), P=1024, steps=1)
+    elif name == "P3D":
+        w = inputs.p3d(n=(256, 96, 256), grid=(16, 6, 16), steps=1)      # the paper's pitch of 16
+    elif name == "P2D":
+        w = inputs.p2d(n=(2048, 1024), grid=(72, 36), steps=1)           # the paper's pitch of 28.44
     else:
         raise KeyError(name)
     f = orc.init(w.dim, w.n)
@@ -169,7 +173,8 @@ def run_reference(args):
         if it >= args.warmup:
             vals.append(v)
     value = float(np.mean(vals))
-    w = {"C3": (256, 1008, 256), "C4": (8192, 32768), "C2": (1024, 4096), "C5": (128, 512, 128)}[args.workload]
+    w = {"C3": (256, 1008, 256), "C4": (8192, 32768), "C2": (1024, 4096), "C5": (128, 512, 128),
+         "P2D": (15360, 61440), "P3D": (512, 2016, 512)}[args.workload]
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": None, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -186,15 +191,19 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--workload", default="C3", choices=["C2", "C3", "C4", "C5"])
+    ap.add_argument("--workload", default="C3", choices=["C2", "C3", "C4", "C5", "P2D", "P3D"],
+                    help="C2..C5 = BASELINE.json configs; P2D / P3D = the paper's own suspensions at full size "
+                         "(PAPER.md:117, Table 2; coupled with DEM; P3D needs --streaming aa, the default for it)")
     ap.add_argument("--impl", default="lbmimb", choices=["lbmimb", "reference"])
     ap.add_argument("--map-mode", default="sampling", choices=["sampling", "table"],
                     help="a1 variant: sub-cell sampling (BASELINE.json configs) or the paper's table look-up")
-    ap.add_argument("--streaming", default="ab", choices=["ab", "aa"],
+    ap.add_argument("--streaming", default=None, choices=["ab", "aa"],
                     help="a2 variant: pull with two arrays (A-B) or in-place AA-pattern on one array")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
+    if args.streaming is None:      # 2 x 80.3 GB of distributions do not fit one B200: P3D runs in place
+        args.streaming = "aa" if args.workload == "P3D" else "ab"
     if args.impl == "reference":
         return run_reference(args)
     if args.warmup < 3:
@@ -297,6 +306,16 @@ def main():
                "d2h_bytes_per_step": int(d2h), "ms_per_step": e_ms / args.steps}
 
     lat.synchronize()
+    diag = diag_ms = None
+    if dem:                        # the Figs. 5/7 time-series sample: one device reduction per output step
+        lat.map_particles()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        dd = lat.diagnostics()
+        b.record()
+        torch.cuda.synchronize()
+        diag_ms = a.elapsed_time(b)
+        diag = {"slip_y": float(dd["slip"][1]), "drag_y": float(dd["drag"][1]), "t": lat.time()}
     if rank != 0:
         lat.close()
         replicas.shutdown()
@@ -330,7 +349,8 @@ def main():
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
             "breakdown_ms": {"map_particles": float(seg[:, 0].mean()), "step": kern_ms,
                              "reduce_particle_forces": float(seg[:, 2].mean()),
-                             "dem_step": float(seg[:, 3].mean()) if dem else 0.0},
+                             "dem_step": float(seg[:, 3].mean()) if dem else 0.0, "diagnostics_once": diag_ms},
+            "diagnostics": diag,
             "version": lb.version()}
     print(json.dumps(line))
     lat.close()

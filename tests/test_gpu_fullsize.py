@@ -50,10 +50,10 @@ def _fetch_wrapped(lat, lb, what, lo, size, n, bc):
     return out
 
 
-def _check_boxes(orc, lb, w, nsteps, boxes):
+def _check_boxes(orc, lb, w, nsteps, boxes, streaming=0):
     R = float(w.radius.max())
     rim = nsteps + int(2 * R) + 3
-    lat = lb.from_workload(w)
+    lat = lb.from_workload(w, streaming=streaming)
     lat.map_particles()
     lat.step(nsteps)
     gF, gT = lat.reduce_particle_forces()
@@ -124,4 +124,39 @@ def test_c4_full_size_sampled_boxes_and_mass(orc, lb):
     for j0 in range(0, 32768, 4096):                              # slab-wise: 268 M nodes
         total += lat.fetch_fields(lb.FIELD_RHO, (0, j0, 0), (8192, j0 + 4096, 1)).sum()
     assert abs(total - m0) / m0 < 1e-12
+    lat.close()
+
+
+def test_p3d_paper_size_in_place_sampled_boxes_mass_and_diagnostics(orc, lb):
+    """The paper's 3D suspension at its own size (512 x 2016 x 512, 129,024 spheres of d = 10, PAPER.md:117,
+    Table 2 parameters) on one GPU with AA-pattern in-place streaming (80.3 GB of distributions)."""
+    w = inputs.p3d()
+    n = 5                                                             # odd: the array is in its swapped layout
+    boxes = [((200, 1000, 300), (72, 72, 72), (0, 0, 0)),
+             ((-30, -25, 480), (70, 72, 72), (0, 0, 0)),              # across the x, y and z seams
+             ((470, 1990, -20), (72, 70, 70), (0, 0, 0))]
+    lat, worst = _check_boxes(orc, lb, w, n, boxes, streaming=lb.STREAM_AA)
+    d = lat.diagnostics()
+    m0 = float(w.nodes)
+    assert abs(d["mass"] - m0) / m0 < 1e-12                           # mass conserved (P2)
+    vol = 4.0 / 3.0 * np.pi * 125.0
+    # sampled gas volume = N - sum of the particle volumes, to the sampling accuracy of P10 (0.5 %)
+    assert abs((m0 - d["gas_area"]) / (w.P * vol) - 1) < 5e-3
+    assert np.abs(d["solid_velocity"] - w.vel.mean(axis=1)).max() < 1e-15
+    assert lat.time() == n
+    lat.close()
+
+
+def test_p2d_paper_size_sampled_boxes_and_mass(orc, lb):
+    """The paper's 2D suspension at its own size (15360 x 61440, 1,166,400 disks of d = 10), in place."""
+    w = inputs.p2d()
+    n = 6
+    boxes = [((7000, 30000), (100, 100), (0, 0)),
+             ((-40, -35), (100, 96), (0, 0)),
+             ((15360 - 60, 61440 - 50), (110, 100), (0, 0))]
+    lat, worst = _check_boxes(orc, lb, w, n, boxes, streaming=lb.STREAM_AA)
+    d = lat.diagnostics()
+    m0 = float(w.nodes)
+    assert abs(d["mass"] - m0) / m0 < 1e-12
+    assert abs((m0 - d["gas_area"]) / (w.P * np.pi * 25.0) - 1) < 5e-3
     lat.close()
