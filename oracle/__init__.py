@@ -34,6 +34,9 @@ def lib():
         _lib.orc_map_table.restype = C.c_int
         _lib.orc_dem_step.restype = C.c_int
         _lib.orc_num_threads.restype = C.c_int
+        _lib.orc_verlet_build.restype = C.c_int64
+        _lib.orc_verlet_max_disp2.restype = C.c_double
+        _lib.orc_dem_step_verlet.restype = C.c_int
     return _lib
 
 
@@ -256,6 +259,78 @@ def dem_step(dim, n, bc, pos, vel, omega, radius, mass, fh, th, kn, e, gp, dt=1.
                             C.c_double(e), _p(gp3), C.c_double(dt))
     if rc != 0:
         raise RuntimeError("orc_dem_step failed")
+    return pos, vel, omega
+
+
+def verlet_build(dim, n, bc, pos, radius, skin):
+    """The neighbour lists by their definition (R19): CSR (start[P+1] int64, items int32), j ascending."""
+    n3, bc3 = _n3(n), _bc3(bc)
+    pos = _f64(pos).reshape(dim, -1)
+    P = pos.shape[1]
+    start = np.zeros(P + 1, dtype=np.int64)
+    cap = max(64 * P, 1)
+    while True:
+        items = np.zeros(cap, dtype=np.int32)
+        t = int(lib().orc_verlet_build(C.c_int(dim), _p(n3), _p(bc3), C.c_int64(P), _p(pos), _p(_f64(radius)),
+                                       C.c_double(skin), _p(start), _p(items), C.c_int64(cap)))
+        if t >= 0:
+            return start, items[:t].copy()
+        cap = -t
+
+
+def verlet_max_disp2(dim, n, bc, pos, pos_ref):
+    n3, bc3 = _n3(n), _bc3(bc)
+    pos = _f64(pos).reshape(dim, -1)
+    ref = _f64(pos_ref).reshape(dim, -1)
+    return float(lib().orc_verlet_max_disp2(C.c_int(dim), _p(n3), _p(bc3), C.c_int64(pos.shape[1]), _p(pos), _p(ref)))
+
+
+def contact_forces_list(dim, n, bc, pos, vel, radius, mass, kn, e, start, items):
+    n3, bc3 = _n3(n), _bc3(bc)
+    pos = _f64(pos).reshape(dim, -1)
+    vel = _f64(vel).reshape(dim, -1)
+    P = pos.shape[1]
+    fc = np.zeros((dim, P))
+    start = np.ascontiguousarray(start, dtype=np.int64)
+    items = np.ascontiguousarray(items, dtype=np.int32)
+    lib().orc_contact_forces_list(C.c_int(dim), _p(n3), _p(bc3), C.c_int64(P), _p(pos), _p(vel), _p(_f64(radius)),
+                                  _p(_f64(mass)), C.c_double(kn), C.c_double(e), _p(start), _p(items), _p(fc))
+    return fc
+
+
+class VerletState:
+    """What the neighbour-list variant of the DEM step carries from step to step (R19)."""
+
+    def __init__(self, dim, P, skin, every, cap_per_particle=128):
+        self.skin, self.every = float(skin), int(every)
+        self.state = np.zeros(3, dtype=np.int64)          # valid, age (steps), number of builds
+        self.x_ref = np.zeros((dim, P))
+        self.start = np.zeros(P + 1, dtype=np.int64)
+        self.items = np.zeros(max(cap_per_particle * P, 1), dtype=np.int32)
+
+    valid = property(lambda self: bool(self.state[0]))
+    age = property(lambda self: int(self.state[1]))
+    builds = property(lambda self: int(self.state[2]))
+
+    def lists(self):
+        return self.start.copy(), self.items[:self.start[-1]].copy()
+
+
+def dem_step_verlet(dim, n, bc, pos, vel, omega, radius, mass, fh, th, kn, e, gp, vs, dt=1.0):
+    """One DEM step (R11) with the neighbour list `vs` (VerletState, updated in place) and the rebuild rule
+    R19; returns new (pos, vel, omega) copies."""
+    n3, bc3, gp3 = _n3(n), _bc3(bc), _g3(gp)
+    pos = _f64(pos).reshape(dim, -1).copy()
+    vel = _f64(vel).reshape(dim, -1).copy()
+    omega = _f64(omega).reshape(1 if dim == 2 else 3, -1).copy()
+    P = pos.shape[1]
+    rc = lib().orc_dem_step_verlet(C.c_int(dim), _p(n3), _p(bc3), C.c_int64(P), _p(pos), _p(vel), _p(omega),
+                                   _p(_f64(radius)), _p(_f64(mass)), _p(_f64(fh)), _p(_f64(th)), C.c_double(kn),
+                                   C.c_double(e), _p(gp3), C.c_double(dt), C.c_double(vs.skin),
+                                   C.c_int64(vs.every), _p(vs.state), _p(vs.x_ref), _p(vs.start), _p(vs.items),
+                                   C.c_int64(vs.items.size))
+    if rc != 0:
+        raise RuntimeError("orc_dem_step_verlet failed (list capacity?)")
     return pos, vel, omega
 
 

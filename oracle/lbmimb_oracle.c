@@ -31,6 +31,9 @@
  *     brute-forced on tiny inputs only),
  *   - orc_dem_step's wall contact (R10) and the coupling order (R11):
  *     "parity unpinned" beyond the two-sphere bounce pins.
+ * The Verlet-list functions (orc_verlet_*, orc_dem_step_verlet, R19)
+ * are pinned in tests/test_oracle_verlet_pins.py (hand lists, lattice shell
+ * counts, bitwise equality with the all-pairs trajectory, rebuild counts).
  */
 #include <math.h>
 #include <stdint.h>
@@ -675,6 +678,196 @@ int orc_dem_step(int dim, const int64_t *n, const int32_t *bc, int64_t P,
       omega[id] = omega[id] + dt * th[id] / I;
     }
   }
+  free(fc);
+  return 0;
+}
+
+/* ------------------------------------------------------------------------ */
+/* Verlet neighbour list ("The neighbor-list of each solid      */
+/* particle is established roughly every 100th time step"), reading R19.      */
+/* ------------------------------------------------------------------------ */
+
+/*
+ * The list of particle i, by its definition (brute force over all j):
+ *   L(i) = { j != i : |r_i - r_j|^2 < (R_i + R_j + skin)^2 }   (minimum image),
+ * j ascending.  dist2 is summed left to right without FMA.  start[P+1] (CSR
+ * offsets) and items[cap] are outputs.  Returns the number of entries, or
+ * -(needed) when cap is too small (nothing useful written then).
+ */
+int64_t orc_verlet_build(int dim, const int64_t *n, const int32_t *bc, int64_t P,
+                         const double *x, const double *radius, double skin,
+                         int64_t *start /*[P+1]*/, int32_t *items, int64_t cap) {
+  int64_t total = 0;
+  for (int64_t i = 0; i < P; ++i) {
+    start[i] = total;
+    for (int64_t j = 0; j < P; ++j) {
+      if (j == i) continue;
+      double dist2 = 0.0;
+      for (int a = 0; a < dim; ++a) {
+        double d = x[(int64_t)a * P + i] - x[(int64_t)a * P + j];
+        if (bc[a] == 0) d = min_image(d, n[a]);
+        dist2 += d * d;
+      }
+      double Rc = (radius[i] + radius[j]) + skin;
+      if (dist2 < Rc * Rc) {
+        if (total < cap) items[total] = (int32_t)j;
+        ++total;
+      }
+    }
+  }
+  start[P] = total;
+  return total <= cap ? total : -total;
+}
+
+/* Largest squared displacement (minimum image) of any particle from the
+ * positions x_ref at which the list was built. */
+double orc_verlet_max_disp2(int dim, const int64_t *n, const int32_t *bc, int64_t P,
+                            const double *x, const double *x_ref) {
+  double m = 0.0;
+  for (int64_t i = 0; i < P; ++i) {
+    double d2 = 0.0;
+    for (int a = 0; a < dim; ++a) {
+      double d = x[(int64_t)a * P + i] - x_ref[(int64_t)a * P + i];
+      if (bc[a] == 0) d = min_image(d, n[a]);
+      d2 += d * d;
+    }
+    if (d2 > m) m = d2;
+  }
+  return m;
+}
+
+/* Contact forces as in contact_forces(), but particle i only looks at the
+ * members of its list (in list order); walls as before. */
+static void contact_forces_list(int dim, const int64_t *n, const int32_t *bc,
+                                int64_t P, const double *x, const double *v,
+                                const double *radius, const double *mass,
+                                double kn, double e, const int64_t *start,
+                                const int32_t *items, double *fc) {
+  for (int64_t i = 0; i < P; ++i) {
+    double F[3] = {0.0, 0.0, 0.0};
+    for (int64_t t = start[i]; t < start[i + 1]; ++t) {
+      int64_t j = items[t];
+      double d[3] = {0.0, 0.0, 0.0}, dist2 = 0.0;
+      for (int a = 0; a < dim; ++a) {
+        d[a] = x[(int64_t)a * P + i] - x[(int64_t)a * P + j];
+        if (bc[a] == 0) d[a] = min_image(d[a], n[a]);
+        dist2 += d[a] * d[a];
+      }
+      double Rs = radius[i] + radius[j];
+      if (dist2 >= Rs * Rs) continue;
+      double dist = sqrt(dist2);
+      double delta = Rs - dist;
+      if (!(delta > 0.0)) continue;
+      double meff = mass[i] * mass[j] / (mass[i] + mass[j]);
+      double eta = orc_damping(kn, e, meff);
+      double nrm[3], vn = 0.0;
+      for (int a = 0; a < dim; ++a) {
+        nrm[a] = d[a] / dist;
+        vn += (v[(int64_t)a * P + i] - v[(int64_t)a * P + j]) * nrm[a];
+      }
+      for (int a = 0; a < dim; ++a)
+        F[a] += kn * delta * nrm[a] - eta * vn * nrm[a];
+    }
+    for (int a = 0; a < dim; ++a) {
+      if (bc[a] == 0) continue;
+      double eta = orc_damping(kn, e, mass[i]);
+      double xa = x[(int64_t)a * P + i], va = v[(int64_t)a * P + i];
+      double delta = radius[i] - (xa + 0.5);
+      if (delta > 0.0) F[a] += kn * delta * 1.0 - eta * (va * 1.0) * 1.0;
+      delta = radius[i] - (((double)n[a] - 0.5) - xa);
+      if (delta > 0.0) F[a] += kn * delta * (-1.0) - eta * (va * -1.0) * (-1.0);
+    }
+    for (int a = 0; a < dim; ++a) fc[(int64_t)a * P + i] = F[a];
+  }
+}
+
+void orc_contact_forces_list(int dim, const int64_t *n, const int32_t *bc, int64_t P,
+                             const double *x, const double *v, const double *radius,
+                             const double *mass, double kn, double e,
+                             const int64_t *start, const int32_t *items, double *fc) {
+  contact_forces_list(dim, n, bc, P, x, v, radius, mass, kn, e, start, items, fc);
+}
+
+
+/*
+ * Rebuild rule (R19), applied before EVERY contact evaluation (two per step):
+ * rebuild at the current positions when there is no list yet, or the list is
+ * `every` or more steps old ("roughly every 100th time step"), or
+ * some particle has moved farther than skin/2 from where it was when the list
+ * was built (squared displacement > (skin/2)^2).  The last condition is what
+ * makes the list exact: while it holds for nobody, two particles that touch
+ * now (distance < R_i + R_j) were closer than R_i + R_j + skin at build time,
+ * so they are in each other's lists and the forces equal the all-pairs sum.
+ * state[0] = list valid, state[1] = age in steps, state[2] = number of builds.
+ * Returns 0, or -1 when the list does not fit cap.
+ */
+static int verlet_ensure(int dim, const int64_t *n, const int32_t *bc, int64_t P,
+                         const double *x, const double *radius, double skin,
+                         int64_t every, int64_t *state, double *x_ref,
+                         int64_t *start, int32_t *items, int64_t cap) {
+  int need = !state[0] || state[1] >= every;
+  if (!need) {
+    double h = 0.5 * skin;
+    need = orc_verlet_max_disp2(dim, n, bc, P, x, x_ref) > h * h;
+  }
+  if (!need) return 0;
+  if (orc_verlet_build(dim, n, bc, P, x, radius, skin, start, items, cap) < 0) return -1;
+  memcpy(x_ref, x, sizeof(double) * (size_t)(dim * P));
+  state[0] = 1;
+  state[1] = 0;
+  state[2] += 1;
+  return 0;
+}
+
+/*
+ * a4 with the neighbour list: the step of orc_dem_step (R11), with both contact
+ * evaluations summing over the lists kept in (state, x_ref, start, items) and
+ * the rebuild rule above in front of each.  The list ages by one per step.
+ */
+int orc_dem_step_verlet(int dim, const int64_t *n, const int32_t *bc, int64_t P,
+                        double *pos, double *vel, double *omega, const double *radius,
+                        const double *mass, const double *fh, const double *th,
+                        double kn, double e, const double *gp, double dt,
+                        double skin, int64_t every, int64_t *state, double *x_ref,
+                        int64_t *start, int32_t *items, int64_t cap) {
+  double *fc = (double *)malloc(sizeof(double) * (size_t)(dim * P));
+  if (!fc) return -1;
+  if (verlet_ensure(dim, n, bc, P, pos, radius, skin, every, state, x_ref, start, items, cap)) {
+    free(fc);
+    return -1;
+  }
+  contact_forces_list(dim, n, bc, P, pos, vel, radius, mass, kn, e, start, items, fc);
+  for (int64_t p = 0; p < P; ++p)
+    for (int a = 0; a < dim; ++a) {
+      int64_t id = (int64_t)a * P + p;
+      double a0 = (fh[id] + fc[id]) / mass[p] + gp[a];
+      vel[id] = vel[id] + 0.5 * dt * a0;
+      double xn = pos[id] + dt * vel[id];
+      if (bc[a] == 0) {
+        if (xn >= (double)n[a]) xn -= (double)n[a];
+        if (xn < 0.0) xn += (double)n[a];
+      }
+      pos[id] = xn;
+    }
+  if (verlet_ensure(dim, n, bc, P, pos, radius, skin, every, state, x_ref, start, items, cap)) {
+    free(fc);
+    return -1;
+  }
+  contact_forces_list(dim, n, bc, P, pos, vel, radius, mass, kn, e, start, items, fc);
+  for (int64_t p = 0; p < P; ++p) {
+    for (int a = 0; a < dim; ++a) {
+      int64_t id = (int64_t)a * P + p;
+      double a1 = (fh[id] + fc[id]) / mass[p] + gp[a];
+      vel[id] = vel[id] + 0.5 * dt * a1;
+    }
+    double I = (dim == 3 ? 0.4 : 0.5) * mass[p] * radius[p] * radius[p];
+    int nt = dim == 2 ? 1 : 3;
+    for (int a = 0; a < nt; ++a) {
+      int64_t id = (int64_t)a * P + p;
+      omega[id] = omega[id] + dt * th[id] / I;
+    }
+  }
+  state[1] += 1;
   free(fc);
   return 0;
 }
