@@ -203,6 +203,40 @@ lbmimb_status lbmimb_reduce_particle_forces(lbmimb_lattice *h, double *force, do
 lbmimb_status lbmimb_dem_step(lbmimb_lattice *h, const lbmimb_dem_params *dem);
 
 /*
+ * Contact search of a4 (lbmimb_set_neighbor_mode).
+ * CELLS (default): a cell list over the particles, rebuilt whenever positions change.
+ * VERLET: the paper's scheme ("The neighbor-list of each solid particle is established
+ *   roughly every 100th time step"; it "uses more memory to trade for less searching work").  The paper
+ *   prints neither the list's cut-off nor what triggers a rebuild; R19:
+ *     L(i) = { j != i : |r_i - r_j|^2 < ((R_i + R_j) + skin)^2 }  (minimum image; fp64, no FMA, the squared
+ *     distance summed x, y, z left to right), j ascending;
+ *     before EVERY contact evaluation (two per dem_step) the lists are rebuilt at the current positions
+ *     if there is no valid list (first use, or set_particles since), or the list is `every` or more
+ *     dem_steps old, or some particle's squared displacement (minimum image, same arithmetic) from its
+ *     position at the last build exceeds (skin/2)^2.  While no displacement exceeds skin/2, every
+ *     touching pair is in the lists, so the contact forces equal the all-pairs sum of R8 exactly.
+ *   The decision is taken on the device (no host synchronisation); contact sums run over the lists in
+ *   ascending j.  List storage is allocated by the library (cudaMalloc, outside the workspace) from
+ *   packing bounds on the particles' radii: slots per particle K = (2 (2 R_max + skin)/(1.5 R_min) + 1)^D;
+ *   particle sets that overlap so deeply that a list (or a cell of the build grid) overflows make
+ *   lbmimb_synchronize / lbmimb_fetch_neighbor_list return ESTATE.
+ * set_neighbor_mode: skin > 0 and every >= 1 for VERLET (ignored for CELLS); drops any existing list.
+ * EINVAL on an unknown mode or bad skin / every.
+ */
+enum { LBMIMB_NEIGHBOR_CELLS = 0, LBMIMB_NEIGHBOR_VERLET = 1 };
+lbmimb_status lbmimb_set_neighbor_mode(lbmimb_lattice *h, int32_t mode, double skin, int64_t every);
+/*
+ * Copies the current neighbour lists to the host as CSR: start[P+1] (int64 offsets), items[start[P]]
+ * (int32, j ascending inside each list); capacity = entries available at items.  info[4] (may be NULL):
+ * [0] 1 if a valid list exists (else start is all zero), [1] its age in dem_steps, [2] number of list
+ * builds since set_neighbor_mode, [3] total entries start[P].  Synchronous.
+ * ESTATE if VERLET mode is not selected or a list overflowed; EINVAL if capacity < info[3] (info is still
+ * filled, nothing else is written).
+ */
+lbmimb_status lbmimb_fetch_neighbor_list(lbmimb_lattice *h, int64_t *start, int32_t *items, int64_t capacity,
+                                         int64_t *info);
+
+/*
  * a5. Copies a field of the sub-box [lo, hi) (node coordinates, x first; 2D: lo[2]=0, hi[2]=1)
  * into dst, laid out [component][k][j][i] over the box, x fastest.  `what` is one of
  * LBMIMB_FIELD_*.  Synchronous.  EPS_CNT / PID need a valid map, S needs a step after it.

@@ -18,6 +18,7 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE = range(5)
 FIELD_F, FIELD_RHO, FIELD_U, FIELD_EPS_CNT, FIELD_PID, FIELD_S = range(6)
 MAP_SAMPLING, MAP_TABLE = 0, 1
 STREAM_AB, STREAM_AA = 0, 1
+NEIGHBOR_CELLS, NEIGHBOR_VERLET = 0, 1
 TABLE_DEN = 255
 TABLE_SHAPE = {2: (128, 32), 3: (128, 16, 16)}      # LBMIMB_TABLE_ND/NT_* of include/lbmimb.h
 
@@ -28,6 +29,7 @@ EXPORTS = [
     "lbmimb_set_distributions", "lbmimb_set_particles_dev", "lbmimb_reduce_particle_forces_dev",
     "lbmimb_synchronize", "lbmimb_time", "lbmimb_launch_count", "lbmimb_last_error", "lbmimb_version",
     "lbmimb_set_mapping_mode", "lbmimb_fetch_eps_table", "lbmimb_diagnostics",
+    "lbmimb_set_neighbor_mode", "lbmimb_fetch_neighbor_list",
 ]
 DIAG_LEN = 20
 
@@ -80,6 +82,8 @@ def load():
     lib.lbmimb_reduce_particle_forces.argtypes = [vp, vp, vp]
     lib.lbmimb_reduce_particle_forces_dev.argtypes = [vp, vp, vp]
     lib.lbmimb_dem_step.argtypes = [vp, C.POINTER(DemParams)]
+    lib.lbmimb_set_neighbor_mode.argtypes = [vp, i32, C.c_double, i64]
+    lib.lbmimb_fetch_neighbor_list.argtypes = [vp, vp, vp, i64, vp]
     lib.lbmimb_fetch_fields.argtypes = [vp, i32, C.POINTER(i64), C.POINTER(i64), vp]
     lib.lbmimb_set_distributions.argtypes = [vp, vp]
     lib.lbmimb_diagnostics.argtypes = [vp, vp]
@@ -252,6 +256,22 @@ class Lattice:
         for a in range(3):
             d.g_particle[a] = g[a]
         _check(self.lib.lbmimb_dem_step(self.h, C.byref(d)))
+
+    def set_neighbor_mode(self, mode, skin=0.0, every=0):
+        _check(self.lib.lbmimb_set_neighbor_mode(self.h, mode, float(skin), int(every)))
+
+    def fetch_neighbor_list(self):
+        """(start[P+1] int64, items int32, info) with info = dict(valid, age, builds)."""
+        P = self.num_particles()
+        start = np.zeros(P + 1, dtype=np.int64)
+        info = np.zeros(4, dtype=np.int64)
+        items = np.zeros(max(16 * P, 1), dtype=np.int32)
+        st = self.lib.lbmimb_fetch_neighbor_list(self.h, _hp(start), _hp(items), items.size, _hp(info))
+        if st == EINVAL and info[3] > items.size:      # grow to the size the library reported
+            items = np.zeros(int(info[3]), dtype=np.int32)
+            st = self.lib.lbmimb_fetch_neighbor_list(self.h, _hp(start), _hp(items), items.size, _hp(info))
+        _check(st)
+        return start, items[:int(start[-1])].copy(), {"valid": bool(info[0]), "age": int(info[1]), "builds": int(info[2])}
 
     def fetch_fields(self, what, lo=None, hi=None, out=None):
         lo = [0, 0, 0] if lo is None else list(lo) + [0] * (3 - len(lo))

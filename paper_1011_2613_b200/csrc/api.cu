@@ -132,7 +132,7 @@ using namespace lbmimb;
 extern "C" {
 
 const char *lbmimb_last_error(void) { return g_err; }
-const char *lbmimb_version(void) { return "lbmimb 0.2 (sm_100a, fused collide-stream: pull A-B and in-place AA)"; }
+const char *lbmimb_version(void) { return "lbmimb 0.3 (sm_100a, fused collide-stream: pull A-B and in-place AA; DEM: cell list or Verlet lists)"; }
 
 uint64_t lbmimb_workspace_bytes(const lbmimb_params *params, int64_t max_particles) {
   if (!valid_params(params, max_particles)) return 0;
@@ -257,6 +257,7 @@ lbmimb_status lbmimb_destroy_lattice(lbmimb_lattice *h) {
   if (!h) return LBMIMB_OK;
   cudaSetDevice(h->prm.device);
   cudaStreamSynchronize(h->stream);
+  neighbor_list_release(h);
   if (h->owns_ws) cudaFree(h->ws);
   delete h;
   return LBMIMB_OK;
@@ -268,6 +269,8 @@ static lbmimb_status after_particles_changed(lbmimb_lattice *h, bool positions) 
     h->cl_valid = false;
     h->s_valid = false;
     h->forces_valid = false;
+    lbmimb_status st = neighbor_list_invalidate(h);
+    if (st != LBMIMB_OK) return st;
   }
   if (h->P > 0) return launch_pack_records(h);
   return LBMIMB_OK;
@@ -406,6 +409,13 @@ lbmimb_status lbmimb_synchronize(lbmimb_lattice *h) {
   int32_t c[4];
   LBMIMB_CUDA(cudaMemcpy(c, h->counters, sizeof(c), cudaMemcpyDeviceToHost));
   if (c[1] != 0) return fail(LBMIMB_ESTATE, "particle map: contested-node list overflowed (particles overlap too much)");
+  if (h->nl.mem) {
+    int32_t s[8];
+    LBMIMB_CUDA(cudaMemcpy(s, h->nl.state, sizeof(s), cudaMemcpyDeviceToHost));
+    if (s[4] != 0 || s[5] != 0)
+      return fail(LBMIMB_ESTATE, "neighbour list: %s overflowed (particles overlap more deeply than the sizing allows)",
+                  s[4] ? "a particle's list" : "a cell of the build grid");
+  }
   return LBMIMB_OK;
 }
 
@@ -528,6 +538,65 @@ lbmimb_status lbmimb_dem_step(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
   h->map_valid = false;
   h->s_valid = false;
   return launch_pack_records(h);
+}
+
+lbmimb_status lbmimb_set_neighbor_mode(lbmimb_lattice *h, int32_t mode, double skin, int64_t every) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (mode != LBMIMB_NEIGHBOR_CELLS && mode != LBMIMB_NEIGHBOR_VERLET)
+    return fail(LBMIMB_EINVAL, "unknown neighbour mode %d", mode);
+  if (mode == LBMIMB_NEIGHBOR_VERLET && (!(skin > 0.0) || !std::isfinite(skin) || every < 1))
+    return fail(LBMIMB_EINVAL, "neighbour lists need skin > 0 and every >= 1");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+  neighbor_list_release(h);
+  h->nl.mode = mode;
+  h->nl.skin = mode == LBMIMB_NEIGHBOR_VERLET ? skin : 0.0;
+  h->nl.every = mode == LBMIMB_NEIGHBOR_VERLET ? (int)(every > 0x7fffffff ? 0x7fffffff : every) : 0;
+  return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_fetch_neighbor_list(lbmimb_lattice *h, int64_t *start, int32_t *items, int64_t capacity,
+                                         int64_t *info) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (!start || (capacity > 0 && !items) || capacity < 0) return fail(LBMIMB_EINVAL, "NULL output / negative capacity");
+  if (h->nl.mode != LBMIMB_NEIGHBOR_VERLET) return fail(LBMIMB_ESTATE, "neighbour-list mode is not selected");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+  const int64_t P = h->P;
+  int32_t s[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  if (h->nl.mem) LBMIMB_CUDA(cudaMemcpy(s, h->nl.state, sizeof(s), cudaMemcpyDeviceToHost));
+  if (s[4] != 0 || s[5] != 0)
+    return fail(LBMIMB_ESTATE, "neighbour list: %s overflowed (particles overlap more deeply than the sizing allows)",
+                s[4] ? "a particle's list" : "a cell of the build grid");
+  if (info) {
+    info[0] = s[0];
+    info[1] = s[1];
+    info[2] = s[2];
+    info[3] = 0;
+  }
+  if (!s[0] || P == 0) {   // no valid list: all lists empty
+    for (int64_t p = 0; p <= P; ++p) start[p] = 0;
+    return LBMIMB_OK;
+  }
+  // marshalling only: the device keeps K slots per particle (slot-major); the ABI speaks CSR
+  std::vector<int32_t> cnt((size_t)P), slots((size_t)h->nl.K * P);
+  LBMIMB_CUDA(cudaMemcpy(cnt.data(), h->nl.count, (size_t)P * 4, cudaMemcpyDeviceToHost));
+  LBMIMB_CUDA(cudaMemcpy2D(slots.data(), (size_t)P * 4, h->nl.items, (size_t)h->nl.Pcap * 4, (size_t)P * 4,
+                           (size_t)h->nl.K, cudaMemcpyDeviceToHost));
+  int64_t total = 0;
+  for (int64_t p = 0; p < P; ++p) total += cnt[p];
+  if (info) info[3] = total;
+  if (capacity < total)
+    return fail(LBMIMB_EINVAL, "items holds %lld entries, the lists have %lld", (long long)capacity, (long long)total);
+  int64_t o = 0;
+  for (int64_t p = 0; p < P; ++p) {
+    start[p] = o;
+    for (int k = 0; k < cnt[p]; ++k) items[o++] = slots[(size_t)k * P + p];
+  }
+  start[P] = o;
+  return LBMIMB_OK;
 }
 
 lbmimb_status lbmimb_fetch_fields(lbmimb_lattice *h, int32_t what, const int64_t lo[3], const int64_t hi[3], void *dst) {

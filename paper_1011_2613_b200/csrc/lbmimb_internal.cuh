@@ -83,6 +83,26 @@ struct CellList {
   int64_t ncells_max;
 };
 
+// Verlet neighbour lists of a4 (R19).  Library-allocated (sized from the radii).
+//   items [K][Pcap] slot-major (thread i reading slot k is coalesced), count [Pcap], x_ref [3][Pcap];
+//   build grid: cells of edge >= 2 R_max + skin with C slots each (gcount [ncells], gitems [ncells][C]);
+//   state (device): [0] valid [1] age in dem_steps [2] builds [3] displacement flag
+//                   [4] list overflow [5] grid overflow.
+struct NeighborList {
+  int mode;            // LBMIMB_NEIGHBOR_*
+  double skin;
+  int every;
+  void *mem;           // one cudaMalloc holding everything below
+  int64_t Pcap;
+  int K, C;
+  int32_t *items, *count, *state, *gcount, *gitems;
+  double *x_ref;
+  int nc[3];
+  double inv_e[3];
+  int64_t ncells;
+  double rmax, rmin;   // radii the storage was sized for
+};
+
 }  // namespace lbmimb
 
 struct lbmimb_lattice {
@@ -121,6 +141,7 @@ struct lbmimb_lattice {
   double table_R;
   lbmimb::CellList cl;
   bool cl_valid;
+  lbmimb::NeighborList nl;
 
   bool map_valid;     // eps_cnt/pid match the particle positions
   bool s_valid;       // s holds the exchange vectors of the last step under the current map
@@ -160,6 +181,9 @@ lbmimb_status ensure_eps_table(lbmimb_lattice *h);
 int64_t eps_table_entries(int dim);
 lbmimb_status launch_reduce(lbmimb_lattice *h);
 lbmimb_status launch_dem(lbmimb_lattice *h, const lbmimb_dem_params *dem);
+lbmimb_status neighbor_list_prepare(lbmimb_lattice *h);   // (re)allocates the list storage for the current radii
+void neighbor_list_release(lbmimb_lattice *h);
+lbmimb_status neighbor_list_invalidate(lbmimb_lattice *h);  // positions were replaced
 lbmimb_status launch_diagnostics(lbmimb_lattice *h, double eps_den);
 constexpr int kDiagBlocksMax = 148 * 8;
 

@@ -85,6 +85,8 @@ __device__ __forceinline__ int cell_coord(double x, const CellGeom &cg, int a) {
   return c;
 }
 
+#include "verlet.cuh"
+
 __global__ void cl_count_kernel(CellGeom cg, int64_t P, const double *__restrict__ pos, int32_t *__restrict__ cell_of,
                                 int32_t *__restrict__ count) {
   const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -713,7 +715,8 @@ lbmimb_status launch_reduce(lbmimb_lattice *h) {
 }
 
 // ---------------------------------------------------------------------------
-// a4: DEM, eq. (4)-(5) with the readings R8-R11.
+// a4: DEM, eq. (4)-(5) with the readings R8-R11.  Contact search: the cell list above, or the
+// Verlet neighbour lists of verlet.cuh (R19).
 // ---------------------------------------------------------------------------
 struct DemArgs {
   Geom g;
@@ -726,7 +729,57 @@ struct DemArgs {
   double kn, ce;  // eta = ce * sqrt(kn * m_eff), ce = -2 ln e / sqrt(pi^2 + ln^2 e)
   double gp[3];
   double dt;
+  // Verlet mode only (else nl_state == nullptr)
+  int32_t *nl_state;
+  const int32_t *nl_items, *nl_count;
+  const double *nl_xref;
+  int64_t nl_Pcap;
+  int nl_every;
+  double nl_h2;   // (skin/2)^2
 };
+
+// force of particle j on particle i (R8): k_n delta n_ij - eta (v_ij . n_ij) n_ij, added to F
+template <int D>
+__device__ __forceinline__ void pair_force(const DemArgs &a, const int *n, const double *xi, const double *vi,
+                                           double Ri, double mi, int j, double *F) {
+  double d[3] = {0.0, 0.0, 0.0}, dist2 = 0.0;
+  for (int q = 0; q < D; ++q) {
+    d[q] = xi[q] - a.pos[(int64_t)q * a.P + j];
+    const bool per = q == 0 ? !a.g.bcx : (q == 1 ? !a.g.bcy : !a.g.bcz);
+    if (per) d[q] = min_image_d(d[q], n[q]);
+    dist2 += d[q] * d[q];
+  }
+  const double Rs = Ri + a.radius[j];
+  if (dist2 >= Rs * Rs) return;
+  const double dist = sqrt(dist2);
+  const double delta = Rs - dist;
+  if (!(delta > 0.0)) return;
+  const double mj = a.mass[j];
+  const double meff = mi * mj / (mi + mj);
+  const double eta = a.ce * sqrt(a.kn * meff);
+  double nrm[3], vn = 0.0;
+  for (int q = 0; q < D; ++q) {
+    nrm[q] = d[q] / dist;
+    vn += (vi[q] - a.vel[(int64_t)q * a.P + j]) * nrm[q];
+  }
+  const double mag = a.kn * delta - eta * vn;
+  for (int q = 0; q < D; ++q) F[q] += mag * nrm[q];
+}
+
+// walls: planes at -1/2 and n-1/2 of a wall axis, m_eff = m_i (R10)
+template <int D>
+__device__ __forceinline__ void wall_force(const DemArgs &a, const int *n, const double *xi, const double *vi,
+                                           double Ri, double mi, double *F) {
+  for (int q = 0; q < D; ++q) {
+    const bool wall = q == 0 ? a.g.bcx : (q == 1 ? a.g.bcy : a.g.bcz);
+    if (!wall) continue;
+    const double eta = a.ce * sqrt(a.kn * mi);
+    double delta = Ri - (xi[q] + 0.5);
+    if (delta > 0.0) F[q] += a.kn * delta - eta * vi[q];
+    delta = Ri - (((double)n[q] - 0.5) - xi[q]);
+    if (delta > 0.0) F[q] += -a.kn * delta - eta * vi[q];
+  }
+}
 
 template <int D>
 __global__ void dem_contact_kernel(const DemArgs a) {
@@ -758,69 +811,73 @@ __global__ void dem_contact_kernel(const DemArgs a) {
         for (int it = a.start[c]; it < a.start[c + 1]; ++it) {
           const int j = a.items[it];
           if (j == (int)i) continue;
-          double d[3] = {0.0, 0.0, 0.0}, dist2 = 0.0;
-          for (int q = 0; q < D; ++q) {
-            d[q] = xi[q] - a.pos[(int64_t)q * a.P + j];
-            const bool per = q == 0 ? !a.g.bcx : (q == 1 ? !a.g.bcy : !a.g.bcz);
-            if (per) d[q] = min_image_d(d[q], n[q]);
-            dist2 += d[q] * d[q];
-          }
-          const double Rs = Ri + a.radius[j];
-          if (dist2 >= Rs * Rs) continue;
-          const double dist = sqrt(dist2);
-          const double delta = Rs - dist;
-          if (!(delta > 0.0)) continue;
-          const double mj = a.mass[j];
-          const double meff = mi * mj / (mi + mj);
-          const double eta = a.ce * sqrt(a.kn * meff);
-          double nrm[3], vn = 0.0;
-          for (int q = 0; q < D; ++q) {
-            nrm[q] = d[q] / dist;
-            vn += (vi[q] - a.vel[(int64_t)q * a.P + j]) * nrm[q];
-          }
-          const double mag = a.kn * delta - eta * vn;
-          for (int q = 0; q < D; ++q) F[q] += mag * nrm[q];
+          pair_force<D>(a, n, xi, vi, Ri, mi, j, F);
         }
       }
-  // walls: planes at -1/2 and n-1/2 of a wall axis, m_eff = m_i (R10)
-  for (int q = 0; q < D; ++q) {
-    const bool wall = q == 0 ? a.g.bcx : (q == 1 ? a.g.bcy : a.g.bcz);
-    if (!wall) continue;
-    const double eta = a.ce * sqrt(a.kn * mi);
-    double delta = Ri - (xi[q] + 0.5);
-    if (delta > 0.0) F[q] += a.kn * delta - eta * vi[q];
-    delta = Ri - (((double)n[q] - 0.5) - xi[q]);
-    if (delta > 0.0) F[q] += -a.kn * delta - eta * vi[q];
-  }
+  wall_force<D>(a, n, xi, vi, Ri, mi, F);
   for (int q = 0; q < D; ++q) a.fc[(int64_t)q * a.P + i] = F[q];
 }
 
-// first half: v += dt/2 a0; x += dt v (wrapped into [0,n) on periodic axes)
+// the same sums over the neighbour lists (ascending j).  Runs right after the three predicated
+// build kernels of this evaluation, so one thread commits their outcome to the list state.
+template <int D>
+__global__ void dem_contact_list_kernel(const DemArgs a) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0 && nl_need(a.nl_state, a.nl_every)) {
+    a.nl_state[NL_VALID] = 1;
+    a.nl_state[NL_AGE] = 0;
+    a.nl_state[NL_BUILDS] += 1;
+    a.nl_state[NL_DISP] = 0;
+  }
+  if (i >= a.P) return;
+  const int n[3] = {a.g.nx, a.g.ny, a.g.nz};
+  double xi[3], vi[3], F[3] = {0.0, 0.0, 0.0};
+  for (int c = 0; c < D; ++c) {
+    xi[c] = a.pos[(int64_t)c * a.P + i];
+    vi[c] = a.vel[(int64_t)c * a.P + i];
+  }
+  const double Ri = a.radius[i], mi = a.mass[i];
+  const int cnt = a.nl_count[i];
+  for (int k = 0; k < cnt; ++k) {
+    const int j = a.nl_items[(int64_t)k * a.nl_Pcap + i];
+    pair_force<D>(a, n, xi, vi, Ri, mi, j, F);
+  }
+  wall_force<D>(a, n, xi, vi, Ri, mi, F);
+  for (int q = 0; q < D; ++q) a.fc[(int64_t)q * a.P + i] = F[q];
+}
+
+// first half: v += dt/2 a0; x += dt v (wrapped into [0,n) on periodic axes).  Verlet mode: raises
+// the displacement flag of the rebuild rule when this particle is now farther than skin/2 from
+// where it was when the lists were built.
 template <int D>
 __global__ void dem_kick_drift_kernel(const DemArgs a) {
   const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= a.P) return;
   const int n[3] = {a.g.nx, a.g.ny, a.g.nz};
+  const bool per[3] = {!a.g.bcx, !a.g.bcy, !a.g.bcz};
   const double m = a.mass[p];
+  double xn[3] = {0.0, 0.0, 0.0};
   for (int q = 0; q < D; ++q) {
     const int64_t id = (int64_t)q * a.P + p;
     const double a0 = (a.force[id] + a.fc[id]) / m + a.gp[q];
     const double v = a.vel[id] + 0.5 * a.dt * a0;
     a.vel[id] = v;
     double x = a.pos[id] + a.dt * v;
-    const bool per = q == 0 ? !a.g.bcx : (q == 1 ? !a.g.bcy : !a.g.bcz);
-    if (per) {
+    if (per[q]) {
       if (x >= (double)n[q]) x -= (double)n[q];
       if (x < 0.0) x += (double)n[q];
     }
     a.pos[id] = x;
+    xn[q] = x;
   }
+  if (a.nl_state != nullptr && verlet_disp2<D>(xn, a.nl_xref, a.nl_Pcap, p, n, per) > a.nl_h2) a.nl_state[NL_DISP] = 1;
 }
 
-// second half: v += dt/2 a1; omega += dt T_h / I
+// second half: v += dt/2 a1; omega += dt T_h / I.  Verlet mode: the lists age by one step.
 template <int D>
 __global__ void dem_kick_kernel(const DemArgs a) {
   const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p == 0 && a.nl_state != nullptr) a.nl_state[NL_AGE] += 1;
   if (p >= a.P) return;
   const double m = a.mass[p], R = a.radius[p];
   for (int q = 0; q < D; ++q) {
@@ -836,10 +893,127 @@ __global__ void dem_kick_kernel(const DemArgs a) {
   }
 }
 
+// ---- neighbour-list storage (library-allocated; sized from packing bounds on the radii) ----
+void neighbor_list_release(lbmimb_lattice *h) {
+  if (h->nl.mem) cudaFree(h->nl.mem);
+  h->nl.mem = nullptr;
+  h->nl.items = h->nl.count = h->nl.state = h->nl.gcount = h->nl.gitems = nullptr;
+  h->nl.x_ref = nullptr;
+}
+
+lbmimb_status neighbor_list_invalidate(lbmimb_lattice *h) {
+  if (h->nl.mem) LBMIMB_CUDA(cudaMemsetAsync(h->nl.state + NL_VALID, 0, 4, h->stream));
+  return LBMIMB_OK;
+}
+
+lbmimb_status neighbor_list_prepare(lbmimb_lattice *h) {
+  NeighborList &nl = h->nl;
+  if (nl.mem && nl.rmax == h->rmax && nl.rmin == h->rmin) return LBMIMB_OK;
+  neighbor_list_release(h);
+  const int D = h->g.dim;
+  const int n[3] = {h->g.nx, h->g.ny, h->g.nz};
+  const double cutoff = (2.0 * h->rmax + nl.skin) * (1.0 + 1e-9);  // margin: cell binning is rounded
+  const double dmin = 1.5 * h->rmin;  // closest centres the sizing allows for (soft spheres overlap)
+  double edge_max = 0.0;
+  nl.ncells = 1;
+  for (int a = 0; a < 3; ++a) {
+    nl.nc[a] = 1;
+    nl.inv_e[a] = 1.0;
+    if (a >= D) continue;
+    nl.nc[a] = (int)floor((double)n[a] / cutoff);
+    if (nl.nc[a] < 1) nl.nc[a] = 1;
+    nl.inv_e[a] = (double)nl.nc[a] / (double)n[a];
+    nl.ncells *= nl.nc[a];
+    const double e = (double)n[a] / (double)nl.nc[a];
+    if (nl.nc[a] > 1 && e > edge_max) edge_max = e;
+  }
+  if (edge_max == 0.0) edge_max = cutoff;
+  const int64_t pm = h->Pmax > 0 ? h->Pmax : 1;
+  double c = 2.0 * pow(edge_max / dmin + 1.0, (double)D);
+  double k = pow(2.0 * cutoff / dmin + 1.0, (double)D);
+  if (c > (double)pm) c = (double)pm;
+  if (k > (double)(pm > 1 ? pm - 1 : 1)) k = (double)(pm > 1 ? pm - 1 : 1);
+  nl.C = (int)ceil(c);
+  nl.K = (int)ceil(k);
+  nl.Pcap = pm;
+  auto al = [](uint64_t v) { return (v + 255) & ~(uint64_t)255; };
+  const uint64_t b_items = al((uint64_t)nl.K * pm * 4), b_count = al((uint64_t)pm * 4), b_state = 256;
+  const uint64_t b_gcount = al((uint64_t)nl.ncells * 4), b_gitems = al((uint64_t)nl.ncells * nl.C * 4);
+  const uint64_t b_xref = al((uint64_t)3 * pm * 8);
+  const uint64_t total = b_items + b_count + b_state + b_gcount + b_gitems + b_xref;
+  if (total > ((uint64_t)16 << 30))
+    return fail(LBMIMB_ENOMEM, "neighbour lists would need %.1f GB (K = %d slots per particle, R_min = %g, R_max = %g)",
+                (double)total / 1073741824.0, nl.K, h->rmin, h->rmax);
+  void *mem = nullptr;
+  cudaError_t e = cudaMalloc(&mem, total);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc(neighbour lists)");
+  char *q = (char *)mem;
+  nl.mem = mem;
+  nl.items = (int32_t *)q;   q += b_items;
+  nl.count = (int32_t *)q;   q += b_count;
+  nl.state = (int32_t *)q;   q += b_state;
+  nl.gcount = (int32_t *)q;  q += b_gcount;
+  nl.gitems = (int32_t *)q;  q += b_gitems;
+  nl.x_ref = (double *)q;
+  nl.rmax = h->rmax;
+  nl.rmin = h->rmin;
+  LBMIMB_CUDA(cudaMemsetAsync(nl.state, 0, 256, h->stream));
+  return LBMIMB_OK;
+}
+
+static VerletArgs verlet_args(const lbmimb_lattice *h) {
+  const NeighborList &nl = h->nl;
+  VerletArgs v;
+  v.g = h->g;
+  v.cg.dim = h->g.dim;
+  for (int a = 0; a < 3; ++a) {
+    v.cg.nc[a] = nl.nc[a];
+    v.cg.inv_e[a] = nl.inv_e[a];
+  }
+  v.cg.periodic[0] = !h->g.bcx;
+  v.cg.periodic[1] = !h->g.bcy;
+  v.cg.periodic[2] = !h->g.bcz;
+  v.P = h->P;
+  v.Pcap = nl.Pcap;
+  v.ncells = nl.ncells;
+  v.pos = h->pos;
+  v.radius = h->radius;
+  v.skin = nl.skin;
+  v.every = nl.every;
+  v.K = nl.K;
+  v.C = nl.C;
+  v.items = nl.items;
+  v.count = nl.count;
+  v.state = nl.state;
+  v.gcount = nl.gcount;
+  v.gitems = nl.gitems;
+  v.x_ref = nl.x_ref;
+  return v;
+}
+
+// the three predicated build kernels in front of a contact evaluation (rebuild rule of R19)
+template <int D>
+static lbmimb_status verlet_ensure(lbmimb_lattice *h, const VerletArgs &v) {
+  int nbc = blocks_for(v.ncells, 256);
+  if (nbc > 148 * 8) nbc = 148 * 8;
+  verlet_clear_kernel<<<nbc, 256, 0, h->stream>>>(v);
+  LBMIMB_LAUNCH_CHECK(h, "verlet_clear_kernel");
+  verlet_bin_kernel<D><<<blocks_for(h->P, 256), 256, 0, h->stream>>>(v);
+  LBMIMB_LAUNCH_CHECK(h, "verlet_bin_kernel");
+  verlet_list_kernel<D><<<blocks_for(h->P, 128), 128, 0, h->stream>>>(v);
+  LBMIMB_LAUNCH_CHECK(h, "verlet_list_kernel");
+  return LBMIMB_OK;
+}
+
 template <int D>
 static lbmimb_status dem_impl(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
   lbmimb_status st;
-  if (!h->cl_valid && (st = build_cell_list(h)) != LBMIMB_OK) return st;
+  const bool verlet = h->nl.mode == LBMIMB_NEIGHBOR_VERLET;
+  if (verlet) {
+    if ((st = neighbor_list_prepare(h)) != LBMIMB_OK) return st;
+  } else if (!h->cl_valid && (st = build_cell_list(h)) != LBMIMB_OK) {
+    return st;
+  }
   DemArgs a;
   a.g = h->g;
   a.P = h->P;
@@ -858,8 +1032,37 @@ static lbmimb_status dem_impl(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
   a.ce = -2.0 * le / sqrt(M_PI * M_PI + le * le);
   for (int c = 0; c < 3; ++c) a.gp[c] = dem->g_particle[c];
   a.dt = dem->dt;
+  a.nl_state = nullptr;
+  a.nl_items = a.nl_count = nullptr;
+  a.nl_xref = nullptr;
+  a.nl_Pcap = 0;
+  a.nl_every = 0;
+  a.nl_h2 = 0.0;
   const int nb = blocks_for(h->P, 128);
   a.cg = cell_geom(h);
+  if (verlet) {
+    const VerletArgs v = verlet_args(h);
+    a.nl_state = h->nl.state;
+    a.nl_items = h->nl.items;
+    a.nl_count = h->nl.count;
+    a.nl_xref = h->nl.x_ref;
+    a.nl_Pcap = h->nl.Pcap;
+    a.nl_every = h->nl.every;
+    const double hs = 0.5 * h->nl.skin;
+    a.nl_h2 = hs * hs;
+    if ((st = verlet_ensure<D>(h, v)) != LBMIMB_OK) return st;
+    dem_contact_list_kernel<D><<<nb, 128, 0, h->stream>>>(a);
+    LBMIMB_LAUNCH_CHECK(h, "dem_contact_list_kernel");
+    dem_kick_drift_kernel<D><<<nb, 128, 0, h->stream>>>(a);
+    LBMIMB_LAUNCH_CHECK(h, "dem_kick_drift_kernel");
+    if ((st = verlet_ensure<D>(h, v)) != LBMIMB_OK) return st;
+    dem_contact_list_kernel<D><<<nb, 128, 0, h->stream>>>(a);
+    LBMIMB_LAUNCH_CHECK(h, "dem_contact_list_kernel");
+    dem_kick_kernel<D><<<nb, 128, 0, h->stream>>>(a);
+    LBMIMB_LAUNCH_CHECK(h, "dem_kick_kernel");
+    h->cl_valid = false;   // the particles moved and no cell list was built at the new positions
+    return LBMIMB_OK;
+  }
   dem_contact_kernel<D><<<nb, 128, 0, h->stream>>>(a);
   LBMIMB_LAUNCH_CHECK(h, "dem_contact_kernel");
   dem_kick_drift_kernel<D><<<nb, 128, 0, h->stream>>>(a);
