@@ -199,6 +199,11 @@ def main():
                     help="a1 variant: sub-cell sampling (BASELINE.json configs) or the paper's table look-up")
     ap.add_argument("--streaming", default=None, choices=["ab", "aa"],
                     help="a2 variant: pull with two arrays (A-B) or in-place AA-pattern on one array")
+    ap.add_argument("--neighbor-mode", default="cells", choices=["cells", "verlet"],
+                    help="a4 variant (coupled workloads C5 / P2D / P3D): cell list rebuilt every step, or the paper's "
+                         "neighbour lists (PAPER.md:69, DESIGN.md R19)")
+    ap.add_argument("--skin", type=float, default=1.0, help="neighbour-list skin in lattice units")
+    ap.add_argument("--every", type=int, default=100, help="neighbour lists are at most this many steps old")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -219,6 +224,8 @@ def main():
     lat = lb.from_workload(w, device=local, map_mode=lb.MAP_TABLE if args.map_mode == "table" else lb.MAP_SAMPLING,
                            streaming=lb.STREAM_AA if args.streaming == "aa" else lb.STREAM_AB)
     dem = w.dem
+    if args.neighbor_mode == "verlet":
+        lat.set_neighbor_mode(lb.NEIGHBOR_VERLET, args.skin, args.every)
     Q = w.Q
     bytes_per_node = 2 * Q * 8 + 1 + 4
     N = w.nodes
@@ -316,6 +323,7 @@ def main():
         torch.cuda.synchronize()
         diag_ms = a.elapsed_time(b)
         diag = {"slip_y": float(dd["slip"][1]), "drag_y": float(dd["drag"][1]), "t": lat.time()}
+    nl_info = lat.fetch_neighbor_list()[2] if (dem and args.neighbor_mode == "verlet") else None
     if rank != 0:
         lat.close()
         replicas.shutdown()
@@ -343,14 +351,17 @@ def main():
             "config": {"workload": args.workload, "lattice": list(w.n), "Q": Q, "particles": w.P, "tau": w.tau,
                        "bc": list(w.bc), "map_mode": args.map_mode, "streaming": args.streaming,
                        "step": "map_particles + step(1) + reduce_particle_forces" +
-                       (" + dem_step" if dem else ""), "parallelism": "replicas x%d" % world,
+                       (" + dem_step" if dem else ""),
+                       "neighbor_mode": (args.neighbor_mode + (" skin=%g every=%d" % (args.skin, args.every)
+                                                               if args.neighbor_mode == "verlet" else "")) if dem else None,
+                       "parallelism": "replicas x%d" % world,
                        "l2": "inputs (%.1f GB of distributions) exceed the 126 MB L2; no flush needed" %
                        ((1 if args.streaming == "aa" else 2) * Q * N * 8 / 1e9)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
             "breakdown_ms": {"map_particles": float(seg[:, 0].mean()), "step": kern_ms,
                              "reduce_particle_forces": float(seg[:, 2].mean()),
                              "dem_step": float(seg[:, 3].mean()) if dem else 0.0, "diagnostics_once": diag_ms},
-            "diagnostics": diag,
+            "diagnostics": diag, "neighbor_list": nl_info,
             "version": lb.version()}
     print(json.dumps(line))
     lat.close()
