@@ -116,21 +116,32 @@ __device__ __forceinline__ void group_sync() {
   else __syncthreads();
 }
 
+// Dense walk of the bounding box.  A sphere fills a third of its box, so classifying every box node
+// (phase A of map_particles_kernel) spends most of its time on nodes that are plainly empty.  Here every
+// row (j,k) of the box first gets the interval of columns that can pass the "not surely empty" test,
+//   max(|dx| - hs, 0)^2 <= r2_none - ny_^2 - nz_^2   <=>   |dx| <= hs + sqrt(...)   (+ margin: a superset),
+// the interval lengths of a chunk of G rows are scanned, and phase A walks the concatenated intervals with the
+// SAME per-node classification as before; phase B is unchanged.  Rows of a particle whose box crosses the
+// periodic seam in x keep their full length (no unwrapped coordinate to take the interval in).
 template <int D, int G, int SFIX>
 __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
   constexpr int groups = 128 / G;
-  constexpr int CH = G >= 64 ? kMapChunk : 8 * G;   // bounding-box nodes per pass of a group
+  constexpr int CH = G >= 64 ? kMapChunk : 8 * G;   // candidate nodes per pass of a group
+  constexpr int NW = G >= 32 ? G / 32 : 1;
+  constexpr int SW = G < 32 ? G : 32;               // shuffle width of a group's scan
   __shared__ double sub[256];
   __shared__ int list[groups][CH];
   __shared__ int nlist[groups];
-  __shared__ int smax;
+  __shared__ int pre[groups][G + 1];   // exclusive prefix of the interval lengths of this chunk of rows
+  __shared__ int beg[groups][G];       // first box column of each row's interval
+  __shared__ int wtot[groups][NW];
   for (int t = threadIdx.x; t < a.S; t += blockDim.x) sub[t] = sub_offset(t, a.S);
-  if (threadIdx.x == 0) smax = 0;
-  const int grp = threadIdx.x / G, gl = threadIdx.x % G;
+  const int grp = threadIdx.x / G, gl = threadIdx.x % G, wid = gl >> 5;
+  const int sl = gl % SW;              // lane inside the scan segment
   const int64_t p = (int64_t)blockIdx.x * groups + grp;
   const bool active = p < a.P;
   double cx = 0, cy = 0, cz = 0, R = 1;
-  int lo[3] = {0, 0, 0}, ext[3] = {1, 1, 1};
+  int lo[3] = {0, 0, 0}, ext[3] = {0, 1, 1};
   bool wx = false, wy = false, wz = false;
   if (active) {
     cx = a.pos[p];
@@ -144,10 +155,14 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
     wy = crosses_seam(cy, R, a.g.ny, a.g.bcy);
     wz = D == 3 && crosses_seam(cz, R, a.g.nz, a.g.bcz);
   }
-  const int64_t nbox64 = active ? (int64_t)ext[0] * ext[1] * ext[2] : 0;
-  const int nbox = nbox64 > 0x7fffffff ? 0x7fffffff : (int)nbox64;
-  const bool fast = nbox < (1 << 24);
-  const float inv0 = 1.0f / (float)ext[0], inv1 = 1.0f / (float)ext[1];
+  int nrows = 0;
+  if (active && ext[0] > 0) {
+    const int64_t r64 = (int64_t)ext[1] * ext[2];
+    nrows = r64 > (1 << 24) ? (1 << 24) : (int)r64;   // (a box of 16 M rows does not occur)
+  }
+  // groups that share a warp (G < 32) synchronise with __syncwarp: they run the same number of passes
+  const int nrows_u = G < 32 ? __reduce_max_sync(0xffffffffu, nrows) : nrows;
+  const float inv1 = 1.0f / (float)(ext[1] > 0 ? ext[1] : 1);
   const double R2 = __dmul_rn(R, R);
   // Classification of a node by the box [|d| - hs, |d| + hs] per axis that holds its sample cloud
   // (hs = 1/2 - 1/(2S)): its farthest corner inside the particle => every sample is inside, its nearest
@@ -155,25 +170,12 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
   const double hs = a.hs;
   const double r2_full = R2 - 1e-9 * (R2 + 1.0), r2_none = R2 + 1e-9 * (R2 + 1.0);
   __syncthreads();
-  atomicMax(&smax, nbox);
-  __syncthreads();
-  const int maxbox = smax;
 
-  auto node_of = [&](int b, int &i, int &j, int &k) {
-    int bi, bj, bk, t;
-    if (fast) {
-      fast_divmod(b, ext[0], inv0, t, bi);
-      fast_divmod(t, ext[1], inv1, bk, bj);
-    } else {
-      bi = b % ext[0];
-      t = b / ext[0];
-      bj = t % ext[1];
-      bk = t / ext[1];
-    }
-    i = lo[0] + bi;
+  auto row_of = [&](int row, int &j, int &k) {
+    int bk = 0, bj = row;
+    if (D == 3) fast_divmod(row, ext[1], inv1, bk, bj);
     j = lo[1] + bj;
     k = lo[2] + bk;
-    if (wx) i = wrap_i(i, a.g.nx);
     if (wy) j = wrap_i(j, a.g.ny);
     if (D == 3 && wz) k = wrap_i(k, a.g.nz);
   };
@@ -197,42 +199,98 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
     a.eps_cnt[x] = (uint8_t)cnt;
   };
 
-  for (int base = 0; base < maxbox; base += CH) {
-    if (gl == 0) nlist[grp] = 0;
-    group_sync<G>();
-    // phase A: classify nodes
-    for (int b = base + gl; b < nbox && b < base + CH; b += G) {
-      int i, j, k;
-      node_of(b, i, j, k);
-      double dx = (double)i - cx, dy = (double)j - cy, dz = D == 3 ? (double)k - cz : 0.0;
-      if (wx) dx = min_image_d(dx, a.g.nx);
+  for (int row0 = 0; row0 < nrows_u; row0 += G) {
+    // ---- candidate interval of each row of this chunk
+    int b0 = 0, len = 0;
+    if (row0 + gl < nrows) {
+      int j, k;
+      row_of(row0 + gl, j, k);
+      double dy = (double)j - cy, dz = D == 3 ? (double)k - cz : 0.0;
       if (wy) dy = min_image_d(dy, a.g.ny);
       if (D == 3 && wz) dz = min_image_d(dz, a.g.nz);
-      dx = fabs(dx);
-      dy = fabs(dy);
-      dz = fabs(dz);
-      const double fx = dx + hs, fy = dy + hs, fz = D == 3 ? dz + hs : 0.0;
-      const double nx_ = fmax(dx - hs, 0.0), ny_ = fmax(dy - hs, 0.0), nz_ = D == 3 ? fmax(dz - hs, 0.0) : 0.0;
-      if (fx * fx + fy * fy + fz * fz <= r2_full) {
-        commit(i, j, k, a.SD);
-      } else if (nx_ * nx_ + ny_ * ny_ + nz_ * nz_ <= r2_none) {
-        const int slot = atomicAdd(&nlist[grp], 1);
-        list[grp][slot] = b;            // boundary cell: sample it
+      const double ny_ = fmax(fabs(dy) - hs, 0.0), nz_ = D == 3 ? fmax(fabs(dz) - hs, 0.0) : 0.0;
+      const double rad = r2_none - ny_ * ny_ - nz_ * nz_;
+      if (rad > -1e-9) {
+        if (wx) {
+          len = ext[0];
+        } else {
+          const double xo = hs + sqrt(fmax(rad, 0.0) + 1e-9) + 1e-9;
+          int il = (int)ceil(cx - xo), ih = (int)floor(cx + xo);
+          if (il < lo[0]) il = lo[0];
+          if (ih > lo[0] + ext[0] - 1) ih = lo[0] + ext[0] - 1;
+          b0 = il - lo[0];
+          len = ih >= il ? ih - il + 1 : 0;
+        }
       }
     }
-    group_sync<G>();
-    // phase B: one thread per boundary cell
-    const int nl = nlist[grp];
-    for (int e = gl; e < nl; e += G) {
-      int i, j, k;
-      node_of(list[grp][e], i, j, k);
-      int cnt;
-      if (SFIX > 0) cnt = thread_count_fixed<D, (SFIX > 0 ? SFIX : 1)>(a.g, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
-      else cnt = thread_count_generic<D>(a.g, a.S, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
-      if (cnt > 0) commit(i, j, k, cnt);
+    int incl = len;
+#pragma unroll
+    for (int o = 1; o < SW; o <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, incl, o, SW);
+      if (sl >= o) incl += t;
     }
+    int off = 0, total;
+    if (NW > 1) {
+      if (sl == 31) wtot[grp][wid] = incl;
+      __syncthreads();
+      total = 0;
+#pragma unroll
+      for (int w = 0; w < NW; ++w) {
+        if (w < wid) off += wtot[grp][w];
+        total += wtot[grp][w];
+      }
+    } else {
+      total = __shfl_sync(0xffffffffu, incl, SW - 1, SW);
+    }
+    pre[grp][gl] = off + incl - len;
+    beg[grp][gl] = b0;
+    const int total_u = G < 32 ? __reduce_max_sync(0xffffffffu, total) : total;
     group_sync<G>();
+
+    for (int tb = 0; tb < total_u; tb += CH) {
+      if (gl == 0) nlist[grp] = 0;
+      group_sync<G>();
+      // ---- phase A: classify the candidate nodes
+      for (int t = tb + gl; t < total && t < tb + CH; t += G) {
+        int r = 0;   // largest r with pre[r] <= t
+#pragma unroll
+        for (int step = G / 2; step > 0; step >>= 1)
+          if (pre[grp][r + step] <= t) r += step;
+        const int bi = beg[grp][r] + (t - pre[grp][r]);
+        int i = lo[0] + bi, j, k;
+        row_of(row0 + r, j, k);
+        if (wx) i = wrap_i(i, a.g.nx);
+        double dx = (double)i - cx, dy = (double)j - cy, dz = D == 3 ? (double)k - cz : 0.0;
+        if (wx) dx = min_image_d(dx, a.g.nx);
+        if (wy) dy = min_image_d(dy, a.g.ny);
+        if (D == 3 && wz) dz = min_image_d(dz, a.g.nz);
+        dx = fabs(dx);
+        dy = fabs(dy);
+        dz = fabs(dz);
+        const double fx = dx + hs, fy = dy + hs, fz = D == 3 ? dz + hs : 0.0;
+        const double nx_ = fmax(dx - hs, 0.0), ny_ = fmax(dy - hs, 0.0), nz_ = D == 3 ? fmax(dz - hs, 0.0) : 0.0;
+        if (fx * fx + fy * fy + fz * fz <= r2_full) {
+          commit(i, j, k, a.SD);
+        } else if (nx_ * nx_ + ny_ * ny_ + nz_ * nz_ <= r2_none) {
+          const int slot = atomicAdd(&nlist[grp], 1);
+          list[grp][slot] = (r << 16) | bi;   // boundary cell: sample it (r < G <= 128, bi < 2^16)
+        }
+      }
+      group_sync<G>();
+      // ---- phase B: one thread per boundary cell
+      const int nl = nlist[grp];
+      for (int e = gl; e < nl; e += G) {
+        const int code = list[grp][e];
+        int i = lo[0] + (code & 0xffff), j, k;
+        row_of(row0 + (code >> 16), j, k);
+        if (wx) i = wrap_i(i, a.g.nx);
+        int cnt;
+        if (SFIX > 0) cnt = thread_count_fixed<D, (SFIX > 0 ? SFIX : 1)>(a.g, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
+        else cnt = thread_count_generic<D>(a.g, a.S, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
+        if (cnt > 0) commit(i, j, k, cnt);
+      }
+      group_sync<G>();
+    }
   }
   settle();
 }
-
