@@ -712,14 +712,15 @@ __global__ void __launch_bounds__(128) reduce_forces_dense_kernel(Geom g, int64_
                                                                   double *__restrict__ force,
                                                                   double *__restrict__ torque) {
   constexpr int groups = 128 / G;
-  constexpr int NW = G / 32;
+  constexpr int NW = G >= 32 ? G / 32 : 1;
+  constexpr int SW = G < 32 ? G : 32;   // shuffle width of a group (two groups share a warp when G = 16)
   constexpr int NV = D == 2 ? 3 : 6;
   constexpr int U = 4;
   __shared__ double sh[groups][NW][NV];
   __shared__ int pre[groups][G + 1];   // exclusive prefix of the interval lengths of this chunk of rows
   __shared__ int beg[groups][G];       // first box column of each row's interval
   __shared__ int wtot[groups][NW];
-  const int grp = threadIdx.x / G, gl = threadIdx.x % G, lane = threadIdx.x & 31, wid = gl >> 5;
+  const int grp = threadIdx.x / G, gl = threadIdx.x % G, lane = gl % SW, wid = gl >> 5;
   const int64_t p = (int64_t)blockIdx.x * groups + grp;
   double acc[NV];
 #pragma unroll
@@ -742,9 +743,11 @@ __global__ void __launch_bounds__(128) reduce_forces_dense_kernel(Geom g, int64_
   }
   auto wrap1 = [](int v, int n) { return v < 0 ? v + n : (v >= n ? v - n : v); };
   const int nrows = (p < P && ext[0] > 0) ? ext[1] * ext[2] : 0;
+  // groups that share a warp synchronise with __syncwarp: they run the same number of passes
+  const int nrows_u = G < 32 ? __reduce_max_sync(0xffffffffu, nrows) : nrows;
   const float inv_e1 = 1.0f / (float)(ext[1] > 0 ? ext[1] : 1);
   // G == 128: one group per block, so nrows is block-uniform and the block barrier is safe
-  for (int row0 = 0; row0 < nrows; row0 += G) {
+  for (int row0 = 0; row0 < nrows_u; row0 += G) {
     int b0 = 0, len = 0;
     {
       const int row = row0 + gl;
@@ -774,8 +777,8 @@ __global__ void __launch_bounds__(128) reduce_forces_dense_kernel(Geom g, int64_
     }
     int incl = len;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int t = __shfl_up_sync(0xffffffffu, incl, o);
+    for (int o = 1; o < SW; o <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, incl, o, SW);
       if (lane >= o) incl += t;
     }
     int off = 0, total;
@@ -789,13 +792,14 @@ __global__ void __launch_bounds__(128) reduce_forces_dense_kernel(Geom g, int64_
         total += wtot[grp][w];
       }
     } else {
-      total = __shfl_sync(0xffffffffu, incl, 31);
+      total = __shfl_sync(0xffffffffu, incl, SW - 1, SW);
     }
+    const int total_u = G < 32 ? __reduce_max_sync(0xffffffffu, total) : total;
     pre[grp][gl] = off + incl - len;
     beg[grp][gl] = b0;
     if (gl == 0) pre[grp][G] = total;
     group_sync<G>();
-    for (int t0 = gl; t0 < total; t0 += U * G) {
+    for (int t0 = gl; t0 < total_u; t0 += U * G) {
       int32_t owner[U];
       double2 s01[U], s23[U];
       double rx[U], ry[U], rz[U];
@@ -856,7 +860,7 @@ __global__ void __launch_bounds__(128) reduce_forces_dense_kernel(Geom g, int64_
   }
 #pragma unroll
   for (int v = 0; v < NV; ++v)
-    for (int o = 16; o > 0; o >>= 1) acc[v] += __shfl_down_sync(0xffffffffu, acc[v], o);
+    for (int o = SW / 2; o > 0; o >>= 1) acc[v] += __shfl_down_sync(0xffffffffu, acc[v], o, SW);
   if (lane == 0)
     for (int v = 0; v < NV; ++v) sh[grp][wid][v] = acc[v];
   __syncthreads();
@@ -882,9 +886,8 @@ static double sample_cloud_radius(const lbmimb_lattice *h) {
   return sqrt((double)h->g.dim) * (0.5 - 0.5 / (double)h->prm.subsamples) + 1e-6;
 }
 
-// Default: the dense kernel in 3D (C3 0.275 -> 0.196 ms, P3D 1.74 -> 1.45 ms), the box-walking kernel in 2D
-// (a disk fills most of its 12-node rows: C4 0.95 vs 0.99 ms).  LBMIMB_REDUCE_VARIANT=1 forces the box
-// walk, 2 the dense kernel (A/B numbers of profiles/).
+// Default: the dense kernel (B200: C3 0.275 -> 0.196 ms, P3D 1.74 -> 1.45 ms, C4 0.97 -> 0.69 ms, P2D 1.12 -> 0.91 ms).
+// LBMIMB_REDUCE_VARIANT=1 selects the box-walking kernel (A/B numbers of profiles/).
 static int reduce_variant() {
   static int v = -1;
   if (v < 0) {
@@ -896,14 +899,13 @@ static int reduce_variant() {
 
 lbmimb_status launch_reduce(lbmimb_lattice *h) {
   const double ho = sample_cloud_radius(h);
-  const int rv = reduce_variant();
-  const bool box = rv == 1 || (rv != 2 && h->g.dim == 2);
+  const bool box = reduce_variant() == 1;
   if (h->g.dim == 2) {
     if (box)
       reduce_forces_kernel<2, 32><<<blocks_for(h->P, 4), 128, 0, h->stream>>>(h->g, h->P, ho, h->pos, h->radius,
                                                                              h->pid, h->s, h->force, h->torque);
     else
-      reduce_forces_dense_kernel<2, 32><<<blocks_for(h->P, 4), 128, 0, h->stream>>>(
+      reduce_forces_dense_kernel<2, 16><<<blocks_for(h->P, 8), 128, 0, h->stream>>>(
           h->g, h->P, ho, h->pos, h->radius, h->pid, h->s, h->force, h->torque);
   } else {
     if (box)
