@@ -1,8 +1,9 @@
 // a1, pass 1 of the particle -> lattice mapping (included by particles.cu).
 //
 // One group of G threads per particle walks the particle's bounding box.
-//   phase A: every node is classified by the distance of its centre to the particle centre:
-//            surely full (count = S^D), surely empty, or a boundary cell that must be sampled;
+//   phase A: the nodes of the row intervals that can hold a covered node (dense walk, below) are classified
+//            by the distance of their centre to the particle centre: surely full (count = S^D), surely
+//            empty, or a boundary cell that must be sampled;
 //   phase B: one THREAD per boundary cell counts the inside samples.  The squared distance is
 //            separable, d2 = (dx^2 + dy^2) + dz^2 with dx depending on (i, ax) only, so the S
 //            values per axis are formed once (S*D subtract/multiply) and the S^D samples cost one
@@ -11,6 +12,8 @@
 //            bit-exact; only the order in which samples are visited differs.
 // Nodes reached by more than one particle are detected with an atomic exchange on pid and
 // queued for pass 2 (map_contested_kernel), which recomputes them from the definition.
+// (Measured and dropped: one thread per ROW that writes the full columns itself and lists only the
+//  shell -- no per-node classification, but serial commits per thread: C3 0.325 -> 0.369 ms, C4 1.50 -> 1.73 ms.)
 #pragma once
 // (included inside namespace lbmimb, after MapArgs / bbox_axis / min_image_d / wrap_i / sub_offset)
 
@@ -116,6 +119,67 @@ __device__ __forceinline__ void group_sync() {
   else __syncthreads();
 }
 
+// ---- dense walks of a particle's bounding box (map pass 1, table map, force reduction) ----
+// Each of the G threads of a group brings the candidate interval [b0, b0 + len) of columns of ONE row of the
+// box; the intervals are concatenated: pre[r] = number of candidates in rows < r (exclusive scan), beg[r] =
+// first column of row r.  Candidate t then sits in row interval_row<G>(pre, t) at column beg[r] + t - pre[r].
+// Returns the number of candidates of the G rows.  Ends with a group barrier (pre / beg are readable).
+// pre: [G + 1] ints, beg: [G], wtot: [G / 32] (groups of more than one warp), all in shared memory.
+template <int G>
+__device__ __forceinline__ int scan_row_intervals(int len, int b0, int gl, int *pre, int *beg, int *wtot) {
+  constexpr int NW = G >= 32 ? G / 32 : 1;
+  constexpr int SW = G < 32 ? G : 32;   // two groups share a warp when G = 16
+  const int sl = gl % SW, wid = gl >> 5;
+  int incl = len;
+#pragma unroll
+  for (int o = 1; o < SW; o <<= 1) {
+    const int t = __shfl_up_sync(0xffffffffu, incl, o, SW);
+    if (sl >= o) incl += t;
+  }
+  int off = 0, total;
+  if (NW > 1) {
+    if (sl == 31) wtot[wid] = incl;
+    __syncthreads();
+    total = 0;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) {
+      if (w < wid) off += wtot[w];
+      total += wtot[w];
+    }
+  } else {
+    total = __shfl_sync(0xffffffffu, incl, SW - 1, SW);
+  }
+  pre[gl] = off + incl - len;
+  beg[gl] = b0;
+  group_sync<G>();
+  return total;
+}
+
+// largest r in [0, G) with pre[r] <= t
+template <int G>
+__device__ __forceinline__ int interval_row(const int *pre, int t) {
+  int r = 0;
+#pragma unroll
+  for (int step = G / 2; step > 0; step >>= 1)
+    if (pre[r + step] <= t) r += step;
+  return r;
+}
+
+// loop bounds of groups that share a warp (G < 32) must agree: they synchronise with __syncwarp
+template <int G>
+__device__ __forceinline__ int group_uniform_max(int v) {
+  return G < 32 ? __reduce_max_sync(0xffffffffu, v) : v;
+}
+
+// candidate columns of a row: lattice columns i of the box [lo, lo + ext) with |i - c| <= half
+__device__ __forceinline__ void clip_interval(double c, double half, int lo, int ext, int &b0, int &len) {
+  int il = (int)ceil(c - half), ih = (int)floor(c + half);
+  if (il < lo) il = lo;
+  if (ih > lo + ext - 1) ih = lo + ext - 1;
+  b0 = il - lo;
+  len = ih >= il ? ih - il + 1 : 0;
+}
+
 // Dense walk of the bounding box.  A sphere fills a third of its box, so classifying every box node
 // (phase A of map_particles_kernel) spends most of its time on nodes that are plainly empty.  Here every
 // row (j,k) of the box first gets the interval of columns that can pass the "not surely empty" test,
@@ -128,7 +192,6 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
   constexpr int groups = 128 / G;
   constexpr int CH = G >= 64 ? kMapChunk : 8 * G;   // candidate nodes per pass of a group
   constexpr int NW = G >= 32 ? G / 32 : 1;
-  constexpr int SW = G < 32 ? G : 32;               // shuffle width of a group's scan
   __shared__ double sub[256];
   __shared__ int list[groups][CH];
   __shared__ int nlist[groups];
@@ -136,8 +199,7 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
   __shared__ int beg[groups][G];       // first box column of each row's interval
   __shared__ int wtot[groups][NW];
   for (int t = threadIdx.x; t < a.S; t += blockDim.x) sub[t] = sub_offset(t, a.S);
-  const int grp = threadIdx.x / G, gl = threadIdx.x % G, wid = gl >> 5;
-  const int sl = gl % SW;              // lane inside the scan segment
+  const int grp = threadIdx.x / G, gl = threadIdx.x % G;
   const int64_t p = (int64_t)blockIdx.x * groups + grp;
   const bool active = p < a.P;
   double cx = 0, cy = 0, cz = 0, R = 1;
@@ -161,7 +223,7 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
     nrows = r64 > (1 << 24) ? (1 << 24) : (int)r64;   // (a box of 16 M rows does not occur)
   }
   // groups that share a warp (G < 32) synchronise with __syncwarp: they run the same number of passes
-  const int nrows_u = G < 32 ? __reduce_max_sync(0xffffffffu, nrows) : nrows;
+  const int nrows_u = group_uniform_max<G>(nrows);
   const float inv1 = 1.0f / (float)(ext[1] > 0 ? ext[1] : 1);
   const double R2 = __dmul_rn(R, R);
   // Classification of a node by the box [|d| - hs, |d| + hs] per axis that holds its sample cloud
@@ -214,48 +276,19 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
         if (wx) {
           len = ext[0];
         } else {
-          const double xo = hs + sqrt(fmax(rad, 0.0) + 1e-9) + 1e-9;
-          int il = (int)ceil(cx - xo), ih = (int)floor(cx + xo);
-          if (il < lo[0]) il = lo[0];
-          if (ih > lo[0] + ext[0] - 1) ih = lo[0] + ext[0] - 1;
-          b0 = il - lo[0];
-          len = ih >= il ? ih - il + 1 : 0;
+          clip_interval(cx, hs + sqrt(fmax(rad, 0.0) + 1e-9) + 1e-9, lo[0], ext[0], b0, len);
         }
       }
     }
-    int incl = len;
-#pragma unroll
-    for (int o = 1; o < SW; o <<= 1) {
-      const int t = __shfl_up_sync(0xffffffffu, incl, o, SW);
-      if (sl >= o) incl += t;
-    }
-    int off = 0, total;
-    if (NW > 1) {
-      if (sl == 31) wtot[grp][wid] = incl;
-      __syncthreads();
-      total = 0;
-#pragma unroll
-      for (int w = 0; w < NW; ++w) {
-        if (w < wid) off += wtot[grp][w];
-        total += wtot[grp][w];
-      }
-    } else {
-      total = __shfl_sync(0xffffffffu, incl, SW - 1, SW);
-    }
-    pre[grp][gl] = off + incl - len;
-    beg[grp][gl] = b0;
-    const int total_u = G < 32 ? __reduce_max_sync(0xffffffffu, total) : total;
-    group_sync<G>();
+    const int total = scan_row_intervals<G>(len, b0, gl, pre[grp], beg[grp], wtot[grp]);
+    const int total_u = group_uniform_max<G>(total);
 
     for (int tb = 0; tb < total_u; tb += CH) {
       if (gl == 0) nlist[grp] = 0;
       group_sync<G>();
       // ---- phase A: classify the candidate nodes
       for (int t = tb + gl; t < total && t < tb + CH; t += G) {
-        int r = 0;   // largest r with pre[r] <= t
-#pragma unroll
-        for (int step = G / 2; step > 0; step >>= 1)
-          if (pre[grp][r + step] <= t) r += step;
+        const int r = interval_row<G>(pre[grp], t);
         const int bi = beg[grp][r] + (t - pre[grp][r]);
         int i = lo[0] + bi, j, k;
         row_of(row0 + r, j, k);

@@ -102,27 +102,52 @@ __device__ __forceinline__ int table_code(const TableGeom &t, double dx, double 
 }
 
 // ---------------------------------------------------------------------------
-// pass 1: one group of G threads per particle walks its bounding box, one look-up per node.
-// Shared nodes are detected like in the sampled map (exchange on pid, examined one commit later).
+// pass 1: one group of G threads per particle, one look-up per candidate node.  Dense walk of the bounding
+// box (map_pass1.cuh): a node can have a non-zero code only if d^2 <= none2, so every row (j,k) contributes
+// the columns with |dx| <= sqrt(none2 - dy^2 - dz^2) (+ margin: a superset) and the group walks the
+// concatenated intervals.  The look-up itself is unchanged.  Shared nodes are detected like in the sampled
+// map (exchange on pid, examined one commit later).
 // ---------------------------------------------------------------------------
 template <int D, int G>
 __global__ void __launch_bounds__(128) map_table_kernel(const MapArgs a, const TableGeom t) {
   constexpr int groups = 128 / G;
+  constexpr int NW = G >= 32 ? G / 32 : 1;
+  __shared__ int pre[groups][G + 1];
+  __shared__ int beg[groups][G];
+  __shared__ int wtot[groups][NW];
   const int grp = threadIdx.x / G, gl = threadIdx.x % G;
   const int64_t p = (int64_t)blockIdx.x * groups + grp;
-  if (p >= a.P) return;
-  const double cx = a.pos[p], cy = a.pos[a.P + p], cz = D == 3 ? a.pos[2 * a.P + p] : 0.0;
+  const bool active = p < a.P;
+  double cx = 0.0, cy = 0.0, cz = 0.0;
   const double R = t.R;
-  int lo[3] = {0, 0, 0}, ext[3] = {1, 1, 1};
-  bbox_axis(cx, R, a.g.nx, a.g.bcx, lo[0], ext[0]);
-  bbox_axis(cy, R, a.g.ny, a.g.bcy, lo[1], ext[1]);
-  if (D == 3) bbox_axis(cz, R, a.g.nz, a.g.bcz, lo[2], ext[2]);
-  const bool wx = crosses_seam(cx, R, a.g.nx, a.g.bcx), wy = crosses_seam(cy, R, a.g.ny, a.g.bcy);
-  const bool wz = D == 3 && crosses_seam(cz, R, a.g.nz, a.g.bcz);
-  const int64_t nbox64 = (int64_t)ext[0] * ext[1] * ext[2];
-  const int nbox = nbox64 > 0x7fffffff ? 0x7fffffff : (int)nbox64;
-  const bool fast = nbox < (1 << 24);
-  const float inv0 = 1.0f / (float)ext[0], inv1 = 1.0f / (float)ext[1];
+  int lo[3] = {0, 0, 0}, ext[3] = {0, 1, 1};
+  bool wx = false, wy = false, wz = false;
+  if (active) {
+    cx = a.pos[p];
+    cy = a.pos[a.P + p];
+    cz = D == 3 ? a.pos[2 * a.P + p] : 0.0;
+    bbox_axis(cx, R, a.g.nx, a.g.bcx, lo[0], ext[0]);
+    bbox_axis(cy, R, a.g.ny, a.g.bcy, lo[1], ext[1]);
+    if (D == 3) bbox_axis(cz, R, a.g.nz, a.g.bcz, lo[2], ext[2]);
+    wx = crosses_seam(cx, R, a.g.nx, a.g.bcx);
+    wy = crosses_seam(cy, R, a.g.ny, a.g.bcy);
+    wz = D == 3 && crosses_seam(cz, R, a.g.nz, a.g.bcz);
+  }
+  int nrows = 0;
+  if (active && ext[0] > 0) {
+    const int64_t r64 = (int64_t)ext[1] * ext[2];
+    nrows = r64 > (1 << 24) ? (1 << 24) : (int)r64;
+  }
+  const int nrows_u = group_uniform_max<G>(nrows);
+  const float inv1 = 1.0f / (float)(ext[1] > 0 ? ext[1] : 1);
+  auto row_of = [&](int row, int &j, int &k) {
+    int bk = 0, bj = row;
+    if (D == 3) fast_divmod(row, ext[1], inv1, bk, bj);
+    j = lo[1] + bj;
+    k = lo[2] + bk;
+    if (wy) j = wrap_i(j, a.g.ny);
+    if (D == 3 && wz) k = wrap_i(k, a.g.nz);
+  };
   int64_t pend_x = -1;
   int32_t pend_old = -1;
   auto settle = [&]() {
@@ -133,33 +158,40 @@ __global__ void __launch_bounds__(128) map_table_kernel(const MapArgs a, const T
     }
     pend_x = -1;
   };
-  for (int b = gl; b < nbox; b += G) {
-    int bi, bj, bk, q;
-    if (fast) {
-      fast_divmod(b, ext[0], inv0, q, bi);
-      fast_divmod(q, ext[1], inv1, bk, bj);
-    } else {
-      bi = b % ext[0];
-      q = b / ext[0];
-      bj = q % ext[1];
-      bk = q / ext[1];
+  for (int row0 = 0; row0 < nrows_u; row0 += G) {
+    int b0 = 0, len = 0;
+    if (row0 + gl < nrows) {
+      int j, k;
+      row_of(row0 + gl, j, k);
+      double dy = (double)j - cy, dz = D == 3 ? (double)k - cz : 0.0;
+      if (wy) dy = min_image_d(dy, a.g.ny);
+      if (D == 3 && wz) dz = min_image_d(dz, a.g.nz);
+      const double rad = t.none2 - dy * dy - dz * dz;
+      if (rad > -1e-9) {
+        if (wx) len = ext[0];
+        else clip_interval(cx, sqrt(fmax(rad, 0.0) + 1e-9) + 1e-9, lo[0], ext[0], b0, len);
+      }
     }
-    int i = lo[0] + bi, j = lo[1] + bj, k = lo[2] + bk;
-    if (wx) i = wrap_i(i, a.g.nx);
-    if (wy) j = wrap_i(j, a.g.ny);
-    if (D == 3 && wz) k = wrap_i(k, a.g.nz);
-    double dx = __dsub_rn((double)i, cx), dy = __dsub_rn((double)j, cy), dz = D == 3 ? __dsub_rn((double)k, cz) : 0.0;
-    if (wx) dx = min_image_d(dx, a.g.nx);
-    if (wy) dy = min_image_d(dy, a.g.ny);
-    if (D == 3 && wz) dz = min_image_d(dz, a.g.nz);
-    const int code = table_code<D>(t, dx, dy, dz);
-    if (code > 0) {
-      const int64_t x = ((int64_t)k * a.g.ny + j) * a.g.nx + i;
-      settle();
-      pend_old = atomicExch(a.pid + x, (int32_t)p);
-      pend_x = x;
-      a.eps_cnt[x] = (uint8_t)code;
+    const int total = scan_row_intervals<G>(len, b0, gl, pre[grp], beg[grp], wtot[grp]);
+    for (int c = gl; c < total; c += G) {
+      const int r = interval_row<G>(pre[grp], c);
+      int i = lo[0] + beg[grp][r] + (c - pre[grp][r]), j, k;
+      row_of(row0 + r, j, k);
+      if (wx) i = wrap_i(i, a.g.nx);
+      double dx = __dsub_rn((double)i, cx), dy = __dsub_rn((double)j, cy), dz = D == 3 ? __dsub_rn((double)k, cz) : 0.0;
+      if (wx) dx = min_image_d(dx, a.g.nx);
+      if (wy) dy = min_image_d(dy, a.g.ny);
+      if (D == 3 && wz) dz = min_image_d(dz, a.g.nz);
+      const int code = table_code<D>(t, dx, dy, dz);
+      if (code > 0) {
+        const int64_t x = ((int64_t)k * a.g.ny + j) * a.g.nx + i;
+        settle();
+        pend_old = atomicExch(a.pid + x, (int32_t)p);
+        pend_x = x;
+        a.eps_cnt[x] = (uint8_t)code;
+      }
     }
+    group_sync<G>();
   }
   settle();
 }

@@ -744,7 +744,7 @@ __global__ void __launch_bounds__(128) reduce_forces_dense_kernel(Geom g, int64_
   auto wrap1 = [](int v, int n) { return v < 0 ? v + n : (v >= n ? v - n : v); };
   const int nrows = (p < P && ext[0] > 0) ? ext[1] * ext[2] : 0;
   // groups that share a warp synchronise with __syncwarp: they run the same number of passes
-  const int nrows_u = G < 32 ? __reduce_max_sync(0xffffffffu, nrows) : nrows;
+  const int nrows_u = group_uniform_max<G>(nrows);
   const float inv_e1 = 1.0f / (float)(ext[1] > 0 ? ext[1] : 1);
   // G == 128: one group per block, so nrows is block-uniform and the block barrier is safe
   for (int row0 = 0; row0 < nrows_u; row0 += G) {
@@ -765,40 +765,13 @@ __global__ void __launch_bounds__(128) reduce_forces_dense_kernel(Geom g, int64_
           if (wx) {
             len = ext[0];
           } else {
-            const double hw = sqrt(fmax(hw2, 0.0) + 1e-6);
-            int il = (int)ceil(cx - hw), ih = (int)floor(cx + hw);
-            if (il < lo[0]) il = lo[0];
-            if (ih > lo[0] + ext[0] - 1) ih = lo[0] + ext[0] - 1;
-            b0 = il - lo[0];
-            len = ih >= il ? ih - il + 1 : 0;
+            clip_interval(cx, sqrt(fmax(hw2, 0.0) + 1e-6), lo[0], ext[0], b0, len);
           }
         }
       }
     }
-    int incl = len;
-#pragma unroll
-    for (int o = 1; o < SW; o <<= 1) {
-      const int t = __shfl_up_sync(0xffffffffu, incl, o, SW);
-      if (lane >= o) incl += t;
-    }
-    int off = 0, total;
-    if (NW > 1) {
-      if (lane == 31) wtot[grp][wid] = incl;
-      __syncthreads();
-      total = 0;
-#pragma unroll
-      for (int w = 0; w < NW; ++w) {
-        if (w < wid) off += wtot[grp][w];
-        total += wtot[grp][w];
-      }
-    } else {
-      total = __shfl_sync(0xffffffffu, incl, SW - 1, SW);
-    }
-    const int total_u = G < 32 ? __reduce_max_sync(0xffffffffu, total) : total;
-    pre[grp][gl] = off + incl - len;
-    beg[grp][gl] = b0;
-    if (gl == 0) pre[grp][G] = total;
-    group_sync<G>();
+    const int total = scan_row_intervals<G>(len, b0, gl, pre[grp], beg[grp], wtot[grp]);
+    const int total_u = group_uniform_max<G>(total);
     for (int t0 = gl; t0 < total_u; t0 += U * G) {
       int32_t owner[U];
       double2 s01[U], s23[U];
@@ -810,10 +783,7 @@ __global__ void __launch_bounds__(128) reduce_forces_dense_kernel(Geom g, int64_
         s01[u] = s23[u] = make_double2(0.0, 0.0);
         rx[u] = ry[u] = rz[u] = 0.0;
         if (t < total) {
-          int r = 0;   // largest r with pre[r] <= t
-#pragma unroll
-          for (int step = G / 2; step > 0; step >>= 1)
-            if (pre[grp][r + step] <= t) r += step;
+          const int r = interval_row<G>(pre[grp], t);
           const int bi = beg[grp][r] + (t - pre[grp][r]);
           const int row = row0 + r;
           int bk = 0, bj = row;

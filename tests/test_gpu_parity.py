@@ -136,6 +136,42 @@ def test_map_box_wider_than_the_periodic_domain(orc, lb):
     _map_both(orc, lb, 3, (6, 5, 7), (0, 0, 0), 4, np.array([[3.1], [2.2], [3.3]]), np.array([4.0]))
 
 
+@pytest.mark.parametrize("dim", [2, 3])
+def test_big_particles_many_row_chunks_map_table_and_forces(orc, lb, dim):
+    """Particles whose bounding box has more rows than a thread group (several row chunks and several
+    candidate passes of the dense box walk), next to small ones, across a seam and against a wall:
+    sampled map and table map bit-exact, fields and forces at the usual tolerances."""
+    if dim == 2:
+        n, bc, S = (150, 131), (0, 1), 8
+        pos = np.array([[60.3, 140.2, 20.7, 100.1], [66.6, 30.4, 100.9, 110.3]])
+        radius = np.array([40.25, 17.5, 3.0, 16.0])
+    else:
+        n, bc, S = (61, 50, 57), (0, 1, 0), 4
+        pos = np.array([[25.3, 55.2, 50.7], [24.6, 12.4, 40.9], [30.1, 50.3, 8.2]])
+        radius = np.array([20.5, 6.25, 9.0])
+    P = radius.size
+    _map_both(orc, lb, dim, n, bc, S, pos, radius)
+    rng = np.random.default_rng(5 + dim)
+    w = inputs.Workload("big", dim, n, bc, 0.8, (0.0, -1e-5, 0.0)[:dim], S, 5, pos, rng.uniform(-0.01, 0.01, (dim, P)),
+                        rng.uniform(-1e-3, 1e-3, (1 if dim == 2 else 3, P)), radius, np.full(P, 100.0))
+    ref = oracle_run(orc, w, 5)
+    lat, got = gpu_run(lb, w, 5)
+    assert np.array_equal(got["eps"], ref["eps"]) and np.array_equal(got["pid"], ref["pid"])
+    assert_fields_close(got["f"], ref["f"])
+    assert_forces_close(got["force"], got["torque"], ref)
+    lat.close()
+    # the paper's table look-up needs one radius
+    rad1 = np.full(P, radius[0] / 2)
+    lat = lb.Lattice(dim, n, bc, 0.8, (0,) * dim, S, max_particles=P)
+    lat.set_mapping_mode(lb.MAP_TABLE)
+    lat.set_particles(pos, np.zeros((dim, P)), None, rad1, np.ones(P))
+    lat.map_particles()
+    eo, po = orc.map_particles_table(dim, n, bc, pos, rad1)
+    assert np.array_equal(lat.fetch_fields(lb.FIELD_EPS_CNT), eo)
+    assert np.array_equal(lat.fetch_fields(lb.FIELD_PID), po)
+    lat.close()
+
+
 def test_map_is_translation_invariant_on_the_gpu_too(orc, lb):
     w = inputs.reduced("C2")
     e0, p0 = _map_both(orc, lb, w.dim, w.n, (0, 0), 8, w.pos, w.radius)
