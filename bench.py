@@ -38,7 +38,7 @@ UNIT = "MLUPS"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused kernel from the committed
 # `ncu --set full` capture (profiles/r1_traffic.md); None where no capture exists for the workload.
-NCU_TRAFFIC_BYTES = {"C3": 20849638000, "C4": 41870191000}
+NCU_TRAFFIC_BYTES = {"C3": 20850708000, "C4": 41871111000}   # profiles/r1_traffic.md
 
 
 def measured_peak_gbs():
