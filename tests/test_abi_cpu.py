@@ -102,6 +102,33 @@ def test_no_cpu_fallback(lb):
     assert b"no CPU fallback" in lb.load().lbmimb_last_error()
 
 
+def test_null_handle_is_rejected_by_every_entry_point(lb):
+    """Argument checks run before any CUDA call, so they can be exercised without a GPU."""
+    lib = lb.load()
+    d = lb.DemParams()
+    d.kn, d.restitution, d.dt = 1.0, 0.9, 1.0
+    buf = np.zeros(8)
+    i64 = np.zeros(4, dtype=np.int64)
+    calls = [lambda: lib.lbmimb_set_particles(None, 0, None, None, None, None, None),
+             lambda: lib.lbmimb_set_particle_velocities(None, None, None),
+             lambda: lib.lbmimb_get_particles(None, None, None, None),
+             lambda: lib.lbmimb_map_particles(None),
+             lambda: lib.lbmimb_set_mapping_mode(None, 0),
+             lambda: lib.lbmimb_step(None, 1),
+             lambda: lib.lbmimb_reduce_particle_forces(None, None, None),
+             lambda: lib.lbmimb_dem_step(None, C.byref(d)),
+             lambda: lib.lbmimb_set_neighbor_mode(None, 1, 1.0, 100),
+             lambda: lib.lbmimb_fetch_neighbor_list(None, i64.ctypes.data_as(C.c_void_p), None, 0, None),
+             lambda: lib.lbmimb_diagnostics(None, buf.ctypes.data_as(C.c_void_p)),
+             lambda: lib.lbmimb_set_distributions(None, buf.ctypes.data_as(C.c_void_p)),
+             lambda: lib.lbmimb_synchronize(None)]
+    for k, call in enumerate(calls):
+        assert call() == lb.EINVAL, "entry point %d accepted a NULL handle" % k
+        assert b"NULL" in lib.lbmimb_last_error()
+    assert lib.lbmimb_destroy_lattice(None) == lb.OK
+    assert lib.lbmimb_num_particles(None) == -1 and lib.lbmimb_time(None) == -1
+
+
 def test_product_never_imports_the_oracle():
     """The oracle is test infrastructure: nothing under paper_1011_2613_b200/ may name it."""
     pkg = os.path.join(ROOT, "paper_1011_2613_b200")
