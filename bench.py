@@ -204,6 +204,8 @@ def main():
                          "neighbour lists (PAPER.md:69, DESIGN.md R19)")
     ap.add_argument("--skin", type=float, default=1.0, help="neighbour-list skin in lattice units")
     ap.add_argument("--every", type=int, default=100, help="neighbour lists are at most this many steps old")
+    ap.add_argument("--coupled-api", action="store_true",
+                    help="coupled workloads: also time lbmimb_run_coupled (the same loop replayed from a CUDA graph)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -313,6 +315,21 @@ def main():
                "d2h_bytes_per_step": int(d2h), "ms_per_step": e_ms / args.steps}
 
     lat.synchronize()
+    coupled = None
+    if dem and args.coupled_api:      # the same K steps through ONE call: launches replayed from a CUDA graph
+        dargs = (dem["kn"], dem["restitution"], dem["g_particle"], dem["dt"])
+        lat.run_coupled(5, *dargs)
+        replicas.barrier()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        lat.run_coupled(args.steps, *dargs)
+        b.record()
+        torch.cuda.synchronize()
+        replicas.barrier()
+        c_units, c_ms = replicas.aggregate(float(N) * args.steps, a.elapsed_time(b))
+        coupled = {"value": replicas.mlups(c_units, c_ms), "unit": UNIT, "ms_per_step": c_ms / args.steps,
+                   "call": "lbmimb_run_coupled(%d)" % args.steps}
     diag = diag_ms = None
     if dem:                        # the Figs. 5/7 time-series sample: one device reduction per output step
         lat.map_particles()
@@ -361,7 +378,7 @@ def main():
             "breakdown_ms": {"map_particles": float(seg[:, 0].mean()), "step": kern_ms,
                              "reduce_particle_forces": float(seg[:, 2].mean()),
                              "dem_step": float(seg[:, 3].mean()) if dem else 0.0, "diagnostics_once": diag_ms},
-            "diagnostics": diag, "neighbor_list": nl_info,
+            "diagnostics": diag, "neighbor_list": nl_info, "coupled_api": coupled,
             "version": lb.version()}
     print(json.dumps(line))
     lat.close()

@@ -203,6 +203,18 @@ lbmimb_status lbmimb_reduce_particle_forces(lbmimb_lattice *h, double *force, do
 lbmimb_status lbmimb_dem_step(lbmimb_lattice *h, const lbmimb_dem_params *dem);
 
 /*
+ * nsteps coupled steps of the paper's method, each = map_particles -> step(1) -> reduce_particle_forces
+ * (results kept on the device) -> dem_step, the order of BASELINE.json configs[4].  Bit for bit
+ * what calling the four entry points in a loop gives.  The first step is launched call by call; the launches of
+ * the following steps are captured ONCE, two steps at a time (both parities of the distribution arrays), into a
+ * CUDA graph and replayed, which removes the per-launch host cost of the ~25 small particle-side kernels of a
+ * step (the neighbour-list rebuild rule is decided on the device, so the launch sequence never changes).  The
+ * graph is re-captured when the number of particles, their radii, a mode or the DEM parameters change.
+ * LBMIMB_NO_GRAPH=1 in the environment keeps to plain launches.  Asynchronous.  Errors as for the four calls.
+ */
+lbmimb_status lbmimb_run_coupled(lbmimb_lattice *h, const lbmimb_dem_params *dem, int32_t nsteps);
+
+/*
  * Contact search of a4 (lbmimb_set_neighbor_mode).
  * CELLS (default): a cell list over the particles, rebuilt whenever positions change.
  * VERLET: the paper's scheme ("The neighbor-list of each solid particle is established

@@ -29,7 +29,7 @@ EXPORTS = [
     "lbmimb_set_distributions", "lbmimb_set_particles_dev", "lbmimb_reduce_particle_forces_dev",
     "lbmimb_synchronize", "lbmimb_time", "lbmimb_launch_count", "lbmimb_last_error", "lbmimb_version",
     "lbmimb_set_mapping_mode", "lbmimb_fetch_eps_table", "lbmimb_diagnostics",
-    "lbmimb_set_neighbor_mode", "lbmimb_fetch_neighbor_list",
+    "lbmimb_set_neighbor_mode", "lbmimb_fetch_neighbor_list", "lbmimb_run_coupled",
 ]
 DIAG_LEN = 20
 
@@ -82,6 +82,7 @@ def load():
     lib.lbmimb_reduce_particle_forces.argtypes = [vp, vp, vp]
     lib.lbmimb_reduce_particle_forces_dev.argtypes = [vp, vp, vp]
     lib.lbmimb_dem_step.argtypes = [vp, C.POINTER(DemParams)]
+    lib.lbmimb_run_coupled.argtypes = [vp, C.POINTER(DemParams), i32]
     lib.lbmimb_set_neighbor_mode.argtypes = [vp, i32, C.c_double, i64]
     lib.lbmimb_fetch_neighbor_list.argtypes = [vp, vp, vp, i64, vp]
     lib.lbmimb_fetch_fields.argtypes = [vp, i32, C.POINTER(i64), C.POINTER(i64), vp]
@@ -249,13 +250,20 @@ class Lattice:
     def reduce_particle_forces_dev(self, force_ptr, torque_ptr):
         _check(self.lib.lbmimb_reduce_particle_forces_dev(self.h, force_ptr or None, torque_ptr or None))
 
-    def dem_step(self, kn, restitution, g_particle, dt=1.0):
+    @staticmethod
+    def _dem_params(kn, restitution, g_particle, dt):
         d = DemParams()
         d.kn, d.restitution, d.dt = kn, restitution, dt
         g = list(g_particle) + [0.0] * (3 - len(g_particle))
         for a in range(3):
             d.g_particle[a] = g[a]
-        _check(self.lib.lbmimb_dem_step(self.h, C.byref(d)))
+        return d
+
+    def dem_step(self, kn, restitution, g_particle, dt=1.0):
+        _check(self.lib.lbmimb_dem_step(self.h, C.byref(self._dem_params(kn, restitution, g_particle, dt))))
+
+    def run_coupled(self, nsteps, kn, restitution, g_particle, dt=1.0):
+        _check(self.lib.lbmimb_run_coupled(self.h, C.byref(self._dem_params(kn, restitution, g_particle, dt)), nsteps))
 
     def set_neighbor_mode(self, mode, skin=0.0, every=0):
         _check(self.lib.lbmimb_set_neighbor_mode(self.h, mode, float(skin), int(every)))

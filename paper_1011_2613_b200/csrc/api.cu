@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -253,10 +254,14 @@ lbmimb_status lbmimb_create_lattice(const lbmimb_params *params, int64_t max_par
   return LBMIMB_OK;
 }
 
+static void coupled_graph_drop(lbmimb_lattice *h);
+
 lbmimb_status lbmimb_destroy_lattice(lbmimb_lattice *h) {
   if (!h) return LBMIMB_OK;
   cudaSetDevice(h->prm.device);
   cudaStreamSynchronize(h->stream);
+  coupled_graph_drop(h);
+  if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   neighbor_list_release(h);
   if (h->owns_ws) cudaFree(h->ws);
   delete h;
@@ -419,17 +424,24 @@ lbmimb_status lbmimb_synchronize(lbmimb_lattice *h) {
   return LBMIMB_OK;
 }
 
-lbmimb_status lbmimb_map_particles(lbmimb_lattice *h) {
-  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
-  lbmimb_status st = use_device(h);
-  if (st != LBMIMB_OK) return st;
+// Bodies of the four calls of a coupled step: launches and state machine only (no argument checks, no
+// cudaSetDevice), shared by the entry points and by the graph capture of lbmimb_run_coupled.
+static lbmimb_status map_body(lbmimb_lattice *h) {
   if (h->P > 0) {
-    if ((st = launch_map(h)) != LBMIMB_OK) return st;
+    lbmimb_status st = launch_map(h);
+    if (st != LBMIMB_OK) return st;
   }
   h->map_valid = true;
   h->s_valid = false;
   h->forces_valid = false;
   return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_map_particles(lbmimb_lattice *h) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  return map_body(h);
 }
 
 lbmimb_status lbmimb_set_mapping_mode(lbmimb_lattice *h, int32_t mode) {
@@ -465,12 +477,8 @@ lbmimb_status lbmimb_fetch_eps_table(lbmimb_lattice *h, uint8_t *dst, int64_t ca
   return LBMIMB_OK;
 }
 
-lbmimb_status lbmimb_step(lbmimb_lattice *h, int32_t nsteps) {
-  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
-  if (nsteps < 0) return fail(LBMIMB_EINVAL, "nsteps < 0");
-  if (!h->map_valid) return fail(LBMIMB_ESTATE, "particles were set or moved but not mapped: call lbmimb_map_particles first");
-  lbmimb_status st = use_device(h);
-  if (st != LBMIMB_OK) return st;
+static lbmimb_status step_body(lbmimb_lattice *h, int32_t nsteps) {
+  lbmimb_status st;
   for (int32_t it = 0; it < nsteps; ++it) {
     bool emit = (h->P > 0) && (it == nsteps - 1);
     if ((st = launch_collide_stream(h, emit)) != LBMIMB_OK) return st;
@@ -485,17 +493,31 @@ lbmimb_status lbmimb_step(lbmimb_lattice *h, int32_t nsteps) {
   return LBMIMB_OK;
 }
 
-static lbmimb_status reduce_common(lbmimb_lattice *h) {
+lbmimb_status lbmimb_step(lbmimb_lattice *h, int32_t nsteps) {
   if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
-  if (h->P > 0 && !h->s_valid)
-    return fail(LBMIMB_ESTATE, "no exchange vectors: call lbmimb_step after lbmimb_map_particles first");
+  if (nsteps < 0) return fail(LBMIMB_EINVAL, "nsteps < 0");
+  if (!h->map_valid) return fail(LBMIMB_ESTATE, "particles were set or moved but not mapped: call lbmimb_map_particles first");
   lbmimb_status st = use_device(h);
   if (st != LBMIMB_OK) return st;
+  return step_body(h, nsteps);
+}
+
+static lbmimb_status reduce_body(lbmimb_lattice *h) {
+  if (h->P > 0 && !h->s_valid)
+    return fail(LBMIMB_ESTATE, "no exchange vectors: call lbmimb_step after lbmimb_map_particles first");
   if (h->P > 0) {
-    if ((st = launch_reduce(h)) != LBMIMB_OK) return st;
+    lbmimb_status st = launch_reduce(h);
+    if (st != LBMIMB_OK) return st;
   }
   h->forces_valid = true;
   return LBMIMB_OK;
+}
+
+static lbmimb_status reduce_common(lbmimb_lattice *h) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  return reduce_body(h);
 }
 
 lbmimb_status lbmimb_reduce_particle_forces(lbmimb_lattice *h, double *force, double *torque) {
@@ -524,20 +546,136 @@ lbmimb_status lbmimb_reduce_particle_forces_dev(lbmimb_lattice *h, double *force
   return LBMIMB_OK;
 }
 
-lbmimb_status lbmimb_dem_step(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
-  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+static lbmimb_status check_dem_params(const lbmimb_dem_params *dem) {
   if (!dem) return fail(LBMIMB_EINVAL, "dem params is NULL");
   if (!(dem->kn > 0.0) || !(dem->restitution > 0.0) || !(dem->restitution <= 1.0) || !(dem->dt > 0.0))
     return fail(LBMIMB_EINVAL, "dem params: need kn > 0, 0 < restitution <= 1, dt > 0");
+  return LBMIMB_OK;
+}
+
+static lbmimb_status dem_body(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
   if (h->P == 0) return LBMIMB_OK;
-  lbmimb_status st = use_device(h);
-  if (st != LBMIMB_OK) return st;
+  lbmimb_status st;
   if ((st = launch_dem(h, dem)) != LBMIMB_OK) return st;
   // positions moved: the map and the exchange vectors are stale; the cell list was rebuilt at
   // the new positions inside the step and stays valid; force/torque stay "the last reduction"
   h->map_valid = false;
   h->s_valid = false;
   return launch_pack_records(h);
+}
+
+lbmimb_status lbmimb_dem_step(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  lbmimb_status st = check_dem_params(dem);
+  if (st != LBMIMB_OK) return st;
+  if (h->P == 0) return LBMIMB_OK;
+  if ((st = use_device(h)) != LBMIMB_OK) return st;
+  return dem_body(h, dem);
+}
+
+// ---- lbmimb_run_coupled: the coupled loop with its launches replayed from a CUDA graph ----
+static lbmimb_status coupled_step_body(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
+  lbmimb_status st;
+  if ((st = map_body(h)) != LBMIMB_OK) return st;
+  if ((st = step_body(h, 1)) != LBMIMB_OK) return st;
+  if ((st = reduce_body(h)) != LBMIMB_OK) return st;
+  return dem_body(h, dem);
+}
+
+static bool coupled_graph_matches(const lbmimb_lattice *h, const CoupledGraph &g, const lbmimb_dem_params *dem) {
+  return g.valid && g.P == h->P && g.rmax == h->rmax && g.rmin == h->rmin && g.table_R == h->table_R &&
+         g.map_mode == h->map_mode && g.nl_mode == h->nl.mode && g.nl_skin == h->nl.skin &&
+         g.nl_every == h->nl.every && g.nl_mem == h->nl.mem && memcmp(&g.dem, dem, sizeof(*dem)) == 0;
+}
+
+static void coupled_graph_drop(lbmimb_lattice *h) {
+  for (int k = 0; k < 2; ++k) {
+    if (h->cg[k].exec) cudaGraphExecDestroy(h->cg[k].exec);
+    h->cg[k].exec = nullptr;
+    h->cg[k].valid = false;
+  }
+}
+
+// Captures two consecutive coupled steps (both parities of the distribution arrays) on the private stream.
+// The handle must be in the steady state of the loop (one plain step has run): then the host-side state
+// machine ends the pair exactly where it started, and only t and the launch counter are put back.
+static lbmimb_status coupled_graph_capture(lbmimb_lattice *h, const lbmimb_dem_params *dem, CoupledGraph &g) {
+  if (g.exec) cudaGraphExecDestroy(g.exec);
+  g.exec = nullptr;
+  g.valid = false;
+  if (!h->cap_stream) LBMIMB_CUDA(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+  const cudaStream_t user = h->stream;
+  const int64_t t0 = h->t, l0 = h->launches;
+  LBMIMB_CUDA(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+  h->stream = h->cap_stream;
+  lbmimb_status st = coupled_step_body(h, dem);
+  if (st == LBMIMB_OK) st = coupled_step_body(h, dem);
+  h->stream = user;
+  cudaGraph_t graph = nullptr;
+  const cudaError_t e = cudaStreamEndCapture(h->cap_stream, &graph);
+  g.launches = h->launches - l0;
+  h->launches = l0;
+  h->t = t0;
+  if (st != LBMIMB_OK || e != cudaSuccess || !graph) {
+    if (graph) cudaGraphDestroy(graph);
+    cudaGetLastError();
+    return st != LBMIMB_OK ? st : cuda_fail(e, "cudaStreamEndCapture(coupled steps)");
+  }
+  const cudaError_t e2 = cudaGraphInstantiate(&g.exec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (e2 != cudaSuccess) {
+    g.exec = nullptr;
+    return cuda_fail(e2, "cudaGraphInstantiate(coupled steps)");
+  }
+  g.valid = true;
+  g.P = h->P;
+  g.rmax = h->rmax;
+  g.rmin = h->rmin;
+  g.table_R = h->table_R;
+  g.map_mode = h->map_mode;
+  g.nl_mode = h->nl.mode;
+  g.nl_skin = h->nl.skin;
+  g.nl_every = h->nl.every;
+  g.nl_mem = h->nl.mem;
+  g.dem = *dem;
+  return LBMIMB_OK;
+}
+
+static bool coupled_graphs_enabled() {
+  static int v = -1;
+  if (v < 0) {
+    const char *e = getenv("LBMIMB_NO_GRAPH");
+    v = (e && atoi(e) != 0) ? 0 : 1;
+  }
+  return v == 1;
+}
+
+lbmimb_status lbmimb_run_coupled(lbmimb_lattice *h, const lbmimb_dem_params *dem, int32_t nsteps) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  lbmimb_status st = check_dem_params(dem);
+  if (st != LBMIMB_OK) return st;
+  if (nsteps < 0) return fail(LBMIMB_EINVAL, "nsteps < 0");
+  if ((st = use_device(h)) != LBMIMB_OK) return st;
+  if (h->P == 0) return step_body(h, nsteps);   // no particles: the other three calls are no-ops
+  int32_t left = nsteps;
+  if (left > 0) {   // the first step also (re)builds whatever the steady loop takes for granted
+    if ((st = coupled_step_body(h, dem)) != LBMIMB_OK) return st;
+    --left;
+  }
+  if (left >= 2 && coupled_graphs_enabled() && !h->cg_broken) {
+    CoupledGraph &g = h->cg[h->aa ? (h->aa_swapped ? 1 : 0) : h->cur];
+    if (!coupled_graph_matches(h, g, dem) && coupled_graph_capture(h, dem, g) != LBMIMB_OK) h->cg_broken = true;
+    if (g.valid) {
+      for (; left >= 2; left -= 2) {
+        LBMIMB_CUDA(cudaGraphLaunch(g.exec, h->stream));
+        h->t += 2;
+        h->launches += g.launches;
+      }
+    }
+  }
+  for (; left > 0; --left)
+    if ((st = coupled_step_body(h, dem)) != LBMIMB_OK) return st;
+  return LBMIMB_OK;
 }
 
 lbmimb_status lbmimb_set_neighbor_mode(lbmimb_lattice *h, int32_t mode, double skin, int64_t every) {

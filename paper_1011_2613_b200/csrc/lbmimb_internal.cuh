@@ -103,6 +103,19 @@ struct NeighborList {
   double rmax, rmin;   // radii the storage was sized for
 };
 
+// One instantiated CUDA graph of TWO consecutive coupled steps (lbmimb_run_coupled) and everything its
+// launches were captured with: it is replayed only while all of this still holds.
+struct CoupledGraph {
+  cudaGraphExec_t exec;
+  bool valid;
+  int64_t launches;   // kernels per replay
+  int64_t P;
+  double rmax, rmin, table_R, nl_skin;
+  int map_mode, nl_mode, nl_every;
+  const void *nl_mem;
+  lbmimb_dem_params dem;
+};
+
 }  // namespace lbmimb
 
 struct lbmimb_lattice {
@@ -142,6 +155,9 @@ struct lbmimb_lattice {
   lbmimb::CellList cl;
   bool cl_valid;
   lbmimb::NeighborList nl;
+  lbmimb::CoupledGraph cg[2];   // indexed by the distribution-array parity at the start of the pair
+  cudaStream_t cap_stream;      // private stream the pair is captured on
+  bool cg_broken;               // a capture failed once: keep to plain launches
 
   bool map_valid;     // eps_cnt/pid match the particle positions
   bool s_valid;       // s holds the exchange vectors of the last step under the current map
