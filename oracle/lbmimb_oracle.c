@@ -34,6 +34,15 @@
  * The Verlet-list functions (orc_verlet_*, orc_dem_step_verlet, R19)
  * are pinned in tests/test_oracle_verlet_pins.py (hand lists, lattice shell
  * counts, bitwise equality with the all-pairs trajectory, rebuild counts).
+ * The table look-up of the solid fraction (orc_eps_table, orc_map_table;
+ * PAPER.md:71-77, R17) is pinned in tests/test_oracle_table_pins.py (quadrature
+ * of the covered area / volume, symmetries, agreement with a fine sampled map).
+ * The suspension diagnostics (orc_diagnostics, R18) are pinned in
+ * tests/test_oracle_diag_pins.py (closed forms, exact rationals, momentum
+ * conservation); the averaging convention itself (which weights define the
+ * "area-averaged" velocities) is "parity unpinned": the paper prints no formula.
+ * The whole IMB term is checked physically by the drag of a periodic array
+ * against Hasimoto's series (test_P16_...).
  */
 #include <math.h>
 #include <stdint.h>

@@ -667,7 +667,11 @@ lbmimb_status lbmimb_run_coupled(lbmimb_lattice *h, const lbmimb_dem_params *dem
     if (!coupled_graph_matches(h, g, dem) && coupled_graph_capture(h, dem, g) != LBMIMB_OK) h->cg_broken = true;
     if (g.valid) {
       for (; left >= 2; left -= 2) {
-        LBMIMB_CUDA(cudaGraphLaunch(g.exec, h->stream));
+        if (cudaGraphLaunch(g.exec, h->stream) != cudaSuccess) {   // nothing was enqueued: go on call by call
+          cudaGetLastError();
+          h->cg_broken = true;
+          break;
+        }
         h->t += 2;
         h->launches += g.launches;
       }
