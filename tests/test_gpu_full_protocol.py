@@ -2,7 +2,7 @@
 the CPU oracle element by element.  `-m gpu`, and opt-in: the oracle needs tens of minutes per configuration
 (DESIGN.md section 14), so these run only with
 
-    LBMIMB_FULL=C2,C5 [LBMIMB_FULL_WINDOWS=k] python -m pytest tests/test_gpu_full_protocol.py -m gpu -s
+    LBMIMB_FULL=C2,C3,C4,C5 [LBMIMB_FULL_WINDOWS=k] python -m pytest tests/test_gpu_full_protocol.py -m gpu -s
 
 Each test appends one JSON line with what it measured to gpurun_out/full_protocol.jsonl (if that folder
 exists).  Tolerances: tests/parity_util.py (north star).  No expected value comes from the CUDA path."""
@@ -43,9 +43,9 @@ def lb():
     return binding
 
 
-@pytest.mark.parametrize("name", ["C2", "C3"])
+@pytest.mark.parametrize("name", ["C2", "C3", "C4"])
 def test_fixed_particle_config_in_full(orc, lb, name):
-    """BASELINE.json configs[1] / configs[2]: the whole lattice for the stated number of steps with the
+    """BASELINE.json configs[1] / configs[2] / configs[3]: the whole lattice for the stated number of steps with the
     particles held fixed; f, rho, u, the maps and the per-particle force / torque are compared."""
     need(name)
     w = inputs.FULL[name]()

@@ -316,6 +316,33 @@ def test_coupled_reduced_c5_windows(orc, lb):
     lat.close()
 
 
+# ----------------------------------------------------------------------------- device-pointer variants
+def test_device_pointer_variants_match_the_host_variants(orc, lb):
+    """lbmimb_set_particles_dev / lbmimb_reduce_particle_forces_dev with torch tensors (plumbing only) give
+    bit for bit what the host-pointer calls give, and the oracle agrees."""
+    import torch
+    w = inputs.reduced("C3")
+    ref = oracle_run(orc, w, 4)
+    lat_h, got = gpu_run(lb, w, 4)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    tp, tv, to, tr, tm = dev(w.pos), dev(w.vel), dev(w.omega), dev(w.radius), dev(w.mass)
+    lat = lb.Lattice(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, max_particles=w.P)
+    lat.set_particles_dev(w.P, tp.data_ptr(), tv.data_ptr(), to.data_ptr(), tr.data_ptr(), tm.data_ptr())
+    lat.map_particles()
+    lat.step(4)
+    tF = torch.zeros((w.dim, w.P), dtype=torch.float64, device="cuda")
+    tT = torch.zeros((3, w.P), dtype=torch.float64, device="cuda")
+    lat.reduce_particle_forces_dev(tF.data_ptr(), tT.data_ptr())
+    lat.synchronize()
+    assert np.array_equal(tF.cpu().numpy(), got["force"]) and np.array_equal(tT.cpu().numpy(), got["torque"])
+    assert np.array_equal(lat.fetch_fields(lb.FIELD_F), got["f"])
+    assert_forces_close(tF.cpu().numpy(), tT.cpu().numpy(), ref)
+    pg, vg, og = lat.get_particles()
+    assert np.array_equal(pg, w.pos) and np.array_equal(vg, w.vel) and np.array_equal(og, w.omega)
+    lat.close()
+    lat_h.close()
+
+
 # ----------------------------------------------------------------------------- errors
 def test_error_behaviour(lb):
     with pytest.raises(lb.LbmimbError) as ei:
