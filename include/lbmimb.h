@@ -194,7 +194,8 @@ lbmimb_status lbmimb_reduce_particle_forces(lbmimb_lattice *h, double *force, do
 
 /*
  * a4. One soft-sphere DEM step (eq. (4)-(5); R8-R11): linear spring-dashpot
- * normal contacts found with a cell list, wall contacts on wall axes, velocity-Verlet
+ * normal contacts found with a cell list (or neighbour lists, see lbmimb_set_neighbor_mode), wall contacts on
+ * wall axes, velocity-Verlet
  *   a0 = (F_h + F_c(x,v))/m + g_p; v' = v + dt/2 a0; x' = x + dt v' (wrapped into [0,n) on
  *   periodic axes); a1 = (F_h + F_c(x',v'))/m + g_p; v'' = v' + dt/2 a1; omega' = omega + dt T_h/I
  * with F_h, T_h of the last reduce_particle_forces (zero if none ran since set_particles).
