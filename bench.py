@@ -138,14 +138,15 @@ def oracle_sample(name, target_s=15.0, max_steps=50):
     pos, vel, om = w.pos.copy(), w.vel.copy(), w.omega.copy()
 
     def one_step(f, pos, vel, om):
+        if w.dem:
+            d = w.dem
+            f, pos, vel, om, _ = orc.coupled_step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, pos, vel, om,
+                                                  w.radius, w.mass, d["kn"], d["restitution"], d["g_particle"], d["dt"])
+            return f, pos, vel, om
         eps, pid = orc.map_particles(w.dim, w.n, w.bc, w.subsamples, pos, w.radius)
         f, s = orc.step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, eps_cnt=eps, pid=pid, pos=pos, vel=vel,
                         omega=om, want_s=True)
-        F, T, _, _ = orc.forces(w.dim, w.n, w.bc, s, pid, pos)
-        if w.dem:
-            d = w.dem
-            pos, vel, om = orc.dem_step(w.dim, w.n, w.bc, pos, vel, om, w.radius, w.mass, F, T, d["kn"],
-                                        d["restitution"], d["g_particle"], d["dt"])
+        orc.forces(w.dim, w.n, w.bc, s, pid, pos)
         return f, pos, vel, om
 
     f, pos, vel, om = one_step(f, pos, vel, om)          # warm-up (page faults, OpenMP pool)

@@ -262,6 +262,25 @@ def dem_step(dim, n, bc, pos, vel, omega, radius, mass, fh, th, kn, e, gp, dt=1.
     return pos, vel, omega
 
 
+def coupled_step(dim, n, bc, tau, g, S, f, pos, vel, omega, radius, mass, kn, e, gp, dt=1.0, verlet=None):
+    """One coupled step of the method in the order BASELINE.json configs[4] fixes (R11):
+         1. map      eps, pid at the CURRENT positions x(t)
+         2. LBM step f(t) -> f(t+1) with V_S from the CURRENT v(t), omega(t); the exchange vectors s are
+                     those of this collision, i.e. they come from the PRE-collision state f(t)
+         3. forces   F_h, T_h = eq. (3) over s
+         4. DEM step x, v, omega advance by dt with F_h, T_h held constant over the step
+       (`verlet`: a VerletState -> the neighbour-list variant of step 4, R19).
+    Returns (f, pos, vel, omega, info) with info = dict(eps, pid, s, force, torque, abs_f, abs_t) of this step."""
+    eps, pid = map_particles(dim, n, bc, S, pos, radius)
+    f, s = step(dim, n, bc, tau, g, S, f, eps_cnt=eps, pid=pid, pos=pos, vel=vel, omega=omega, want_s=True)
+    F, T, aF, aT = forces(dim, n, bc, s, pid, pos)
+    if verlet is None:
+        pos, vel, omega = dem_step(dim, n, bc, pos, vel, omega, radius, mass, F, T, kn, e, gp, dt)
+    else:
+        pos, vel, omega = dem_step_verlet(dim, n, bc, pos, vel, omega, radius, mass, F, T, kn, e, gp, verlet, dt)
+    return f, pos, vel, omega, dict(eps=eps, pid=pid, s=s, force=F, torque=T, abs_f=aF, abs_t=aT)
+
+
 def verlet_build(dim, n, bc, pos, radius, skin):
     """The neighbour lists by their definition (R19): CSR (start[P+1] int64, items int32), j ascending."""
     n3, bc3 = _n3(n), _bc3(bc)

@@ -25,12 +25,21 @@
  * section "Readings" (R1..R16 = SURVEY.md section 8(c) G1..G16).
  *
  * Parity pins (tests/test_oracle_pins.py): every function below is pinned by at
- * least one closed form / invariant / hand value, EXCEPT the conventions
+ * least one closed form / invariant / hand value, EXCEPT the convention
  *   - orc_map's choice of the covering particle when two particles share a node
  *     (R5: most samples, ties -> lowest index): "parity unpinned" (convention;
- *     brute-forced on tiny inputs only),
- *   - orc_dem_step's wall contact (R10) and the coupling order (R11):
- *     "parity unpinned" beyond the two-sphere bounce pins.
+ *     brute-forced on tiny inputs only).
+ * The wall contact of contact_forces (R10) is pinned by the static equilibrium of
+ * a sphere resting on the lower / upper wall (x = R - 1/2 - m|g|/k_n and its
+ * mirror) and by the first-contact law at all four walls of a 2D box
+ * (test_R10_*); the order of a coupled step (R11: map -> step -> forces -> DEM,
+ * load from the pre-collision state, held over the DEM step) lives in
+ * oracle/__init__.py: coupled_step and is pinned by two hand-derived steps of a
+ * light particle in a uniform stream (test_R11_*).
+ * Precision: everything is fp64 except the exchange vector s of a node and the
+ * per-particle sums of orc_forces, which are formed in long double and rounded
+ * once (R12: the literal sum_i Omega_i c_i cancels f-sized terms; see
+ * orc_collide_node).
  * The Verlet-list functions (orc_verlet_*, orc_dem_step_verlet, R19)
  * are pinned in tests/test_oracle_verlet_pins.py (hand lists, lattice shell
  * counts, bitwise equality with the all-pairs trajectory, rebuild counts).
@@ -100,6 +109,22 @@ static double feq_i(int dim, int i, double rho, const double *u) {
   return wgt(dim, i) * rho * (1.0 + 3.0 * cu + 4.5 * cu * cu - 1.5 * uu);
 }
 
+/* the same expression in long double (used only for the exchange vector s of
+ * orc_collide_node, see there) */
+static long double wgt_ld(int dim, int i) { /* the weights of R1 as long double quotients */
+  if (dim == 2) return i == 0 ? 4.0L / 9.0L : (i < 5 ? 1.0L / 9.0L : 1.0L / 36.0L);
+  return i == 0 ? 1.0L / 3.0L : (i < 7 ? 1.0L / 18.0L : 1.0L / 36.0L);
+}
+static long double feq_i_ld(int dim, int i, long double rho, const long double *u) {
+  const int *c = cvec(dim, i);
+  long double cu = 0.0L, uu = 0.0L;
+  for (int a = 0; a < dim; ++a) {
+    cu += c[a] * u[a];
+    uu += u[a] * u[a];
+  }
+  return wgt_ld(dim, i) * rho * (1.0L + 3.0L * cu + 4.5L * cu * cu - 1.5L * uu);
+}
+
 void orc_feq(int dim, double rho, const double *u, double *out /*[Q]*/) {
   int Q = nq(dim);
   for (int i = 0; i < Q; ++i) out[i] = feq_i(dim, i, rho, u);
@@ -138,10 +163,29 @@ void orc_collide_node(int dim, double tau, const double *g /*[3]*/,
     else
       omega[i] = 0.0;
   }
+  /* s = beta sum_{i>=1} Omega_i c_i, the literal sum, evaluated in long double:
+   * the sum cancels f-sized terms (|f| <= 0.45) down to rho (V_S - u), so in
+   * fp64 every node's s would carry an absolute rounding error of ~Q 2^-53 |f|
+   * ~ 1e-15 however small s is, which is 1e-10 of s itself on slowly moving
+   * nodes: not good enough to referee a 1e-10 relative force tolerance
+   * (R12).  rho and u are re-formed in long double from the same fp64
+   * f, Omega_i from them; the result is rounded once to fp64.  f* above/below
+   * keeps the paper's double precision. */
   s[0] = s[1] = s[2] = 0.0;
-  for (int i = 1; i < Q; ++i)
-    for (int a = 0; a < dim; ++a) s[a] += omega[i] * cvec(dim, i)[a];
-  for (int a = 0; a < 3; ++a) s[a] *= beta;
+  if (beta != 0.0) {
+    long double rl = 0.0L, ml[3] = {0.0L, 0.0L, 0.0L}, ul[3] = {0.0L, 0.0L, 0.0L};
+    long double vl[3] = {vs[0], vs[1], vs[2]}, sl[3] = {0.0L, 0.0L, 0.0L};
+    for (int i = 0; i < Q; ++i) rl += (long double)f[i];
+    for (int i = 0; i < Q; ++i)
+      for (int a = 0; a < dim; ++a) ml[a] += (long double)f[i] * cvec(dim, i)[a];
+    for (int a = 0; a < dim; ++a) ul[a] = ml[a] / rl;
+    for (int i = 1; i < Q; ++i) {
+      long double om = (long double)f[opp(i)] - (long double)f[i] +
+                       feq_i_ld(dim, i, rl, vl) - feq_i_ld(dim, opp(i), rl, ul);
+      for (int a = 0; a < dim; ++a) sl[a] += om * cvec(dim, i)[a];
+    }
+    for (int a = 0; a < dim; ++a) s[a] = (double)((long double)beta * sl[a]);
+  }
 
   for (int i = 0; i < Q; ++i) {
     const int *c = cvec(dim, i);
@@ -534,9 +578,14 @@ void orc_forces(int dim, const int64_t *n, const int32_t *bc, const double *s,
   int64_t nx = n[0], ny = n[1], nz = dim == 3 ? n[2] : 1;
   int64_t N = nx * ny * nz;
   int nt = dim == 2 ? 1 : 3;
+  /* the per-particle sums are accumulated in long double and rounded once (R12: the
+   * oracle must be well inside the 1e-10 relative tolerance it referees) */
+  long double *Fl = (long double *)calloc((size_t)(P > 0 ? P : 1) * 6, sizeof(long double));
+  long double *Tl = Fl + (size_t)(P > 0 ? P : 1) * 3;
   for (int64_t p = 0; p < P * dim; ++p) force[p] = 0.0;
   for (int64_t p = 0; p < P * nt; ++p) torque[p] = 0.0;
   for (int64_t p = 0; p < P; ++p) abs_f[p] = abs_t[p] = 0.0;
+  if (!Fl) return;
   for (int64_t k = 0; k < nz; ++k)
     for (int64_t j = 0; j < ny; ++j)
       for (int64_t i = 0; i < nx; ++i) {
@@ -550,20 +599,24 @@ void orc_forces(int dim, const int64_t *n, const int32_t *bc, const double *s,
         if (dim == 3) r[2] = (double)k - pos[2 * P + p];
         for (int a = 0; a < dim; ++a)
           if (bc[a] == 0) r[a] = min_image(r[a], n[a]);
-        for (int a = 0; a < dim; ++a) force[(int64_t)a * P + p] -= sv[a];
-        double t[3];
-        t[0] = r[1] * sv[2] - r[2] * sv[1];
-        t[1] = r[2] * sv[0] - r[0] * sv[2];
-        t[2] = r[0] * sv[1] - r[1] * sv[0];
+        for (int a = 0; a < dim; ++a) Fl[(int64_t)a * P + p] -= (long double)sv[a];
+        long double tl[3];
+        tl[0] = (long double)r[1] * sv[2] - (long double)r[2] * sv[1];
+        tl[1] = (long double)r[2] * sv[0] - (long double)r[0] * sv[2];
+        tl[2] = (long double)r[0] * sv[1] - (long double)r[1] * sv[0];
+        double t[3] = {(double)tl[0], (double)tl[1], (double)tl[2]};
         if (dim == 2) {
-          torque[p] -= t[2];
+          Tl[p] -= tl[2];
           abs_t[p] += fabs(t[2]);
         } else {
-          for (int a = 0; a < 3; ++a) torque[(int64_t)a * P + p] -= t[a];
+          for (int a = 0; a < 3; ++a) Tl[(int64_t)a * P + p] -= tl[a];
           abs_t[p] += sqrt(t[0] * t[0] + t[1] * t[1] + t[2] * t[2]);
         }
         abs_f[p] += sqrt(sv[0] * sv[0] + sv[1] * sv[1] + sv[2] * sv[2]);
       }
+  for (int64_t p = 0; p < P * dim; ++p) force[p] = (double)Fl[p];
+  for (int64_t p = 0; p < P * nt; ++p) torque[p] = (double)Tl[p];
+  free(Fl);
 }
 
 /* ------------------------------------------------------------------------ */

@@ -300,3 +300,17 @@ def sub_box(w, lo, size):
     idx = np.concatenate(keep_idx)
     pos = np.concatenate(keep_pos, axis=1)
     return pos, w.vel[:, idx].copy(), w.omega[:, idx].copy(), w.radius[idx].copy(), w.mass[idx].copy(), idx
+
+
+def y_slab(w, y_lo, y_hi):
+    """Particle set of workload w seen from the rows [y_lo, y_hi) of its lattice, all other axes kept whole:
+    every particle whose bounding box (centre +- (R + 2)) touches the slab, translated by -y_lo along y
+    (exact: centres are multiples of 2**-16, y_lo is an integer).  For a lattice of (n_x, y_hi - y_lo[, n_z]) nodes
+    whose y edges are walls.  The order of the particles is kept, so that "ties -> lowest index" picks the same
+    particle in the slab as in the whole lattice.  Returns (pos, vel, omega, radius, mass, idx)."""
+    y = w.pos[1]
+    m = (y + w.radius + 2.0 >= float(y_lo)) & (y - w.radius - 2.0 <= float(y_hi) - 1.0)
+    idx = np.nonzero(m)[0]
+    pos = w.pos[:, idx].copy()
+    pos[1] -= float(y_lo)
+    return pos, w.vel[:, idx].copy(), w.omega[:, idx].copy(), w.radius[idx].copy(), w.mass[idx].copy(), idx

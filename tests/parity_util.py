@@ -1,9 +1,11 @@
-"""Shared helpers of the GPU parity tests: run the CPU oracle and the CUDA path on
-the same seeded workload and compare them with the tolerances BASELINE.json's
-north_star states:
+"""Shared helpers of the GPU parity tests: run the CPU oracle and the CUDA path on the same seeded
+workload and compare them with the tolerances BASELINE.json's north_star states:
   lattice runs : max |f_gpu - f_cpu| <= 1e-12 * max |f|
-  forces/torque: |F_gpu - F_cpu| <= 1e-10 * max(|F_cpu|, 1e-3 * A_p) + n_p * 1e-15   (R12)
-                 (torque: the same with A_p = sum |r x s| and the floor times (R_p + 1))
+  forces/torque: |F_gpu - F_cpu| <= 1e-10 * max(|F_cpu|, 1e-3 * A_p)      (R12; A_p = sum_n |s_n| of particle p;
+                 torque: A_p = sum |r x s|).  NO additive floor: the oracle forms the exchange vectors and the
+                 per-particle sums in long double, so it is itself far inside 1e-10.  The one exception is a
+                 suspension in which fluid and particles are at rest with no driving force (true F = 0, both
+                 sides hold rounding noise of f): those callers pass floor=True, which adds n_p * 1e-15.
   eps / pid    : bit-exact
 """
 import numpy as np
@@ -48,28 +50,42 @@ def assert_fields_close(gpu_f, cpu_f, what="f", tol=F_TOL):
 
 
 def force_floor(pid, P):
-    """Absolute rounding floor of a per-particle sum of exchange vectors: the oracle's literal
-    sum_i Omega_i c_i cancels f-sized terms (|f| <= 0.45), so each node's s carries an absolute
-    rounding error of up to ~Q * 2^-53 * max|f| ~ 1e-15 whatever the size of s itself; a sum over
-    the n_p nodes of particle p cannot be trusted below n_p * 1e-15."""
+    """Rounding floor for suspensions AT REST (assert_forces_close(floor=True) only): f carries rounding
+    noise of ~2^-53 max|f| on both sides, so the velocity of a node is unknown below ~Q 2^-53 ~ 1e-15 and a
+    force whose true value is zero comes out as n_p * 1e-15 of noise on either side."""
     n_p = np.bincount(pid[pid >= 0].ravel(), minlength=P).astype(float)
     return 1e-15 * n_p
 
 
-def assert_forces_close(gF, gT, ref, tol=FORCE_TOL):
-    """R12: per particle, |dF| <= tol * max(|F|, 1e-3 * sum_n |s_n|) + n_p * 1e-15; same for the torque
-    with the floor scaled by the lever arm (R_p + 1)."""
+class ForceCheck(tuple):
+    """(force ratio, torque ratio) of the worst particle against the asserted bound, plus
+    .no_floor = the same two ratios against the plain R12 bound (no additive floor) and
+    .rel = worst |dF|/|F|, |dT|/|T| over the particles whose |F| (|T|) is above 1e-3 A_p."""
+    def __new__(cls, rF, rT, no_floor, rel):
+        self = super().__new__(cls, (rF, rT))
+        self.no_floor, self.rel = no_floor, rel
+        return self
+
+
+def assert_forces_close(gF, gT, ref, tol=FORCE_TOL, floor=False):
+    """R12: per particle |dF| <= tol * max(|F|, 1e-3 * sum_n |s_n|), same for the torque with sum |r x s|.
+    floor=True (suspensions at rest only, see the module text) adds n_p * 1e-15 (torque: times R_p + 1)."""
     F, T, aF, aT = ref["force"], ref["torque"], ref["abs_f"], ref["abs_t"]
-    floor = ref["floor"]
+    fl = ref["floor"] if floor else 0.0
     dF = np.sqrt(((gF - F) ** 2).sum(axis=0))
     nF = np.sqrt((F ** 2).sum(axis=0))
-    lim = tol * np.maximum(nF, 1e-3 * aF) + floor
-    assert (dF <= lim + 1e-300).all(), "force: worst ratio %.3e" % (dF / (lim + 1e-300)).max()
+    lim0 = tol * np.maximum(nF, 1e-3 * aF) + 1e-300
     dT = np.sqrt(((gT - T) ** 2).sum(axis=0))
     nT = np.sqrt((T ** 2).sum(axis=0))
-    limT = tol * np.maximum(nT, 1e-3 * aT) + floor * (ref["radius"] + 1.0)
-    assert (dT <= limT + 1e-300).all(), "torque: worst ratio %.3e" % (dT / (limT + 1e-300)).max()
-    return float((dF / (lim + 1e-300)).max()), float((dT / (limT + 1e-300)).max())
+    limT0 = tol * np.maximum(nT, 1e-3 * aT) + 1e-300
+    lim, limT = lim0 + fl, limT0 + fl * (ref["radius"] + 1.0)
+    rF, rT = float((dF / lim).max()), float((dT / limT).max())
+    assert rF <= 1.0, "force: worst ratio %.3e" % rF
+    assert rT <= 1.0, "torque: worst ratio %.3e" % rT
+    bigF, bigT = nF > 1e-3 * aF, nT > 1e-3 * aT
+    rel = (float((dF[bigF] / nF[bigF]).max()) if bigF.any() else 0.0,
+           float((dT[bigT] / nT[bigT]).max()) if bigT.any() else 0.0)
+    return ForceCheck(rF, rT, (float((dF / lim0).max()), float((dT / limT0).max())), rel)
 
 
 def gpu_run(lb, w, steps, f0=None, streaming=0):

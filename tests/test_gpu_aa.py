@@ -32,7 +32,7 @@ def test_aa_reduced_configs_fields_maps_forces(orc, lb, name, steps):
     assert_fields_close(got["rho"], ref["rho"], "rho")
     assert np.abs(got["u"] - ref["u"]).max() <= F_TOL * max(np.abs(ref["f"]).max(), np.abs(ref["u"]).max())
     assert np.abs(got["s"] - ref["s"]).max() <= F_TOL * np.abs(ref["f"]).max()
-    assert_forces_close(got["force"], got["torque"], ref)
+    assert_forces_close(got["force"], got["torque"], ref, floor=(name == "C5"))    # C5 cut: suspension at rest
     assert lat.time() == steps
     lat.close()
 
@@ -112,13 +112,10 @@ def test_aa_coupled_reduced_c5_windows(orc, lb):
         lat.set_distributions(f)
         lat.set_particles(pos, vel, om, w.radius, w.mass)
         for it in range(win):
-            eps, pid = orc.map_particles(w.dim, w.n, w.bc, w.subsamples, pos, w.radius)
-            f, s = orc.step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, eps_cnt=eps, pid=pid, pos=pos,
-                            vel=vel, omega=om, want_s=True)
-            F, T, aF, aT = orc.forces(w.dim, w.n, w.bc, s, pid, pos)
-            ref = dict(force=F, torque=T, abs_f=aF, abs_t=aT, floor=force_floor(pid, w.P), radius=w.radius)
-            pos, vel, om = orc.dem_step(w.dim, w.n, w.bc, pos, vel, om, w.radius, w.mass, F, T, d["kn"],
-                                        d["restitution"], d["g_particle"], d["dt"])
+            f, pos, vel, om, ref = orc.coupled_step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, pos, vel, om,
+                                                    w.radius, w.mass, d["kn"], d["restitution"], d["g_particle"], d["dt"])
+            eps, pid = ref["eps"], ref["pid"]
+            ref.update(floor=force_floor(pid, w.P), radius=w.radius)
             lat.map_particles()
             lat.step(1)
             gF, gT = lat.reduce_particle_forces()

@@ -89,12 +89,8 @@ def test_run_coupled_against_the_oracle(orc, lb):
     pos, vel, om = w.pos.copy(), w.vel.copy(), w.omega.copy()
     n = 8
     for _ in range(n):
-        eps, pid = orc.map_particles(w.dim, w.n, w.bc, w.subsamples, pos, w.radius)
-        f, s = orc.step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, eps_cnt=eps, pid=pid, pos=pos,
-                        vel=vel, omega=om, want_s=True)
-        F, T, _, _ = orc.forces(w.dim, w.n, w.bc, s, pid, pos)
-        pos, vel, om = orc.dem_step(w.dim, w.n, w.bc, pos, vel, om, w.radius, w.mass, F, T, d["kn"],
-                                    d["restitution"], d["g_particle"], d["dt"])
+        f, pos, vel, om, _ = orc.coupled_step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, pos, vel, om,
+                                              w.radius, w.mass, d["kn"], d["restitution"], d["g_particle"], d["dt"])
     lat = lb.from_workload(w)
     lat.run_coupled(n, d["kn"], d["restitution"], d["g_particle"], d["dt"])
     assert_fields_close(lat.fetch_fields(lb.FIELD_F), f)

@@ -160,3 +160,69 @@ def test_p2d_paper_size_sampled_boxes_and_mass(orc, lb):
     assert abs(d["mass"] - m0) / m0 < 1e-12
     assert abs((m0 - d["gas_area"]) / (w.P * np.pi * 25.0) - 1) < 5e-3
     lat.close()
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# The same check at step counts where rounding differences have accumulated (>= 50 steps; C4 and C2 boxes at the
+# configuration's / 200 steps): full-size lattice on the GPU, oracle on the box + rim.  ~2 minutes of oracle in all.
+# ----------------------------------------------------------------------------------------------------------------
+def test_c4_full_size_200_steps_sampled_boxes(orc, lb):
+    """BASELINE.json configs[3] at its size AND its step count (200), on sampled boxes."""
+    w = inputs.c4()
+    n = w.steps
+    assert n == 200
+    rim = n + 11
+    boxes = [((4000, 16000), (70 + 2 * rim, 70 + 2 * rim), (0, 0)),
+             ((-rim - 30, 0), (70 + 2 * rim, 70 + rim), (0, 1))]            # bottom wall, across the x seam
+    lat, worst = _check_boxes(orc, lb, w, n, boxes)
+    lat.close()
+
+
+def test_c2_full_size_200_steps_sampled_boxes(orc, lb):
+    """BASELINE.json configs[1] at its size, 200 of its 1,000 steps, on sampled boxes (spinning disks)."""
+    w = inputs.c2()
+    n = 200
+    rim = n + 11
+    boxes = [((300, 2000), (70 + 2 * rim, 70 + 2 * rim), (0, 0)),
+             ((700, 4096 - 70 - rim), (70 + 2 * rim, 70 + rim), (0, 1))]    # top wall, across the x seam
+    lat, worst = _check_boxes(orc, lb, w, n, boxes)
+    lat.close()
+
+
+def test_c3_full_size_50_steps_sampled_box(orc, lb):
+    """BASELINE.json configs[2] at its size, 50 steps, a box on the bottom wall."""
+    w = inputs.c3()
+    n = 50
+    rim = n + 11
+    boxes = [((100, 0, 90), (32 + 2 * rim, 32 + rim, 32 + 2 * rim), (0, 1, 0))]
+    lat, worst = _check_boxes(orc, lb, w, n, boxes)
+    lat.close()
+
+
+def test_c5_full_size_coupled_window(orc, lb):
+    """BASELINE.json configs[4] at its size: the first 12 coupled steps (map -> step -> reduce -> dem) of the whole
+    128 x 512 x 128 lattice with its 4,096 spheres, from the shared initial state."""
+    w = inputs.c5()
+    d = w.dem
+    dargs = (d["kn"], d["restitution"], d["g_particle"], d["dt"])
+    f = orc.init(w.dim, w.n)
+    pos, vel, om = w.pos.copy(), w.vel.copy(), w.omega.copy()
+    lat = lb.from_workload(w)
+    for it in range(12):
+        f, pos, vel, om, ref = orc.coupled_step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, pos, vel, om,
+                                                w.radius, w.mass, *dargs)
+        lat.map_particles()
+        lat.step(1)
+        gF, gT = lat.reduce_particle_forces()
+        if it in (1, 11):
+            assert np.array_equal(lat.fetch_fields(lb.FIELD_EPS_CNT), ref["eps"])
+            assert np.array_equal(lat.fetch_fields(lb.FIELD_PID), ref["pid"])
+            ref.update(floor=force_floor(ref["pid"], w.P), radius=w.radius)
+            assert_forces_close(gF, gT, ref)
+        lat.dem_step(*dargs)
+    gf = lat.fetch_fields(lb.FIELD_F)
+    assert np.abs(gf - f).max() <= F_TOL * np.abs(f).max()
+    pg, vg, og = lat.get_particles()
+    assert np.abs(pg - pos).max() < 1e-10 and np.abs(vg - vel).max() <= 1e-10 * np.abs(vel).max()
+    assert np.abs(vel).max() > 1e-5
+    lat.close()

@@ -96,13 +96,10 @@ def test_paper_suspension_coupled_windows(orc, lb, name, streaming):
         lat.set_distributions(f)
         lat.set_particles(pos, vel, om, w.radius, w.mass)
         for it in range(win):
-            eps, pid = orc.map_particles(w.dim, w.n, w.bc, w.subsamples, pos, w.radius)
-            f, s = orc.step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, eps_cnt=eps, pid=pid, pos=pos,
-                            vel=vel, omega=om, want_s=True)
-            F, T, aF, aT = orc.forces(w.dim, w.n, w.bc, s, pid, pos)
-            ref = dict(force=F, torque=T, abs_f=aF, abs_t=aT, floor=force_floor(pid, w.P), radius=w.radius)
-            pos, vel, om = orc.dem_step(w.dim, w.n, w.bc, pos, vel, om, w.radius, w.mass, F, T, d["kn"],
-                                        d["restitution"], d["g_particle"], d["dt"])
+            f, pos, vel, om, ref = orc.coupled_step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, pos, vel, om,
+                                                    w.radius, w.mass, d["kn"], d["restitution"], d["g_particle"], d["dt"])
+            eps, pid = ref["eps"], ref["pid"]
+            ref.update(floor=force_floor(pid, w.P), radius=w.radius)
             lat.map_particles()
             if it == 0:
                 assert np.array_equal(lat.fetch_fields(lb.FIELD_EPS_CNT), eps)

@@ -39,7 +39,8 @@ def test_reduced_configs_fields_maps_forces(orc, lb, name):
     assert np.abs(got["u"] - ref["u"]).max() <= F_TOL * max(np.abs(ref["f"]).max(), np.abs(ref["u"]).max())
     # s is a sum of f-sized terms that cancel (sum_i Omega_i c_i): its rounding scale is that of f
     assert np.abs(got["s"] - ref["s"]).max() <= F_TOL * np.abs(ref["f"]).max()
-    assert_forces_close(got["force"], got["torque"], ref)
+    # the fixed-particle cut of C5 is a suspension at rest (v = 0, no body force): true F = 0, noise on both sides
+    assert_forces_close(got["force"], got["torque"], ref, floor=(name == "C5"))
     assert lat.time() == w.steps
     lat.close()
 
@@ -291,13 +292,10 @@ def test_coupled_reduced_c5_windows(orc, lb):
         lat.set_distributions(f)
         lat.set_particles(pos, vel, om, w.radius, w.mass)
         for it in range(win):
-            eps, pid = orc.map_particles(w.dim, w.n, w.bc, w.subsamples, pos, w.radius)
-            f, s = orc.step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, eps_cnt=eps, pid=pid, pos=pos,
-                            vel=vel, omega=om, want_s=True)
-            F, T, aF, aT = orc.forces(w.dim, w.n, w.bc, s, pid, pos)
-            ref = dict(force=F, torque=T, abs_f=aF, abs_t=aT, floor=force_floor(pid, w.P), radius=w.radius)
-            pos, vel, om = orc.dem_step(w.dim, w.n, w.bc, pos, vel, om, w.radius, w.mass, F, T, d["kn"],
-                                        d["restitution"], d["g_particle"], d["dt"])
+            f, pos, vel, om, ref = orc.coupled_step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, pos, vel, om,
+                                                    w.radius, w.mass, d["kn"], d["restitution"], d["g_particle"], d["dt"])
+            eps, pid = ref["eps"], ref["pid"]
+            ref.update(floor=force_floor(pid, w.P), radius=w.radius)
             lat.map_particles()
             if it == 0:
                 assert np.array_equal(lat.fetch_fields(lb.FIELD_EPS_CNT), eps)

@@ -169,13 +169,10 @@ def test_coupled_reduced_c5_windows_with_lists(orc, lb):
         b0 = vs.builds
         g0 = lat.fetch_neighbor_list()[2]["builds"]
         for it in range(win):
-            eps, pid = orc.map_particles(w.dim, w.n, w.bc, w.subsamples, pos, w.radius)
-            f, s = orc.step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, eps_cnt=eps, pid=pid, pos=pos,
-                            vel=vel, omega=om, want_s=True)
-            F, T, aF, aT = orc.forces(w.dim, w.n, w.bc, s, pid, pos)
-            ref = dict(force=F, torque=T, abs_f=aF, abs_t=aT, floor=force_floor(pid, w.P), radius=w.radius)
-            pos, vel, om = orc.dem_step_verlet(w.dim, w.n, w.bc, pos, vel, om, w.radius, w.mass, F, T, d["kn"],
-                                               d["restitution"], d["g_particle"], vs, d["dt"])
+            f, pos, vel, om, ref = orc.coupled_step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, pos, vel, om,
+                                                    w.radius, w.mass, d["kn"], d["restitution"], d["g_particle"], d["dt"],
+                                                    verlet=vs)
+            ref.update(floor=force_floor(ref["pid"], w.P), radius=w.radius)
             lat.map_particles()
             lat.step(1)
             gF, gT = lat.reduce_particle_forces()

@@ -646,3 +646,122 @@ def test_dem_free_fall_and_spin_up(orc):
     assert abs(vel[2, 0] + 4e-3) < 1e-16
     inertia = 0.4 * 10.0 * 4.0
     assert abs(om[2, 0] - 4 * 0.08 / inertia) < 1e-16
+
+
+# ---------------------------------------------------------------- R10: the particle-wall contact, pinned
+@pytest.mark.parametrize("side", ["lower", "upper"])
+def test_R10_sphere_resting_on_a_wall_sits_at_the_static_equilibrium(orc, side):
+    """R10: the wall of a wall axis is the PLANE at -1/2 (lower) / n - 1/2 (upper), contact law of R8 with
+    R_j = 0.  A sphere pressed on it by gravity settles where k_n delta = m |g|, delta = R - (distance of the
+    centre to the plane):  x = R - 1/2 - m|g|/k_n,  mirrored  x = n - 1/2 - R + m|g|/k_n.  The resting point is a
+    fixed point of the integrator (a = 0), so after the damped settle it is met to rounding.  A plane at 0 or
+    at n (instead of -+1/2 outside the first / last node) is off by 0.5."""
+    dim, n, bc = 3, (20, 30, 20), (0, 1, 0)
+    R, m, e, tc, g = 5.0, 1000.0, 0.2, 40.0, 2e-4
+    kn = (math.pi ** 2 + math.log(e) ** 2) * m / tc ** 2          # wall: m_eff = m_i
+    delta = m * g / kn
+    if side == "lower":
+        x0, gp, want = R - 0.5 + 0.01, (0.0, -g, 0.0), R - 0.5 - delta
+    else:
+        x0, gp, want = n[1] - 0.5 - R - 0.01, (0.0, g, 0.0), n[1] - 0.5 - R + delta
+    pos = np.array([[10.0], [x0], [10.0]])
+    vel, om, z = np.zeros((3, 1)), np.zeros((3, 1)), np.zeros((3, 1))
+    radius, mass = np.array([R]), np.array([m])
+    for _ in range(3000):
+        pos, vel, om = orc.dem_step(dim, n, bc, pos, vel, om, radius, mass, z, z, kn, e, gp)
+    assert 0.01 < delta < 0.05
+    assert abs(pos[1, 0] - want) < 1e-12 and abs(vel[1, 0]) < 1e-14
+    assert pos[0, 0] == 10.0 and pos[2, 0] == 10.0 and np.abs(vel[[0, 2]]).max() == 0    # periodic axes: no wall
+
+
+def test_R10_wall_contact_starts_when_the_surface_crosses_the_plane_and_follows_the_law(orc):
+    """Force is exactly zero while x - R >= -1/2 (n - 1/2 - x >= R) and k_n delta - eta v_n the moment the
+    surface is through the plane, eta = -2 ln e sqrt(k_n m_i / (pi^2 + ln^2 e)) (m_eff = m_i, not m_i/2)."""
+    dim, n, bc = 2, (24, 17), (1, 1)
+    R, m, kn, e = 3.0, 80.0, 5.0, 0.7
+    eta = -2 * math.log(e) * math.sqrt(kn * m / (math.pi ** 2 + math.log(e) ** 2))
+    radius, mass = np.array([R]), np.array([m])
+    vel = np.array([[0.02], [-0.01]])
+    d = 2.0 ** -10
+    fc = lambda x, y: orc.contact_forces(dim, n, bc, np.array([[x], [y]]), vel, radius, mass, kn, e)[:, 0]
+    assert np.array_equal(fc(10.0, R - 0.5), [0.0, 0.0])                       # touching: delta = 0, no contact
+    assert np.array_equal(fc(n[0] - 0.5 - R, 8.0), [0.0, 0.0])
+    np.testing.assert_allclose(fc(10.0, R - 0.5 - d), [0.0, kn * d - eta * vel[1, 0]], rtol=1e-13)          # lower y
+    np.testing.assert_allclose(fc(10.0, n[1] - 0.5 - R + d), [0.0, -kn * d - eta * vel[1, 0]], rtol=1e-13)  # upper y
+    np.testing.assert_allclose(fc(R - 0.5 - d, 8.0), [kn * d - eta * vel[0, 0], 0.0], rtol=1e-13)           # lower x
+    np.testing.assert_allclose(fc(n[0] - 0.5 - R + d, 8.0), [-kn * d - eta * vel[0, 0], 0.0], rtol=1e-13)   # upper x
+    both = fc(R - 0.5 - d, n[1] - 0.5 - R + 2 * d)                             # a corner: the two walls add
+    np.testing.assert_allclose(both, [kn * d - eta * vel[0, 0], -2 * kn * d - eta * vel[1, 0]], rtol=1e-13)
+
+
+# ---------------------------------------------------------------- R11: the order of a coupled step, pinned
+@pytest.mark.parametrize("dim", [2, 3])
+def test_R11_coupling_order_two_steps_from_a_uniform_stream(orc, dim):
+    """R11 / BASELINE.json configs[4]: map -> LBM step -> force reduction -> DEM step, the hydrodynamic load
+    taken from the PRE-collision state and held over the DEM step.  One light particle at rest in a uniform
+    stream f = f^eq(1, u0).  Step 1 in closed form from the eps map alone (identity P6, s_n = beta_n rho (V_S - u)):
+      F_1 = u0 sum_n beta_n,  T_1 = sum_n beta_n r_n x u0,  v_1 = (F_1/m + g_p) dt,  x_1 = x_0 + v_1/2,  omega_1 = T_1/I.
+    Step 2 from the same identity with the fluid state after step 1, the map at the NEW position x_1 and the
+    NEW velocities v_1, omega_1.  Any other order fails: a DEM step that runs before the reduction leaves v_1 = g_p;
+    a map that is not redone, V_S from the old velocities, a load from the post-collision state or a load that acts
+    in only one of the two half kicks each change x_2, v_2 by far more than the tolerance."""
+    n = (24, 20) if dim == 2 else (16, 14, 12)
+    bc = (0,) * dim
+    S, tau, R, m, kn, e = (8 if dim == 2 else 4), 0.8, 3.5, (6.0 if dim == 2 else 30.0), 1.0, 0.9
+    u0 = np.array([0.02, -0.01, 0.015][:dim])
+    gp = np.array([0.0, -1e-3, 0.0][:dim])
+    nt = 1 if dim == 2 else 3
+    I = (0.5 if dim == 2 else 0.4) * m * R * R
+    radius, mass = np.array([R]), np.array([m])
+    shape = (1,) * (3 - dim) + tuple(reversed(n))
+    f = np.empty((orc.nq(dim),) + shape)
+    f[...] = orc.feq(dim, 1.0, u0).reshape((-1, 1, 1, 1))
+    pos = np.array([[11.3], [9.6], [5.45]][:dim])
+    vel, om = np.zeros((dim, 1)), np.zeros((nt, 1))
+
+    def load(f_pre, pos, vel, om):
+        """-sum s, -sum r x s with s = beta rho (V_S - u) over the covered nodes (P6), numpy only."""
+        eps, pid = orc.map_particles(dim, n, bc, S, pos, radius)
+        rho, u = orc.macros(dim, f_pre)
+        ee = eps.astype(float) / S ** dim
+        beta = ee * (tau - 0.5) / ((1 - ee) + (tau - 0.5))
+        kk, jj, ii = np.meshgrid(*[np.arange(v) for v in eps.shape], indexing="ij")
+        r = np.zeros((3,) + eps.shape)
+        for a, idx in enumerate((ii, jj, kk)[:dim]):
+            d = idx - pos[a, 0]
+            r[a] = np.where(d > n[a] / 2, d - n[a], np.where(d < -n[a] / 2, d + n[a], d))
+        w3 = np.array([0.0, 0.0, om[0, 0]]) if dim == 2 else om[:, 0]
+        V = np.cross(w3[None, :], r.reshape(3, -1).T).T.reshape(r.shape)
+        s = np.zeros_like(r)
+        for a in range(dim):
+            s[a] = beta * rho * (vel[a, 0] + V[a] - u[a])
+        F = -s.reshape(3, -1).sum(axis=1)
+        T = -np.cross(r.reshape(3, -1).T, s.reshape(3, -1).T).sum(axis=0)
+        return F[:dim], (T[2:] if dim == 2 else T), beta.sum(), eps
+
+    # closed form of step 1 from the eps map alone
+    F1, T1, B, eps0 = load(f, pos, vel, om)
+    np.testing.assert_allclose(F1, u0 * B, rtol=1e-13)
+    x, v, w = pos.copy(), vel.copy(), om.copy()
+    want = []
+    fo = f
+    for k in range(2):
+        F, T, _, eps_k = load(fo, x, v, w)
+        a = F / m + gp
+        x = x + (v[:, 0] + 0.5 * a)[:, None]
+        v = v + a[:, None]
+        w = w + (T / I)[:, None]
+        for c in range(dim):
+            x[c] = x[c] % n[c]
+        want.append((x.copy(), v.copy(), w.copy(), eps_k))
+        if k == 0:                                                   # the fluid after step 1: the oracle's own step
+            fo, *_ = orc.coupled_step(dim, n, bc, tau, (0,) * dim, S, f, pos, vel, om, radius, mass, kn, e, gp)
+    assert not np.array_equal(want[0][3], want[1][3])                # the particle moved enough to change the map
+    fo, p, vv, oo = f, pos, vel, om
+    for k in range(2):
+        fo, p, vv, oo, info = orc.coupled_step(dim, n, bc, tau, (0,) * dim, S, fo, p, vv, oo, radius, mass, kn, e, gp)
+        assert np.array_equal(info["eps"], want[k][3])
+        np.testing.assert_allclose(p, want[k][0], rtol=0, atol=1e-13)
+        np.testing.assert_allclose(vv, want[k][1], rtol=1e-12, atol=1e-16)
+        np.testing.assert_allclose(oo, want[k][2], rtol=1e-11, atol=1e-17)
+    assert np.abs(vv[:, 0] - gp * 2).max() > 1e-3                    # the hydrodynamic load dominates gravity
