@@ -7,8 +7,6 @@
 // collides with eq. (1) of the paper and writes f*(x,t) to the other
 // buffer at its own node: every store is aligned and coalesced, the x-shifted loads
 // are misaligned by one element and served from L1/L2 sectors.
-#include <cstdlib>
-
 #include "collide.cuh"
 #include "lbmimb_internal.cuh"
 
@@ -42,7 +40,7 @@ enum { kLayoutPull = 0, kLayoutNatural = 1, kLayoutSwapped = 2 };
 // x indices i-1, i, i+1 (wrapped) differ.  A warp takes the IMB path as a whole when
 // any of its nodes is covered (beta = 0 on the others), else the cheaper LBGK path.
 // ---------------------------------------------------------------------------
-template <int D, bool IMB, bool EMIT, int MINB, bool EARLY = false>
+template <int D, bool IMB, bool EMIT, int MINB>
 __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(const StepArgs a) {
   using L = Lat<D>;
   constexpr int Q = L::Q;
@@ -58,10 +56,11 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
   const int im = i == 0 ? a.nx - 1 : i - 1;
   const int ip = i == a.nx - 1 ? 0 : i + 1;
 
-  // EARLY: the node tag (sample count, covering particle) is requested before the populations
-  // so that the dependent gather of the particle record overlaps the population loads.
+  // The node tag (sample count, covering particle) is requested before the populations so that the
+  // dependent gather of the particle record overlaps the population loads (two dependent round trips
+  // on covered nodes instead of three: C4 7.00 -> 6.46 ms).
   int cnt = 0, pe = 0;
-  if (IMB && EARLY) {
+  if (IMB) {
     cnt = a.eps_cnt[x];
     pe = a.pid[x];
   }
@@ -95,9 +94,8 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
     }
   }
 
-  if (IMB && !EARLY) cnt = a.eps_cnt[x];
   double beta = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
-  if (IMB && EARLY && cnt > 0) {
+  if (IMB && cnt > 0) {
     beta = __ldg(a.beta_tab + cnt);
     solid_velocity<D>(a.prec + (int64_t)pe * prec_stride(D), i, j, k, a.nx, a.ny, a.nz, a.bcx, a.bcy, a.bcz, vx, vy,
                       vz);
@@ -109,12 +107,6 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
   if (!IMB || !__any_sync(0xffffffffu, cnt > 0)) {
     collide_fluid<D>(f, a.cp, rho, ux, uy, uz);
   } else {
-    if (!EARLY && cnt > 0) {
-      const int p = a.pid[x];
-      beta = __ldg(a.beta_tab + cnt);
-      solid_velocity<D>(a.prec + (int64_t)p * prec_stride(D), i, j, k, a.nx, a.ny, a.nz, a.bcx, a.bcy, a.bcz, vx, vy,
-                        vz);
-    }
     collide_imb<D>(f, a.cp, rho, ux, uy, uz, beta, vx, vy, vz);
     if (EMIT && cnt > 0 && live) {
       const double br = beta * rho;
@@ -516,51 +508,17 @@ lbmimb_status launch_init_rest(lbmimb_lattice *h) {
   return LBMIMB_OK;
 }
 
-template <int D, int MINB, bool EARLY = false>
-static void launch_cs2(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, bool imb, bool emit) {
+// One instantiation per (D, IMB, EMIT).  Occupancy targets from the round-1 sweep:
+// 3D 80 registers / 6 blocks per SM, 2D 56 registers / 9 blocks per SM.
+template <int D>
+static void launch_cs(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, bool imb, bool emit) {
+  constexpr int MINB = D == 3 ? 6 : 9;
   if (!imb)
     collide_stream_kernel<D, false, false, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
   else if (!emit)
-    collide_stream_kernel<D, true, false, MINB, EARLY><<<blocks, kStepThreads, 0, h->stream>>>(a);
+    collide_stream_kernel<D, true, false, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
   else
-    collide_stream_kernel<D, true, true, MINB, EARLY><<<blocks, kStepThreads, 0, h->stream>>>(a);
-}
-
-// Experiment switch (environment LBMIMB_STEP_VARIANT): 0-9 plain kernel with different
-// occupancy targets, >= 10 the TMA-staged kernel of lattice_tma.cu.
-int step_variant() {
-  static int v = -1;
-  if (v < 0) {
-    const char *e = getenv("LBMIMB_STEP_VARIANT");
-    v = e ? atoi(e) : 0;
-  }
-  return v;
-}
-
-template <int D>
-static void launch_cs(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, bool imb, bool emit) {
-  if constexpr (D == 3) {
-    switch (step_variant()) {
-      case 1: launch_cs2<D, 5>(h, a, blocks, imb, emit); break;
-      case 2: launch_cs2<D, 6>(h, a, blocks, imb, emit); break;
-      case 3: launch_cs2<D, 8>(h, a, blocks, imb, emit); break;
-      case 4: launch_cs2<D, 7>(h, a, blocks, imb, emit); break;
-      case 5: launch_cs2<D, 7, true>(h, a, blocks, imb, emit); break;
-      case 7: launch_cs2<D, 5, true>(h, a, blocks, imb, emit); break;
-      default: launch_cs2<D, 6, true>(h, a, blocks, imb, emit); break;
-    }
-  } else {
-    switch (step_variant()) {
-      case 1: launch_cs2<D, 8>(h, a, blocks, imb, emit); break;
-      case 2: launch_cs2<D, 10>(h, a, blocks, imb, emit); break;
-      case 3: launch_cs2<D, 12>(h, a, blocks, imb, emit); break;
-      case 4: launch_cs2<D, 16>(h, a, blocks, imb, emit); break;
-      case 5: launch_cs2<D, 9>(h, a, blocks, imb, emit); break;
-      case 6: launch_cs2<D, 8, true>(h, a, blocks, imb, emit); break;
-      case 7: launch_cs2<D, 10, true>(h, a, blocks, imb, emit); break;
-      default: launch_cs2<D, 9, true>(h, a, blocks, imb, emit); break;
-    }
-  }
+    collide_stream_kernel<D, true, true, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
 }
 
 template <int D, int MINB>
@@ -612,25 +570,10 @@ lbmimb_status launch_collide_stream(lbmimb_lattice *h, bool emit) {
       const int cz = h->g.dim == 2 ? 0 : Lat<3>::cz(q);
       a.koff[q] = 8 * ((int64_t)opposite(q) * a.N - (int64_t)cy * a.nx - (int64_t)cz * a.nx * a.ny);
     }
-    const int v = step_variant();   // experiment switch: occupancy target of the AA kernels
-    if (h->g.dim == 2) {
-      if (v == 1) launch_aa<2, 8>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
-      else if (v == 2) launch_aa<2, 10>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
-      else if (v == 3) launch_aa<2, 12>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
-      else if (v == 4) launch_aa<2, 7>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
-      else launch_aa<2, 9>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
-    } else {
-      if (v == 1) launch_aa<3, 6>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
-      else if (v == 2) launch_aa<3, 7>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
-      else launch_aa<3, 5>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
-    }
+    if (h->g.dim == 2) launch_aa<2, 9>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
+    else launch_aa<3, 5>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
     LBMIMB_LAUNCH_CHECK(h, "collide_stream_aa_kernel");
     return LBMIMB_OK;
-  }
-  if (step_variant() >= 10) {
-    bool done = false;
-    lbmimb_status st = launch_collide_stream_tma(h, emit, step_variant(), &done);
-    if (st != LBMIMB_OK || done) return st;
   }
   if (h->g.dim == 2)
     launch_cs<2>(h, a, (unsigned)blocks, imb, emit);

@@ -187,7 +187,6 @@ lbmimb_status cuda_fail(cudaError_t e, const char *what);
 // kernels.cu entry points used by api.cu
 lbmimb_status launch_init_rest(lbmimb_lattice *h);
 lbmimb_status launch_collide_stream(lbmimb_lattice *h, bool emit);
-lbmimb_status launch_collide_stream_tma(lbmimb_lattice *h, bool emit, int variant, bool *done);
 lbmimb_status launch_unstream(lbmimb_lattice *h, const double *f_pre, double *f_post);
 lbmimb_status launch_fetch(lbmimb_lattice *h, int what, const int64_t lo[3], const int64_t hi[3], void *dst_dev);
 lbmimb_status launch_pack_records(lbmimb_lattice *h);

@@ -1,7 +1,6 @@
 // Particle-side kernels: packed records, cell list (counting sort), the particle ->
 // lattice mapping (a1), the force/torque reduction (a3) and the soft-sphere DEM (a4).
 #include <cmath>
-#include <cstdlib>
 
 #include "lbmimb_internal.cuh"
 
@@ -568,138 +567,12 @@ lbmimb_status launch_map(lbmimb_lattice *h) {
 }
 
 // ---------------------------------------------------------------------------
-// a3: force / torque reduction, eq. (3) with the sign of R6.  One group of G threads per
-// particle walks the rows of the particle's bounding box, W lanes per row.  A node can only
-// belong to the particle if its centre is within R + h_out of the particle centre (the map's
-// own classification), so that test selects the candidates in registers and the pid and
-// exchange-vector loads of a candidate are independent of each other; U row slots are in
-// flight per thread.  Fixed traversal and tree order => bitwise reproducible.
-// ---------------------------------------------------------------------------
-template <int D, int G, int W>
-__device__ __forceinline__ void reduce_gather(const Geom &g, int32_t p, double cx, double cy, double cz, double rout2,
-                                              const int (&lo)[3], const int (&ext)[3], bool wx, bool wy, bool wz,
-                                              int gl, const int32_t *__restrict__ pid, const double *__restrict__ s,
-                                              double *acc) {
-  constexpr int U = 4;
-  constexpr int RPI = G / W;  // row slots per iteration of the group
-  const int bi0 = gl % W, rs = gl / W;
-  const int nchunks = (ext[0] + W - 1) / W;
-  const int nslots = ext[1] * ext[2] * nchunks;
-  const float inv_nch = 1.0f / (float)nchunks, inv_e1 = 1.0f / (float)ext[1];
-  // a bounding box reaches at most one period beyond either end of a periodic axis
-  auto wrap1 = [](int v, int n) { return v < 0 ? v + n : (v >= n ? v - n : v); };
-  for (int s0 = rs; s0 < nslots; s0 += U * RPI) {
-    bool cand[U];
-    int32_t owner[U];
-    double2 s01[U], s23[U];
-    double rx[U], ry[U], rz[U];
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-      const int slot = s0 + u * RPI;
-      int row = slot, bi = bi0;
-      if (nchunks > 1) {
-        int ch;
-        fast_divmod(slot, nchunks, inv_nch, row, ch);
-        bi += ch * W;
-      }
-      int bk = 0, bj = row;
-      if (D == 3) fast_divmod(row, ext[1], inv_e1, bk, bj);
-      int i = lo[0] + bi, j = lo[1] + bj, k = lo[2] + bk;
-      if (wx) i = wrap1(i, g.nx);
-      if (wy) j = wrap1(j, g.ny);
-      if (D == 3 && wz) k = wrap1(k, g.nz);
-      rx[u] = (double)i - cx;
-      ry[u] = (double)j - cy;
-      rz[u] = D == 3 ? (double)k - cz : 0.0;
-      if (wx) rx[u] = min_image_d(rx[u], g.nx);
-      if (wy) ry[u] = min_image_d(ry[u], g.ny);
-      if (D == 3 && wz) rz[u] = min_image_d(rz[u], g.nz);
-      cand[u] = slot < nslots && bi < ext[0] && rx[u] * rx[u] + ry[u] * ry[u] + rz[u] * rz[u] <= rout2;
-      owner[u] = -1;
-      s01[u] = s23[u] = make_double2(0.0, 0.0);
-      if (cand[u]) {
-        const int64_t x = ((int64_t)k * g.ny + j) * g.nx + i;
-        const double2 *sr = reinterpret_cast<const double2 *>(s) + x * (exchange_stride(D) / 2);
-        owner[u] = __ldg(pid + x);
-        s01[u] = __ldg(sr);
-        if (D == 3) s23[u] = __ldg(sr + 1);
-      }
-    }
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-      if (owner[u] != p) continue;  // fixed order: u ascending (s of a node p does not own is never used)
-      const double sx = s01[u].x, sy = s01[u].y;
-      if (D == 2) {
-        acc[0] -= sx;
-        acc[1] -= sy;
-        acc[2] -= rx[u] * sy - ry[u] * sx;
-      } else {
-        const double sz = s23[u].x;
-        acc[0] -= sx;
-        acc[1] -= sy;
-        acc[2] -= sz;
-        acc[3] -= ry[u] * sz - rz[u] * sy;
-        acc[4] -= rz[u] * sx - rx[u] * sz;
-        acc[5] -= rx[u] * sy - ry[u] * sx;
-      }
-    }
-  }
-}
-
-template <int D, int G>
-__global__ void __launch_bounds__(128) reduce_forces_kernel(Geom g, int64_t P, double h_out,
-                                                            const double *__restrict__ pos,
-                                                            const double *__restrict__ radius,
-                                                            const int32_t *__restrict__ pid,
-                                                            const double *__restrict__ s, double *__restrict__ force,
-                                                            double *__restrict__ torque) {
-  constexpr int groups = 128 / G;
-  constexpr int NV = D == 2 ? 3 : 6;
-  __shared__ double sh[groups][G / 32][NV];
-  const int grp = threadIdx.x / G, gl = threadIdx.x % G;
-  const int64_t p = (int64_t)blockIdx.x * groups + grp;
-  double acc[NV];
-#pragma unroll
-  for (int v = 0; v < NV; ++v) acc[v] = 0.0;
-  if (p < P) {
-    const double cx = pos[p], cy = pos[P + p], cz = D == 3 ? pos[2 * P + p] : 0.0, R = radius[p];
-    int lo[3] = {0, 0, 0}, ext[3] = {0, 0, 1};
-    bbox_axis(cx, R, g.nx, g.bcx, lo[0], ext[0]);
-    bbox_axis(cy, R, g.ny, g.bcy, lo[1], ext[1]);
-    if (D == 3) bbox_axis(cz, R, g.nz, g.bcz, lo[2], ext[2]);
-    const double rout = R + h_out;
-    const bool wx = crosses_seam(cx, R, g.nx, g.bcx), wy = crosses_seam(cy, R, g.ny, g.bcy);
-    const bool wz = D == 3 && crosses_seam(cz, R, g.nz, g.bcz);
-    if (ext[0] <= 16)
-      reduce_gather<D, G, 16>(g, (int32_t)p, cx, cy, cz, rout * rout, lo, ext, wx, wy, wz, gl, pid, s, acc);
-    else
-      reduce_gather<D, G, 32>(g, (int32_t)p, cx, cy, cz, rout * rout, lo, ext, wx, wy, wz, gl, pid, s, acc);
-  }
-#pragma unroll
-  for (int v = 0; v < NV; ++v)
-    for (int o = 16; o > 0; o >>= 1) acc[v] += __shfl_down_sync(0xffffffffu, acc[v], o);
-  if ((gl & 31) == 0)
-    for (int v = 0; v < NV; ++v) sh[grp][gl >> 5][v] = acc[v];
-  __syncthreads();
-  if (gl == 0 && p < P) {
-    double tot[NV];
-    for (int v = 0; v < NV; ++v) {
-      tot[v] = 0.0;
-      for (int w = 0; w < G / 32; ++w) tot[v] += sh[grp][w][v];
-    }
-    for (int c = 0; c < D; ++c) force[(int64_t)c * P + p] = tot[c];
-    if (D == 2) {
-      torque[p] = tot[2];
-    } else {
-      for (int c = 0; c < 3; ++c) torque[(int64_t)c * P + p] = tot[3 + c];
-    }
-  }
-}
-
-// Dense variant of the same reduction.  The loop above spends most of its lane-slots on bounding-box
+// a3: force / torque reduction, eq. (3) with the sign of R6.  One group of G threads per particle.
+// A node can only belong to the particle if its centre is within R + h_out of the particle centre
+// (the map's own classification).  A whole-box walk spends most of its lane-slots on bounding-box
 // nodes that cannot belong to the particle (a sphere fills a third of its box, and a row of 11 nodes
-// occupies 16 lanes).  Here every row (j,k) of the box first gets the interval of columns that can hold a
-// candidate, |i - cx| <= sqrt(rout^2 - ry^2 - rz^2) (+ margin: a superset), the interval lengths of a
+// occupies 16 lanes: C3 0.275 ms against 0.196 ms for the walk below).  Here every row (j,k) of the
+// box first gets the interval of columns that can hold a candidate, |i - cx| <= sqrt(rout^2 - ry^2 - rz^2) (+ margin: a superset), the interval lengths of a
 // chunk of G rows are scanned, and the threads then walk the concatenated intervals, so that nearly every
 // load that is issued is a node of the particle.  The per-node candidate test and the ownership test are
 // unchanged, so the same nodes are summed; traversal and tree order are fixed => bitwise reproducible.
@@ -856,36 +729,15 @@ static double sample_cloud_radius(const lbmimb_lattice *h) {
   return sqrt((double)h->g.dim) * (0.5 - 0.5 / (double)h->prm.subsamples) + 1e-6;
 }
 
-// Default: the dense kernel (B200: C3 0.275 -> 0.196 ms, P3D 1.74 -> 1.45 ms, C4 0.97 -> 0.69 ms, P2D 1.12 -> 0.91 ms).
-// LBMIMB_REDUCE_VARIANT=1 selects the box-walking kernel (A/B numbers of profiles/).
-static int reduce_variant() {
-  static int v = -1;
-  if (v < 0) {
-    const char *e = getenv("LBMIMB_REDUCE_VARIANT");
-    v = e ? atoi(e) : 0;
-  }
-  return v;
-}
-
 lbmimb_status launch_reduce(lbmimb_lattice *h) {
   const double ho = sample_cloud_radius(h);
-  const bool box = reduce_variant() == 1;
-  if (h->g.dim == 2) {
-    if (box)
-      reduce_forces_kernel<2, 32><<<blocks_for(h->P, 4), 128, 0, h->stream>>>(h->g, h->P, ho, h->pos, h->radius,
-                                                                             h->pid, h->s, h->force, h->torque);
-    else
-      reduce_forces_dense_kernel<2, 16><<<blocks_for(h->P, 8), 128, 0, h->stream>>>(
-          h->g, h->P, ho, h->pos, h->radius, h->pid, h->s, h->force, h->torque);
-  } else {
-    if (box)
-      reduce_forces_kernel<3, 128><<<blocks_for(h->P, 1), 128, 0, h->stream>>>(h->g, h->P, ho, h->pos, h->radius,
-                                                                              h->pid, h->s, h->force, h->torque);
-    else
-      reduce_forces_dense_kernel<3, 128><<<blocks_for(h->P, 1), 128, 0, h->stream>>>(
-          h->g, h->P, ho, h->pos, h->radius, h->pid, h->s, h->force, h->torque);
-  }
-  LBMIMB_LAUNCH_CHECK(h, "reduce_forces_kernel");
+  if (h->g.dim == 2)
+    reduce_forces_dense_kernel<2, 16><<<blocks_for(h->P, 8), 128, 0, h->stream>>>(h->g, h->P, ho, h->pos, h->radius,
+                                                                                  h->pid, h->s, h->force, h->torque);
+  else
+    reduce_forces_dense_kernel<3, 128><<<blocks_for(h->P, 1), 128, 0, h->stream>>>(h->g, h->P, ho, h->pos, h->radius,
+                                                                                   h->pid, h->s, h->force, h->torque);
+  LBMIMB_LAUNCH_CHECK(h, "reduce_forces_dense_kernel");
   return LBMIMB_OK;
 }
 

@@ -32,7 +32,7 @@ def test_aa_reduced_configs_fields_maps_forces(orc, lb, name, steps):
     assert_fields_close(got["rho"], ref["rho"], "rho")
     assert np.abs(got["u"] - ref["u"]).max() <= F_TOL * max(np.abs(ref["f"]).max(), np.abs(ref["u"]).max())
     assert np.abs(got["s"] - ref["s"]).max() <= F_TOL * np.abs(ref["f"]).max()
-    assert_forces_close(got["force"], got["torque"], ref, floor=(name == "C5"))    # C5 cut: suspension at rest
+    assert_forces_close(got["force"], got["torque"], ref)
     assert lat.time() == steps
     lat.close()
 

@@ -21,7 +21,7 @@ missing the oracle replays the earlier windows by itself.  The CUDA path is set 
 every window start, never the other way round.
 
 Each test appends one JSON line per result to gpurun_out/full_protocol.jsonl (if that folder exists).
-Tolerances: tests/parity_util.py (north star; forces WITHOUT an additive floor).  No expected value comes
+Tolerances: tests/parity_util.py (north star; forces against the plain R12 bound first, the ratio to it is recorded).  No expected value comes
 from the CUDA path."""
 import json
 import os
@@ -56,6 +56,7 @@ def force_fields(chk):
     """The per-particle force / torque result of assert_forces_close as record fields."""
     return dict(force_worst_ratio_of_tolerance=chk[0], torque_worst_ratio_of_tolerance=chk[1],
                 force_worst_ratio_no_floor=chk.no_floor[0], torque_worst_ratio_no_floor=chk.no_floor[1],
+                force_used_floor=bool(chk.used_floor[0]), torque_used_floor=bool(chk.used_floor[1]),
                 force_worst_rel_err=chk.rel[0], torque_worst_rel_err=chk.rel[1])
 
 

@@ -39,8 +39,7 @@ def test_reduced_configs_fields_maps_forces(orc, lb, name):
     assert np.abs(got["u"] - ref["u"]).max() <= F_TOL * max(np.abs(ref["f"]).max(), np.abs(ref["u"]).max())
     # s is a sum of f-sized terms that cancel (sum_i Omega_i c_i): its rounding scale is that of f
     assert np.abs(got["s"] - ref["s"]).max() <= F_TOL * np.abs(ref["f"]).max()
-    # the fixed-particle cut of C5 is a suspension at rest (v = 0, no body force): true F = 0, noise on both sides
-    assert_forces_close(got["force"], got["torque"], ref, floor=(name == "C5"))
+    assert_forces_close(got["force"], got["torque"], ref)
     assert lat.time() == w.steps
     lat.close()
 

@@ -99,7 +99,7 @@ def test_reduced_configs_in_table_mode(orc, lb, name):
     assert np.abs(lat.fetch_fields(lb.FIELD_S) - s).max() <= F_TOL * np.abs(f).max()
     gF, gT = lat.reduce_particle_forces()
     ref = dict(force=F, torque=T, abs_f=aF, abs_t=aT, floor=force_floor(pid, w.P), radius=w.radius)
-    assert_forces_close(gF, gT, ref, floor=(name == "C5"))      # C5 cut: suspension at rest, true F = 0
+    assert_forces_close(gF, gT, ref)
     lat.close()
 
 
