@@ -17,6 +17,8 @@ north_star target (>= 70 % of HBM bandwidth for the fused D3Q19 step) is quoted 
 `cpu_baseline` = the CPU oracle (tests' reference, never tuned) timed on a bounded sample.
 N > 1: "replicas only": N independent replicas, one per GPU, no data-path collective.
 `--impl reference` times the oracle itself (rank 0 only).
+The default run (workload C3) also measures C4, BASELINE.json's "Throughput run" (configs[3]), after the C3
+handle is destroyed (the two do not fit one GPU together), and reports it as `secondary` in the same line.
 """
 import argparse
 import json
@@ -36,9 +38,16 @@ METRIC = "fp64 LBM-IMB MLUPS on 1 B200 and % of HBM roofline (bytes/update count
 UNIT = "MLUPS"
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused kernel from the committed
-# `ncu --set full` capture (profiles/r1_traffic.md); None where no capture exists for the workload.
-NCU_TRAFFIC_BYTES = {"C3": 20850708000, "C4": 41871111000}   # profiles/r1_traffic.md
+def profiled_traffic(workload, streaming):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused kernel, from the committed
+    `ncu --set full` capture of this round (profiles/r2_traffic.json names the capture, the kernel and the
+    commit it was taken at).  Not measured in this run: None where no capture exists for the combination."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.json")) as fh:
+            rec = json.load(fh)["%s/%s" % (workload, streaming)]
+        return rec["dram_bytes_per_launch"], "profiles/r2_traffic.json (%s, commit %s)" % (rec["kernel"], rec["commit"])
+    except Exception:
+        return None, None
 
 
 def measured_peak_gbs():
@@ -187,50 +196,16 @@ def run_reference(args):
     return 0
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
-    ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--workload", default="C3", choices=["C2", "C3", "C4", "C5", "P2D", "P3D"],
-                    help="C2..C5 = BASELINE.json configs; P2D / P3D = the paper's own suspensions at full size "
-                         "(PAPER.md:117, Table 2; coupled with DEM; P3D needs --streaming aa, the default for it)")
-    ap.add_argument("--impl", default="lbmimb", choices=["lbmimb", "reference"])
-    ap.add_argument("--map-mode", default="sampling", choices=["sampling", "table"],
-                    help="a1 variant: sub-cell sampling (BASELINE.json configs) or the paper's table look-up")
-    ap.add_argument("--streaming", default=None, choices=["ab", "aa"],
-                    help="a2 variant: pull with two arrays (A-B) or in-place AA-pattern on one array")
-    ap.add_argument("--neighbor-mode", default="cells", choices=["cells", "verlet"],
-                    help="a4 variant (coupled workloads C5 / P2D / P3D): cell list rebuilt every step, or the paper's "
-                         "neighbour lists (PAPER.md:69, DESIGN.md R19)")
-    ap.add_argument("--skin", type=float, default=1.0, help="neighbour-list skin in lattice units")
-    ap.add_argument("--every", type=int, default=100, help="neighbour lists are at most this many steps old")
-    ap.add_argument("--coupled-api", action="store_true",
-                    help="coupled workloads: also time lbmimb_run_coupled (the same loop replayed from a CUDA graph)")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    args = ap.parse_args()
-    if args.streaming is None:      # 2 x 80.3 GB of distributions do not fit one B200: P3D runs in place
-        args.streaming = "aa" if args.workload == "P3D" else "ab"
-    if args.impl == "reference":
-        return run_reference(args)
-    if args.warmup < 3:
-        args.warmup = 3
-
-    import torch
-    from paper_1011_2613_b200 import binding as lb, replicas
-    rank, world, local = replicas.init_from_env()
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the lbmimb path has no CPU fallback")
-    torch.cuda.set_device(local)
-    w = get_workload(args.workload)
+def measure(args, name, lb, replicas, torch, rank, world, local, streaming, want_e2e, want_coupled, sampler_index):
+    """Times one workload on this rank's GPU; returns the pieces of the JSON line (rank 0) or None."""
+    w = get_workload(name)
     lat = lb.from_workload(w, device=local, map_mode=lb.MAP_TABLE if args.map_mode == "table" else lb.MAP_SAMPLING,
-                           streaming=lb.STREAM_AA if args.streaming == "aa" else lb.STREAM_AB)
+                           streaming=lb.STREAM_AA if streaming == "aa" else lb.STREAM_AB)
     dem = w.dem
     if args.neighbor_mode == "verlet":
         lat.set_neighbor_mode(lb.NEIGHBOR_VERLET, args.skin, args.every)
     Q = w.Q
-    bytes_per_node = 2 * Q * 8 + 1 + 4
+    bytes_per_node = 2 * Q * 8 + 1 + 4        # SURVEY.md 8(d): distributions + eps count + particle id
     N = w.nodes
 
     def whole_step():
@@ -240,7 +215,7 @@ def main():
         if dem:
             lat.dem_step(dem["kn"], dem["restitution"], dem["g_particle"], dem["dt"])
 
-    sampler = ClockSampler(local)
+    sampler = ClockSampler(sampler_index)
     if rank == 0:
         sampler.start()          # nvidia-smi needs a few hundred ms to deliver its first sample
     for _ in range(args.warmup):
@@ -278,7 +253,7 @@ def main():
 
     # ---- end to end through host buffers ------------------------------------------------------
     e2e = None
-    if not args.no_e2e:
+    if want_e2e:
         P, D, nt = w.P, w.dim, (1 if w.dim == 2 else 3)
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
         hpos, hvel, hom, hrad, hmass = pin(w.pos), pin(w.vel), pin(w.omega), pin(w.radius), pin(w.mass)
@@ -317,11 +292,12 @@ def main():
 
     lat.synchronize()
     coupled = None
-    if dem and args.coupled_api:      # the same K steps through ONE call: launches replayed from a CUDA graph
+    if dem and want_coupled:      # the same K steps through ONE call: launches replayed from a CUDA graph
         dargs = (dem["kn"], dem["restitution"], dem["g_particle"], dem["dt"])
         lat.run_coupled(5, *dargs)
         replicas.barrier()
         torch.cuda.synchronize()
+        l0 = lat.launch_count()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
         lat.run_coupled(args.steps, *dargs)
@@ -330,7 +306,8 @@ def main():
         replicas.barrier()
         c_units, c_ms = replicas.aggregate(float(N) * args.steps, a.elapsed_time(b))
         coupled = {"value": replicas.mlups(c_units, c_ms), "unit": UNIT, "ms_per_step": c_ms / args.steps,
-                   "call": "lbmimb_run_coupled(%d)" % args.steps}
+                   "call": "lbmimb_run_coupled(%d)" % args.steps,
+                   "launches_per_step": (lat.launch_count() - l0) / float(args.steps)}
     diag = diag_ms = None
     if dem:                        # the Figs. 5/7 time-series sample: one device reduction per output step
         lat.map_particles()
@@ -342,47 +319,110 @@ def main():
         diag_ms = a.elapsed_time(b)
         diag = {"slip_y": float(dd["slip"][1]), "drag_y": float(dd["drag"][1]), "t": lat.time()}
     nl_info = lat.fetch_neighbor_list()[2] if (dem and args.neighbor_mode == "verlet") else None
+    version = lb.version()
+    lat.close()
+    del lat
+    torch.cuda.empty_cache()
     if rank != 0:
-        lat.close()
-        replicas.shutdown()
-        return 0
+        return None
 
     peak, peak_src = measured_peak_gbs()
     achieved = bytes_per_node * N / (kern_ms * 1e-3) / 1e9
-    roof = {"bound": "hbm", "kernel": ("collide_stream_aa_kernel<%d,IMB,EMIT,even|odd>" if args.streaming == "aa"
-                                       else "collide_stream_kernel<%d,IMB,EMIT>") % w.dim, "achieved": achieved,
-            "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload) if args.streaming == "ab" else None, "peak_source": peak_src,
-            "bytes_per_node": bytes_per_node, "nodes_per_launch": N, "kernel_ms": kern_ms,
+    traffic, traffic_src = profiled_traffic(name, streaming)
+    roof = {"bound": "hbm", "kernel": ("collide_stream_aa_kernel<%d,IMB,forces,even|odd>" if streaming == "aa"
+                                       else "collide_stream_kernel<%d,IMB,forces>") % w.dim, "achieved": achieved,
+            "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
+            "peak_source": peak_src, "bytes_per_node": bytes_per_node, "nodes_per_launch": N, "kernel_ms": kern_ms,
             "kernel_mlups": N / (kern_ms * 1e-3) / 1e6, "frac_of_nominal_8TBs": achieved / 8000.0,
-            "kernel_share_of_step": kern_ms / (total_ms / args.steps)}
-    if args.streaming == "aa":      # the AA array is in its swapped layout after an odd number of steps
+            "kernel_share_of_step": kern_ms / (total_ms / args.steps),
+            "whole_step_frac": bytes_per_node * N / (ms_max / args.steps * 1e-3) / 1e9 / peak}
+    if streaming == "aa":      # the AA array is in its swapped layout after an odd number of steps
         odd = (t_begin + np.arange(args.steps)) % 2 == 1
         roof["kernel_ms_even_step"] = float(seg[~odd, 1].mean()) if (~odd).any() else None
         roof["kernel_ms_odd_step"] = float(seg[odd, 1].mean()) if odd.any() else None
-    cpu = None
-    if not args.no_cpu_baseline:
-        v, cores, desc, secs = oracle_sample(args.workload)
-        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": secs}
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "lattice": list(w.n), "Q": Q, "particles": w.P, "tau": w.tau,
-                       "bc": list(w.bc), "map_mode": args.map_mode, "streaming": args.streaming,
+    return {"value": value, "ms_per_step": ms_max / args.steps,
+            "config": {"workload": name, "lattice": list(w.n), "Q": Q, "particles": w.P, "tau": w.tau,
+                       "bc": list(w.bc), "map_mode": args.map_mode, "streaming": streaming,
                        "step": "map_particles + step(1) + reduce_particle_forces" +
                        (" + dem_step" if dem else ""),
                        "neighbor_mode": (args.neighbor_mode + (" skin=%g every=%d" % (args.skin, args.every)
                                                                if args.neighbor_mode == "verlet" else "")) if dem else None,
                        "parallelism": "replicas x%d" % world,
+                       "env": {k: os.environ[k] for k in ("LBMIMB_NO_GRAPH",) if k in os.environ},
                        "l2": "inputs (%.1f GB of distributions) exceed the 126 MB L2; no flush needed" %
-                       ((1 if args.streaming == "aa" else 2) * Q * N * 8 / 1e9)},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu,
+                       ((1 if streaming == "aa" else 2) * Q * N * 8 / 1e9)},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roof,
             "breakdown_ms": {"map_particles": float(seg[:, 0].mean()), "step": kern_ms,
                              "reduce_particle_forces": float(seg[:, 2].mean()),
                              "dem_step": float(seg[:, 3].mean()) if dem else 0.0, "diagnostics_once": diag_ms},
-            "diagnostics": diag, "neighbor_list": nl_info, "coupled_api": coupled,
-            "version": lb.version()}
+            "diagnostics": diag, "neighbor_list": nl_info, "coupled_api": coupled, "version": version}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--workload", default="C3", choices=["C2", "C3", "C4", "C5", "P2D", "P3D"],
+                    help="C2..C5 = BASELINE.json configs; P2D / P3D = the paper's own suspensions at full size "
+                         "(PAPER.md:117, Table 2; coupled with DEM; P3D needs --streaming aa, the default for it)")
+    ap.add_argument("--impl", default="lbmimb", choices=["lbmimb", "reference"])
+    ap.add_argument("--map-mode", default="sampling", choices=["sampling", "table"],
+                    help="a1 variant: sub-cell sampling (BASELINE.json configs) or the paper's table look-up")
+    ap.add_argument("--streaming", default=None, choices=["ab", "aa"],
+                    help="a2 variant: pull with two arrays (A-B) or in-place AA-pattern on one array")
+    ap.add_argument("--neighbor-mode", default="cells", choices=["cells", "verlet"],
+                    help="a4 variant (coupled workloads C5 / P2D / P3D): cell list rebuilt every step, or the paper's "
+                         "neighbour lists (PAPER.md:69, DESIGN.md R19)")
+    ap.add_argument("--skin", type=float, default=1.0, help="neighbour-list skin in lattice units")
+    ap.add_argument("--every", type=int, default=100, help="neighbour lists are at most this many steps old")
+    ap.add_argument("--coupled-api", action="store_true",
+                    help="coupled workloads: also time lbmimb_run_coupled (the same loop replayed from a CUDA graph)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true",
+                    help="default workload only: skip the second measurement on C4 (BASELINE.json's 'Throughput run')")
+    args = ap.parse_args()
+    if args.streaming is None:      # 2 x 80.3 GB of distributions do not fit one B200: P3D runs in place
+        args.streaming = "aa" if args.workload == "P3D" else "ab"
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.warmup < 3:
+        args.warmup = 3
+
+    import torch
+    from paper_1011_2613_b200 import binding as lb, replicas
+    rank, world, local = replicas.init_from_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the lbmimb path has no CPU fallback")
+    torch.cuda.set_device(local)
+    main_res = measure(args, args.workload, lb, replicas, torch, rank, world, local, args.streaming,
+                       not args.no_e2e, args.coupled_api, local)
+    second = None
+    if args.workload == "C3" and args.streaming == "ab" and not args.no_secondary:
+        second = measure(args, "C4", lb, replicas, torch, rank, world, local, "ab", False, False, local)
+    if rank != 0:
+        replicas.shutdown()
+        return 0
+    cpu = None
+    if not args.no_cpu_baseline:
+        v, cores, desc, secs = oracle_sample(args.workload)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": secs}
+    line = {"metric": METRIC, "value": main_res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": main_res["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic"}
+    for k in ("config", "clocks", "e2e", "gpu_launches", "roofline"):
+        line[k] = main_res[k]
+    line["cpu_baseline"] = cpu
+    for k in ("breakdown_ms", "diagnostics", "neighbor_list", "coupled_api", "version"):
+        line[k] = main_res[k]
+    if second is not None:      # BASELINE.json configs[3], measured in the same invocation with its own clock sample
+        line["secondary"] = {"workload": "C4", "metric": METRIC, "unit": UNIT, "value": second["value"],
+                             "ms_per_step": second["ms_per_step"], "steps": args.steps, "warmup": args.warmup,
+                             "roofline": second["roofline"], "breakdown_ms": second["breakdown_ms"],
+                             "clocks": second["clocks"], "gpu_launches": second["gpu_launches"],
+                             "config": second["config"]}
     print(json.dumps(line))
-    lat.close()
     replicas.shutdown()
     return 0
 

@@ -31,6 +31,11 @@
  * Errors: every call returns an lbmimb_status; nothing throws or aborts across the ABI.
  * On error the handle stays valid and, where possible, unchanged; lbmimb_last_error()
  * returns a thread-local description of the last failure on the calling thread.
+ * Errors that only a kernel can detect (the list of nodes shared by several particles overflowed, a
+ * neighbour list or a cell of its build grid overflowed: particle sets that overlap far more deeply than
+ * soft spheres in contact do) are reported as ESTATE by the next call that synchronises: synchronize,
+ * get_particles, fetch_fields, diagnostics, fetch_neighbor_list and reduce_particle_forces with host outputs.
+ * The flags are cleared by the next map_particles / set_particles.
  *
  * Ordering: the set_, get_ and fetch_ calls and reduce_particle_forces with non-NULL host outputs are
  * complete when they return; map_particles, step, dem_step and the _dev variants are
@@ -68,8 +73,15 @@ typedef struct {
   void *workspace_dev;      /* optional caller-owned device buffer, 256-byte aligned; NULL = library allocates */
   uint64_t workspace_bytes; /* size of workspace_dev; must be >= lbmimb_workspace_bytes() */
   int32_t streaming;  /* LBMIMB_STREAM_AB (0, default) or LBMIMB_STREAM_AA: how step() propagates, see below */
-  int32_t reserved;   /* must be 0 */
+  int32_t flags;      /* 0, or LBMIMB_FLAG_EXCHANGE_FIELD */
 } lbmimb_params;
+
+/*
+ * flags.  EXCHANGE_FIELD: keep the exchange vector s of every covered node of the last step in device memory
+ * (2 or 4 doubles per node) so that lbmimb_fetch_fields(LBMIMB_FIELD_S) can return it -- a diagnostic / test
+ * output.  The per-particle force and torque never need it: they are summed inside the fused step.
+ */
+#define LBMIMB_FLAG_EXCHANGE_FIELD 1
 
 /*
  * Streaming schemes of a2 (same results up to rounding order; both are fused collide-and-stream kernels):
@@ -77,8 +89,8 @@ typedef struct {
  *   AA: in-place AA-pattern on ONE array (Q x N doubles): even steps touch only the own node, odd steps
  *       gather from and scatter to the neighbours.  Halves the footprint, which is what lets the paper's
  *       512 x 2016 x 512 D3Q19 lattice (80.3 GB of distributions) fit one 180 GB B200.
- *       In AA mode fetch_fields stages through a temporary device buffer of the box's size (ENOMEM if
- *       that cannot be allocated: fetch sub-boxes of a large lattice).
+ *       In AA mode fetch_fields stages through a grow-only device buffer of the largest box fetched so far,
+ *       allocated by the library outside the workspace (ENOMEM if that fails: fetch sub-boxes of a large lattice).
  */
 enum { LBMIMB_STREAM_AB = 0, LBMIMB_STREAM_AA = 1 };
 
@@ -96,7 +108,8 @@ enum {
   LBMIMB_FIELD_U = 2,       /* double [D][box]  bare u = sum_i f_i c_i / rho (no half-force shift, R2) */
   LBMIMB_FIELD_EPS_CNT = 3, /* uint8  [box]     inside-sample count n_s, eps = n_s / S^D */
   LBMIMB_FIELD_PID = 4,     /* int32  [box]     covering particle, -1 = none */
-  LBMIMB_FIELD_S = 5        /* double [D][box]  exchange vector s of the last step (0 where eps = 0) */
+  LBMIMB_FIELD_S = 5        /* double [D][box]  exchange vector s of the last step (0 where eps = 0); needs
+                               LBMIMB_FLAG_EXCHANGE_FIELD, else ESTATE */
 };
 
 /*
@@ -132,8 +145,9 @@ uint64_t lbmimb_workspace_bytes(const lbmimb_params *params, int64_t max_particl
 
 /*
  * a0. Creates a lattice at rest: f_i = f_i^eq(rho=1, u=0) = w_i on every node, time t = 0, no
- * particles.  max_particles >= 0 bounds later set_particles calls.  *out receives the handle.
- * EINVAL: bad dim / n / bc / tau <= 0.5 / S^dim > 255; ENOMEM; ECUDA (no device, ...).
+ * particles.  0 <= max_particles <= 2^24 bounds later set_particles calls (a node's tag word holds the
+ * sample count in 8 bits and the covering particle in 24).  *out receives the handle.
+ * EINVAL: bad dim / n / bc / tau <= 0.5 / S^dim > 255 / flags / max_particles; ENOMEM; ECUDA (no device, ...).
  */
 lbmimb_status lbmimb_create_lattice(const lbmimb_params *params, int64_t max_particles,
                                     lbmimb_lattice **out);
@@ -177,7 +191,9 @@ lbmimb_status lbmimb_fetch_eps_table(lbmimb_lattice *h, uint8_t *dst, int64_t ca
  * a2. nsteps fused collide-and-stream steps of eq. (1) with beta,
  * Omega^S of eq. (2) driven by V_S = v_p + omega_p x (x_node - x_p), the body
  * force F_i (R3) and periodic / half-way bounce-back streaming.  Advances t by nsteps.
- * The per-node exchange vectors s = beta sum_i Omega_i c_i are kept for the LAST step only.
+ * The LAST step of the call also forms, inside the same kernel, the per-particle sums of eq. (3) over the
+ * exchange vectors s = beta sum_i Omega_i c_i = beta rho (V_S - u) of its covered nodes (and keeps s per node
+ * if the lattice has LBMIMB_FLAG_EXCHANGE_FIELD).
  * ESTATE if particles are set but not mapped.  nsteps = 0 is a no-op.  Asynchronous.
  */
 lbmimb_status lbmimb_step(lbmimb_lattice *h, int32_t nsteps);
@@ -186,8 +202,10 @@ lbmimb_status lbmimb_step(lbmimb_lattice *h, int32_t nsteps);
  * a3. Hydrodynamic force and torque on every particle from the last step's exchange vectors,
  * eq. (3) with the sign of R6 (force ON the particle):
  *   F_p = - sum_{n: pid=p} s_n,   T_p = - sum_n (x_n - x_p) x s_n   (minimum image), h^D/dt = 1.
- * Deterministic (fixed summation order).  force / torque may be NULL: results stay on the
- * device for dem_step; otherwise they are copied to the host and the call is synchronous.
+ * The sums were formed by the last step (runs of a particle's nodes are pre-summed per warp in a fixed tree
+ * and added as 64-bit fixed-point integers, resolution 2^-92, so the result does not depend on the order
+ * in which thread blocks ran: bitwise reproducible); this call converts them.  force / torque may be NULL:
+ * results stay on the device for dem_step; otherwise they are copied to the host and the call is synchronous.
  * ESTATE if no step has run since the last map_particles.
  */
 lbmimb_status lbmimb_reduce_particle_forces(lbmimb_lattice *h, double *force, double *torque);
@@ -275,7 +293,9 @@ lbmimb_status lbmimb_diagnostics(lbmimb_lattice *h, double *out);
 /* Replaces all distributions: f[Q][nz][ny][nx] = f_i(x, t) as LBMIMB_FIELD_F returns them. */
 lbmimb_status lbmimb_set_distributions(lbmimb_lattice *h, const double *f);
 
-/* Device-pointer variants (asynchronous on the handle's stream; same layouts). */
+/* Device-pointer variants (same layouts).  reduce_particle_forces_dev is asynchronous on the handle's stream;
+ * set_particles_dev first checks the arrays with a kernel (same conditions as set_particles; one small
+ * read-back, so it synchronises) and commits nothing on EINVAL. */
 lbmimb_status lbmimb_set_particles_dev(lbmimb_lattice *h, int64_t P, const double *pos_dev,
                                        const double *vel_dev, const double *omega_dev,
                                        const double *radius_dev, const double *mass_dev);

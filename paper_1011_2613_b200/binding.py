@@ -18,6 +18,7 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE = range(5)
 FIELD_F, FIELD_RHO, FIELD_U, FIELD_EPS_CNT, FIELD_PID, FIELD_S = range(6)
 MAP_SAMPLING, MAP_TABLE = 0, 1
 STREAM_AB, STREAM_AA = 0, 1
+FLAG_EXCHANGE_FIELD = 1
 NEIGHBOR_CELLS, NEIGHBOR_VERLET = 0, 1
 TABLE_DEN = 255
 TABLE_SHAPE = {2: (128, 32), 3: (128, 16, 16)}      # LBMIMB_TABLE_ND/NT_* of include/lbmimb.h
@@ -38,7 +39,7 @@ class Params(C.Structure):
     _fields_ = [("dim", C.c_int32), ("subsamples", C.c_int32), ("n", C.c_int64 * 3), ("bc", C.c_int32 * 3),
                 ("device", C.c_int32), ("tau", C.c_double), ("g_fluid", C.c_double * 3), ("stream", C.c_void_p),
                 ("workspace_dev", C.c_void_p), ("workspace_bytes", C.c_uint64), ("streaming", C.c_int32),
-                ("reserved", C.c_int32)]
+                ("flags", C.c_int32)]
 
 
 class DemParams(C.Structure):
@@ -121,7 +122,7 @@ def version():
 
 
 def make_params(dim, n, bc, tau, g_fluid, subsamples, device=0, stream=0, workspace_dev=0, workspace_bytes=0,
-                streaming=STREAM_AB):
+                streaming=STREAM_AB, flags=0):
     p = Params()
     p.dim = dim
     p.subsamples = subsamples
@@ -138,7 +139,7 @@ def make_params(dim, n, bc, tau, g_fluid, subsamples, device=0, stream=0, worksp
     p.workspace_dev = workspace_dev or None
     p.workspace_bytes = workspace_bytes
     p.streaming = streaming
-    p.reserved = 0
+    p.flags = flags
     return p
 
 
@@ -150,7 +151,7 @@ class Lattice:
     """Owner of one lbmimb_lattice handle.  Method names = C entry points without the prefix."""
 
     def __init__(self, dim, n, bc, tau, g_fluid, subsamples, max_particles=0, device=0, use_torch=True,
-                 streaming=STREAM_AB):
+                 streaming=STREAM_AB, flags=0):
         self.lib = load()
         self.dim = dim
         self.n = tuple(int(v) for v in n) + (1,) * (3 - len(n))
@@ -159,7 +160,7 @@ class Lattice:
         self._ws = None
         stream = 0
         ws_ptr, ws_bytes = 0, 0
-        probe = make_params(dim, n, bc, tau, g_fluid, subsamples, device, streaming=streaming)
+        probe = make_params(dim, n, bc, tau, g_fluid, subsamples, device, streaming=streaming, flags=flags)
         if use_torch:
             import torch
             if not torch.cuda.is_available():
@@ -172,7 +173,7 @@ class Lattice:
                 self._ws = torch.empty(need + 256, dtype=torch.uint8, device="cuda:%d" % device)
             ws_ptr = (self._ws.data_ptr() + 255) & ~255
             ws_bytes = need
-        self.params = make_params(dim, n, bc, tau, g_fluid, subsamples, device, stream, ws_ptr, ws_bytes, streaming)
+        self.params = make_params(dim, n, bc, tau, g_fluid, subsamples, device, stream, ws_ptr, ws_bytes, streaming, flags)
         h = C.c_void_p()
         _check(self.lib.lbmimb_create_lattice(C.byref(self.params), max_particles, C.byref(h)))
         self.h = h
@@ -318,10 +319,11 @@ class Lattice:
         return int(self.lib.lbmimb_launch_count(self.h))
 
 
-def from_workload(w, device=0, max_particles=None, map_mode=MAP_SAMPLING, streaming=STREAM_AB):
+def from_workload(w, device=0, max_particles=None, map_mode=MAP_SAMPLING, streaming=STREAM_AB, flags=0):
     """Lattice for a paper_1011_2613_b200.inputs.Workload with its particles set (not yet mapped)."""
     lat = Lattice(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples,
-                  max_particles=w.P if max_particles is None else max_particles, device=device, streaming=streaming)
+                  max_particles=w.P if max_particles is None else max_particles, device=device, streaming=streaming,
+                  flags=flags)
     if map_mode != MAP_SAMPLING:
         lat.set_mapping_mode(map_mode)
     if w.P:

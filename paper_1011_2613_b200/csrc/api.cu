@@ -1,6 +1,8 @@
 // C-ABI entry points of liblbmimb.so (include/lbmimb.h): argument checks, device
-// memory layout, state machine.  All arithmetic of the method runs in the kernels
-// of lattice.cu / particles.cu; nothing here computes on the host.
+// memory layout, state machine.  All per-node and per-particle arithmetic of the method runs
+// in the kernels of lattice.cu / particles.cu.  The host evaluates parameters only: 1/tau and
+// tau g (collide.cuh), the cell-list geometry, and the 256-entry table beta(n_s / S^D, tau) of
+// PAPER.md:41 (fill_beta_table below), which is uploaded once per lattice / mapping mode.
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -47,8 +49,9 @@ static bool valid_params(const lbmimb_params *p, int64_t maxp) {
   if (sd > 255) return fail(LBMIMB_EINVAL, "subsamples^dim must be <= 255"), false;
   if (p->streaming != LBMIMB_STREAM_AB && p->streaming != LBMIMB_STREAM_AA)
     return fail(LBMIMB_EINVAL, "streaming must be LBMIMB_STREAM_AB or LBMIMB_STREAM_AA"), false;
-  if (p->reserved != 0) return fail(LBMIMB_EINVAL, "reserved must be 0"), false;
-  if (maxp < 0 || maxp > 0x7fffffff) return fail(LBMIMB_EINVAL, "max_particles out of range"), false;
+  if ((p->flags & ~LBMIMB_FLAG_EXCHANGE_FIELD) != 0) return fail(LBMIMB_EINVAL, "unknown bit in flags"), false;
+  if (maxp < 0 || maxp > kMaxParticles)
+    return fail(LBMIMB_EINVAL, "max_particles out of range (node tags hold 24-bit particle indices)"), false;
   double nn = (double)p->n[0] * (double)p->n[1] * (double)p->n[2];
   if (nn > 4.0e12) return fail(LBMIMB_EINVAL, "lattice too large"), false;
   return true;
@@ -56,7 +59,7 @@ static bool valid_params(const lbmimb_params *p, int64_t maxp) {
 
 // One place that decides the device memory layout; used for sizing and for carving.
 struct Layout {
-  uint64_t off_f[2], off_eps, off_pid, off_s, off_beta, off_contested, off_counters, off_table, off_diag;
+  uint64_t off_f[2], off_tag, off_s, off_facc, off_beta, off_contested, off_counters, off_table, off_diag;
   uint64_t off_pos, off_vel, off_omega, off_radius, off_mass, off_force, off_torque, off_fc, off_prec;
   uint64_t off_count, off_start, off_fill, off_items, off_cell_of, off_bsums;
   uint64_t total;
@@ -80,9 +83,9 @@ static Layout make_layout(const lbmimb_params *p, int64_t maxp) {
   };
   L.off_f[0] = take((uint64_t)Q * L.N * 8);
   L.off_f[1] = p->streaming == LBMIMB_STREAM_AA ? L.off_f[0] : take((uint64_t)Q * L.N * 8);
-  L.off_eps = take((uint64_t)L.N);
-  L.off_pid = take((uint64_t)L.N * 4);
-  L.off_s = take((uint64_t)exchange_stride(p->dim) * L.N * 8);
+  L.off_tag = take((uint64_t)L.N * 4);
+  L.off_s = (p->flags & LBMIMB_FLAG_EXCHANGE_FIELD) ? take((uint64_t)exchange_stride(p->dim) * L.N * 8) : 0;
+  L.off_facc = take((uint64_t)pm * force_values(p->dim) * 16);
   L.off_beta = take(256 * 8);
   L.off_contested = take((uint64_t)L.contested_cap * 8);
   L.off_counters = take(64);
@@ -133,7 +136,7 @@ using namespace lbmimb;
 extern "C" {
 
 const char *lbmimb_last_error(void) { return g_err; }
-const char *lbmimb_version(void) { return "lbmimb 0.3 (sm_100a, fused collide-stream: pull A-B and in-place AA; DEM: cell list or Verlet lists)"; }
+const char *lbmimb_version(void) { return "lbmimb 0.4 (sm_100a, fused collide-stream + in-kernel force sums: pull A-B and in-place AA; DEM: cell list or Verlet lists)"; }
 
 uint64_t lbmimb_workspace_bytes(const lbmimb_params *params, int64_t max_particles) {
   if (!valid_params(params, max_particles)) return 0;
@@ -192,9 +195,10 @@ lbmimb_status lbmimb_create_lattice(const lbmimb_params *params, int64_t max_par
   h->ws_bytes = L.total;
   h->f[0] = (double *)(h->ws + L.off_f[0]);
   h->f[1] = (double *)(h->ws + L.off_f[1]);
-  h->eps_cnt = (uint8_t *)(h->ws + L.off_eps);
-  h->pid = (int32_t *)(h->ws + L.off_pid);
-  h->s = (double *)(h->ws + L.off_s);
+  h->tag = (uint32_t *)(h->ws + L.off_tag);
+  h->keep_s = (params->flags & LBMIMB_FLAG_EXCHANGE_FIELD) != 0;
+  h->s = h->keep_s ? (double *)(h->ws + L.off_s) : nullptr;
+  h->facc = (long long *)(h->ws + L.off_facc);
   h->beta_tab = (double *)(h->ws + L.off_beta);
   h->contested = (int64_t *)(h->ws + L.off_contested);
   h->contested_cap = L.contested_cap;
@@ -226,8 +230,8 @@ lbmimb_status lbmimb_create_lattice(const lbmimb_params *params, int64_t max_par
   fill_beta_table(params->tau, h->SD, tab);
   auto body = [&]() -> lbmimb_status {
     LBMIMB_CUDA(cudaMemcpyAsync(h->beta_tab, tab, sizeof(tab), cudaMemcpyHostToDevice, h->stream));
-    LBMIMB_CUDA(cudaMemsetAsync(h->eps_cnt, 0, (size_t)h->g.N, h->stream));
-    LBMIMB_CUDA(cudaMemsetAsync(h->pid, 0xFF, (size_t)h->g.N * 4, h->stream));
+    LBMIMB_CUDA(cudaMemsetAsync(h->tag, 0, (size_t)h->g.N * 4, h->stream));
+    LBMIMB_CUDA(cudaMemsetAsync(h->facc, 0, (size_t)(h->Pmax > 0 ? h->Pmax : 1) * force_values(h->g.dim) * 16, h->stream));
     LBMIMB_CUDA(cudaMemsetAsync(h->counters, 0, 64, h->stream));
     LBMIMB_CUDA(cudaMemsetAsync(h->force, 0, (size_t)3 * (h->Pmax > 0 ? h->Pmax : 1) * 8, h->stream));
     LBMIMB_CUDA(cudaMemsetAsync(h->torque, 0, (size_t)3 * (h->Pmax > 0 ? h->Pmax : 1) * 8, h->stream));
@@ -255,6 +259,7 @@ lbmimb_status lbmimb_create_lattice(const lbmimb_params *params, int64_t max_par
 }
 
 static void coupled_graph_drop(lbmimb_lattice *h);
+static lbmimb_status sync_and_check(lbmimb_lattice *h);
 
 lbmimb_status lbmimb_destroy_lattice(lbmimb_lattice *h) {
   if (!h) return LBMIMB_OK;
@@ -263,6 +268,7 @@ lbmimb_status lbmimb_destroy_lattice(lbmimb_lattice *h) {
   coupled_graph_drop(h);
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   neighbor_list_release(h);
+  if (h->fetch_stage) cudaFree(h->fetch_stage);
   if (h->owns_ws) cudaFree(h->ws);
   delete h;
   return LBMIMB_OK;
@@ -274,6 +280,10 @@ static lbmimb_status after_particles_changed(lbmimb_lattice *h, bool positions) 
     h->cl_valid = false;
     h->s_valid = false;
     h->forces_valid = false;
+    if (h->acc_dirty) {   // sums of a step nobody reduced: the particle set they belong to is gone
+      LBMIMB_CUDA(cudaMemsetAsync(h->facc, 0, (size_t)(h->Pmax > 0 ? h->Pmax : 1) * force_values(h->g.dim) * 16, h->stream));
+      h->acc_dirty = false;
+    }
     lbmimb_status st = neighbor_list_invalidate(h);
     if (st != LBMIMB_OK) return st;
   }
@@ -318,10 +328,7 @@ lbmimb_status lbmimb_set_particles(lbmimb_lattice *h, int64_t P, const double *p
   h->P = P;
   h->rmax = rmax;
   h->rmin = P > 0 ? rmin : 0.0;
-  if (P == 0) {
-    LBMIMB_CUDA(cudaMemsetAsync(h->eps_cnt, 0, (size_t)h->g.N, h->stream));
-    LBMIMB_CUDA(cudaMemsetAsync(h->pid, 0xFF, (size_t)h->g.N * 4, h->stream));
-  }
+  if (P == 0) LBMIMB_CUDA(cudaMemsetAsync(h->tag, 0, (size_t)h->g.N * 4, h->stream));
   st = after_particles_changed(h, true);
   if (st != LBMIMB_OK) return st;
   LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
@@ -338,6 +345,8 @@ lbmimb_status lbmimb_set_particles_dev(lbmimb_lattice *h, int64_t P, const doubl
   int D = h->g.dim, nt = D == 2 ? 1 : 3;
   double rmax = 0.0, rmin = INFINITY;
   if (P > 0) {
+    // checked on the device before anything is committed: on EINVAL the handle is unchanged
+    if ((st = validate_particles_dev(h, P, pos_dev, radius_dev, mass_dev, &rmax, &rmin)) != LBMIMB_OK) return st;
     auto d2d = [&](void *dst, const void *src, uint64_t bytes) -> lbmimb_status {
       LBMIMB_CUDA(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, h->stream));
       return LBMIMB_OK;
@@ -353,23 +362,11 @@ lbmimb_status lbmimb_set_particles_dev(lbmimb_lattice *h, int64_t P, const doubl
     if ((st = d2d(h->mass, mass_dev, (uint64_t)P * 8)) != LBMIMB_OK) return st;
     LBMIMB_CUDA(cudaMemsetAsync(h->force, 0, (size_t)D * P * 8, h->stream));
     LBMIMB_CUDA(cudaMemsetAsync(h->torque, 0, (size_t)nt * P * 8, h->stream));
-    // the cell-list geometry needs the largest radius on the host: one scalar read-back
-    std::vector<double> r((size_t)P);
-    LBMIMB_CUDA(cudaMemcpyAsync(r.data(), h->radius, (size_t)P * 8, cudaMemcpyDeviceToHost, h->stream));
-    LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
-    for (int64_t p = 0; p < P; ++p) {
-      if (!(r[p] > 0.0) || !std::isfinite(r[p])) return fail(LBMIMB_EINVAL, "particle %lld: bad radius", (long long)p);
-      if (r[p] > rmax) rmax = r[p];
-      if (r[p] < rmin) rmin = r[p];
-    }
   }
   h->P = P;
   h->rmax = rmax;
   h->rmin = P > 0 ? rmin : 0.0;
-  if (P == 0) {
-    LBMIMB_CUDA(cudaMemsetAsync(h->eps_cnt, 0, (size_t)h->g.N, h->stream));
-    LBMIMB_CUDA(cudaMemsetAsync(h->pid, 0xFF, (size_t)h->g.N * 4, h->stream));
-  }
+  if (P == 0) LBMIMB_CUDA(cudaMemsetAsync(h->tag, 0, (size_t)h->g.N * 4, h->stream));
   return after_particles_changed(h, true);
 }
 
@@ -398,30 +395,35 @@ lbmimb_status lbmimb_get_particles(lbmimb_lattice *h, double *pos, double *vel, 
     if (omega)
       LBMIMB_CUDA(cudaMemcpyAsync(omega, h->omega, (size_t)nt * h->P * 8, cudaMemcpyDeviceToHost, h->stream));
   }
-  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
-  return LBMIMB_OK;
+  return sync_and_check(h);
 }
 
 int64_t lbmimb_num_particles(const lbmimb_lattice *h) { return h ? h->P : -1; }
 int64_t lbmimb_time(const lbmimb_lattice *h) { return h ? h->t : -1; }
 int64_t lbmimb_launch_count(const lbmimb_lattice *h) { return h ? h->launches : -1; }
 
+// Waits for the handle's stream and reads the error flags kernels raise on the device: overflow of the
+// shared-node list of the map, of a neighbour list or of a cell of its build grid.  Every call that
+// synchronises anyway ends with this, so that a result is never handed out next to a silent overflow.
+static lbmimb_status sync_and_check(lbmimb_lattice *h) {
+  int32_t c[4] = {0, 0, 0, 0}, s[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  LBMIMB_CUDA(cudaMemcpyAsync(c, h->counters, sizeof(c), cudaMemcpyDeviceToHost, h->stream));
+  if (h->nl.mem) LBMIMB_CUDA(cudaMemcpyAsync(s, h->nl.state, sizeof(s), cudaMemcpyDeviceToHost, h->stream));
+  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+  if (c[1] != 0)
+    return fail(LBMIMB_ESTATE, "particle map: the list of nodes shared by several particles overflowed (%lld entries; "
+                               "particles overlap too much)", (long long)h->contested_cap);
+  if (s[4] != 0 || s[5] != 0)
+    return fail(LBMIMB_ESTATE, "neighbour list: %s overflowed (particles overlap more deeply than the sizing allows)",
+                s[4] ? "a particle's list" : "a cell of the build grid");
+  return LBMIMB_OK;
+}
+
 lbmimb_status lbmimb_synchronize(lbmimb_lattice *h) {
   if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
   lbmimb_status st = use_device(h);
   if (st != LBMIMB_OK) return st;
-  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
-  int32_t c[4];
-  LBMIMB_CUDA(cudaMemcpy(c, h->counters, sizeof(c), cudaMemcpyDeviceToHost));
-  if (c[1] != 0) return fail(LBMIMB_ESTATE, "particle map: contested-node list overflowed (particles overlap too much)");
-  if (h->nl.mem) {
-    int32_t s[8];
-    LBMIMB_CUDA(cudaMemcpy(s, h->nl.state, sizeof(s), cudaMemcpyDeviceToHost));
-    if (s[4] != 0 || s[5] != 0)
-      return fail(LBMIMB_ESTATE, "neighbour list: %s overflowed (particles overlap more deeply than the sizing allows)",
-                  s[4] ? "a particle's list" : "a cell of the build grid");
-  }
-  return LBMIMB_OK;
+  return sync_and_check(h);
 }
 
 // Bodies of the four calls of a coupled step: launches and state machine only (no argument checks, no
@@ -481,7 +483,12 @@ static lbmimb_status step_body(lbmimb_lattice *h, int32_t nsteps) {
   lbmimb_status st;
   for (int32_t it = 0; it < nsteps; ++it) {
     bool emit = (h->P > 0) && (it == nsteps - 1);
+    if (emit && h->acc_dirty) {   // sums of an earlier step that no reduce_particle_forces consumed
+      LBMIMB_CUDA(cudaMemsetAsync(h->facc, 0, (size_t)h->P * force_values(h->g.dim) * 16, h->stream));
+      h->acc_dirty = false;
+    }
     if ((st = launch_collide_stream(h, emit)) != LBMIMB_OK) return st;
+    if (emit) h->acc_dirty = true;
     if (h->aa)
       h->aa_swapped = !h->aa_swapped;
     else
@@ -505,9 +512,10 @@ lbmimb_status lbmimb_step(lbmimb_lattice *h, int32_t nsteps) {
 static lbmimb_status reduce_body(lbmimb_lattice *h) {
   if (h->P > 0 && !h->s_valid)
     return fail(LBMIMB_ESTATE, "no exchange vectors: call lbmimb_step after lbmimb_map_particles first");
-  if (h->P > 0) {
-    lbmimb_status st = launch_reduce(h);
+  if (h->P > 0 && !h->forces_valid) {   // (a repeated call finds force / torque already in place)
+    lbmimb_status st = launch_finish_forces(h);
     if (st != LBMIMB_OK) return st;
+    h->acc_dirty = false;
   }
   h->forces_valid = true;
   return LBMIMB_OK;
@@ -528,7 +536,7 @@ lbmimb_status lbmimb_reduce_particle_forces(lbmimb_lattice *h, double *force, do
     if (force) LBMIMB_CUDA(cudaMemcpyAsync(force, h->force, (size_t)D * h->P * 8, cudaMemcpyDeviceToHost, h->stream));
     if (torque)
       LBMIMB_CUDA(cudaMemcpyAsync(torque, h->torque, (size_t)nt * h->P * 8, cudaMemcpyDeviceToHost, h->stream));
-    LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+    return sync_and_check(h);
   }
   return LBMIMB_OK;
 }
@@ -606,6 +614,12 @@ static lbmimb_status coupled_graph_capture(lbmimb_lattice *h, const lbmimb_dem_p
   if (!h->cap_stream) LBMIMB_CUDA(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
   const cudaStream_t user = h->stream;
   const int64_t t0 = h->t, l0 = h->launches;
+  // the host-side state machine as it stands: a capture that fails half way has executed nothing on the
+  // device, so everything the captured calls toggled is put back
+  const int cur0 = h->cur;
+  const bool swapped0 = h->aa_swapped, map0 = h->map_valid, s0 = h->s_valid, forces0 = h->forces_valid;
+  const bool cl0 = h->cl_valid, dirty0 = h->acc_dirty;
+  const double table0 = h->table_R;
   LBMIMB_CUDA(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
   h->stream = h->cap_stream;
   lbmimb_status st = coupled_step_body(h, dem);
@@ -619,6 +633,14 @@ static lbmimb_status coupled_graph_capture(lbmimb_lattice *h, const lbmimb_dem_p
   if (st != LBMIMB_OK || e != cudaSuccess || !graph) {
     if (graph) cudaGraphDestroy(graph);
     cudaGetLastError();
+    h->cur = cur0;
+    h->aa_swapped = swapped0;
+    h->map_valid = map0;
+    h->s_valid = s0;
+    h->forces_valid = forces0;
+    h->cl_valid = cl0;
+    h->acc_dirty = dirty0;
+    h->table_R = table0;
     return st != LBMIMB_OK ? st : cuda_fail(e, "cudaStreamEndCapture(coupled steps)");
   }
   const cudaError_t e2 = cudaGraphInstantiate(&g.exec, graph, 0);
@@ -763,28 +785,30 @@ lbmimb_status lbmimb_fetch_fields(lbmimb_lattice *h, int32_t what, const int64_t
   }
   if ((what == LBMIMB_FIELD_EPS_CNT || what == LBMIMB_FIELD_PID) && !h->map_valid)
     return fail(LBMIMB_ESTATE, "particle map is stale");
+  if (what == LBMIMB_FIELD_S && !h->keep_s)
+    return fail(LBMIMB_ESTATE, "per-node exchange vectors are kept only by a lattice created with LBMIMB_FLAG_EXCHANGE_FIELD");
   if (what == LBMIMB_FIELD_S && h->P > 0 && !h->s_valid) return fail(LBMIMB_ESTATE, "no exchange vectors yet");
   lbmimb_status st = use_device(h);
   if (st != LBMIMB_OK) return st;
   // A-B: the idle distribution buffer is the staging area (every field of a sub-box fits in Q*N
-  // doubles).  AA has no idle buffer: a temporary one of the box's size.
+  // doubles).  AA has no idle buffer: a grow-only staging buffer owned by the handle.
   void *stage = h->f[h->cur ^ 1];
-  void *tmp = nullptr;
+  const size_t bytes = (size_t)comps * box * esz;
   if (h->aa) {
-    cudaError_t e = cudaMalloc(&tmp, (size_t)comps * box * esz);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc(fetch staging, AA mode)");
-    stage = tmp;
+    if (bytes > h->fetch_stage_bytes) {
+      LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+      if (h->fetch_stage) cudaFree(h->fetch_stage);
+      h->fetch_stage = nullptr;
+      h->fetch_stage_bytes = 0;
+      cudaError_t e = cudaMalloc(&h->fetch_stage, bytes);
+      if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc(fetch staging, AA mode)");
+      h->fetch_stage_bytes = bytes;
+    }
+    stage = h->fetch_stage;
   }
-  auto body = [&]() -> lbmimb_status {
-    lbmimb_status s2 = launch_fetch(h, what, lo, hi, stage);
-    if (s2 != LBMIMB_OK) return s2;
-    LBMIMB_CUDA(cudaMemcpyAsync(dst, stage, (size_t)comps * box * esz, cudaMemcpyDeviceToHost, h->stream));
-    LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
-    return LBMIMB_OK;
-  };
-  st = body();
-  if (tmp) cudaFree(tmp);
-  return st;
+  if ((st = launch_fetch(h, what, lo, hi, stage)) != LBMIMB_OK) return st;
+  LBMIMB_CUDA(cudaMemcpyAsync(dst, stage, bytes, cudaMemcpyDeviceToHost, h->stream));
+  return sync_and_check(h);
 }
 
 lbmimb_status lbmimb_diagnostics(lbmimb_lattice *h, double *out) {
@@ -796,8 +820,7 @@ lbmimb_status lbmimb_diagnostics(lbmimb_lattice *h, double *out) {
   const double den = h->map_mode == LBMIMB_MAP_TABLE ? (double)LBMIMB_TABLE_DEN : (double)h->SD;
   if ((st = launch_diagnostics(h, den)) != LBMIMB_OK) return st;
   LBMIMB_CUDA(cudaMemcpyAsync(out, h->diag_out, LBMIMB_DIAG_LEN * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
-  return LBMIMB_OK;
+  return sync_and_check(h);
 }
 
 lbmimb_status lbmimb_set_distributions(lbmimb_lattice *h, const double *f) {

@@ -1,5 +1,5 @@
-// Node-local collision of eq. (1) shared by the step kernels of lattice.cu and
-// lattice_tma.cu.  In place on the gathered populations f[Q].
+// Node-local collision of eq. (1) shared by the step kernels of lattice.cu (pull A-B and
+// in-place AA), and the in-kernel force / torque sums of eq. (3).  In place on the gathered populations f[Q].
 //
 // Algebra (same real-number result as the paper's form, regrouped to cut fp64 work):
 //   om = 1/tau, a = (1-beta) om.  With feq_q(u) = E_u + O_u, feq_-q(u) = E_u - O_u (even / odd part
@@ -136,10 +136,12 @@ __device__ __forceinline__ void store_exchange(double *__restrict__ s, int64_t x
   }
 }
 
-// V_S = v_p + omega_p x (x_node - x_p), minimum image on periodic axes (R5)
+// V_S = v_p + omega_p x (x_node - x_p), minimum image on periodic axes (R5); also returns the lever
+// arm r = x_node - x_p of eq. (3)
 template <int D>
 __device__ __forceinline__ void solid_velocity(const double *__restrict__ pr, int i, int j, int k, int nx, int ny,
-                                               int nz, int bcx, int bcy, int bcz, double &vx, double &vy, double &vz) {
+                                               int nz, int bcx, int bcy, int bcz, double &vx, double &vy, double &vz,
+                                               double &rx, double &ry, double &rz) {
   auto mi = [](double d, int n) {
     const double hn = 0.5 * (double)n;
     if (d > hn) return d - (double)n;
@@ -147,7 +149,9 @@ __device__ __forceinline__ void solid_velocity(const double *__restrict__ pr, in
     return d;
   };
   if (D == 2) {
-    double rx = (double)i - __ldg(pr + 0), ry = (double)j - __ldg(pr + 1);
+    rx = (double)i - __ldg(pr + 0);
+    ry = (double)j - __ldg(pr + 1);
+    rz = 0.0;
     if (!bcx) rx = mi(rx, nx);
     if (!bcy) ry = mi(ry, ny);
     const double w = __ldg(pr + 4);
@@ -155,7 +159,9 @@ __device__ __forceinline__ void solid_velocity(const double *__restrict__ pr, in
     vy = __ldg(pr + 3) + w * rx;
     vz = 0.0;
   } else {
-    double rx = (double)i - __ldg(pr + 0), ry = (double)j - __ldg(pr + 1), rz = (double)k - __ldg(pr + 2);
+    rx = (double)i - __ldg(pr + 0);
+    ry = (double)j - __ldg(pr + 1);
+    rz = (double)k - __ldg(pr + 2);
     if (!bcx) rx = mi(rx, nx);
     if (!bcy) ry = mi(ry, ny);
     if (!bcz) rz = mi(rz, nz);
@@ -163,6 +169,56 @@ __device__ __forceinline__ void solid_velocity(const double *__restrict__ pr, in
     vx = __ldg(pr + 3) + (wy * rz - wz * ry);
     vy = __ldg(pr + 4) + (wz * rx - wx * rz);
     vz = __ldg(pr + 5) + (wx * ry - wy * rx);
+  }
+}
+
+// ---------------------------------------------------------------------------
+// a3 inside a2: F_p = -sum s_n, T_p = -sum r_n x s_n (eq. (3), sign of R6) summed while
+// the step runs.  The lanes of a warp are consecutive nodes of one lattice row, so the nodes of a particle
+// form runs of equal `key` (covering particle, -1 = not covered / not a node).  Each run is summed by a
+// segmented shuffle tree (fixed shape => the fp64 partial sum of a run is reproducible), and the head lane of
+// the run adds the partial sum to the particle's accumulators as 64-bit FIXED-POINT integers: integer
+// addition is associative, so the total does not depend on the order in which warps arrive, and the
+// reduction is bitwise reproducible without a second pass over the lattice.
+//   value = hi 2^-40 + lo 2^-92: hi = rint(v 2^40), lo = rint((v - hi 2^-40) 2^92); the remainder is exact
+//   and |lo| <= 2^51, so runs add without overflow and a sum resolves 2^-92 ~ 2e-28 (|v| < 2^22).
+// ---------------------------------------------------------------------------
+__device__ __forceinline__ void fixed_add(long long *acc, double v) {
+  constexpr double k40 = 1099511627776.0, k52 = 4503599627370496.0;
+  const long long hi = __double2ll_rn(v * k40);
+  const double rem = v - (double)hi * (1.0 / k40);
+  const long long lo = __double2ll_rn((rem * k40) * k52);
+  atomicAdd(reinterpret_cast<unsigned long long *>(acc), (unsigned long long)hi);
+  if (lo != 0) atomicAdd(reinterpret_cast<unsigned long long *>(acc) + 1, (unsigned long long)lo);
+}
+
+__host__ __device__ __forceinline__ double fixed_value(long long hi, long long lo) {
+  return (double)hi * (1.0 / 1099511627776.0) + ((double)lo * (1.0 / 4503599627370496.0)) * (1.0 / 1099511627776.0);
+}
+
+// Whole warp must call.  key < 0: this lane contributes nothing.  v[NV]: this node's -s and -(r x s).
+template <int NV>
+__device__ __forceinline__ void accumulate_runs(int key, double (&v)[NV], long long *__restrict__ facc) {
+  const unsigned lane = threadIdx.x & 31u;
+  const int prev = __shfl_up_sync(0xffffffffu, key, 1);
+  const bool boundary = key < 0 || lane == 0 || prev != key;       // first lane of a run (or an idle lane)
+  const unsigned bmask = __ballot_sync(0xffffffffu, boundary);
+  if (__all_sync(0xffffffffu, key < 0)) return;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    // lanes lane+1 .. lane+d all continue this lane's run?
+    const unsigned between = ((1u << d) - 1u) << 1;
+    const bool take = lane + d < 32u && ((bmask >> lane) & between) == 0u;
+#pragma unroll
+    for (int c = 0; c < NV; ++c) {
+      const double o = __shfl_down_sync(0xffffffffu, v[c], d);
+      if (take) v[c] += o;
+    }
+  }
+  if (boundary && key >= 0) {
+    long long *acc = facc + (int64_t)key * (2 * NV);
+#pragma unroll
+    for (int c = 0; c < NV; ++c) fixed_add(acc + 2 * c, v[c]);
   }
 }
 

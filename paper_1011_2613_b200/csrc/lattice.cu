@@ -15,11 +15,11 @@ namespace lbmimb {
 struct StepArgs {
   const double *__restrict__ fin;
   double *__restrict__ fout;
-  const uint8_t *__restrict__ eps_cnt;
-  const int32_t *__restrict__ pid;
+  const uint32_t *__restrict__ tag;
   const double *__restrict__ prec;
   const double *__restrict__ beta_tab;
-  double *__restrict__ s;
+  double *__restrict__ s;            // per-node exchange records (EMIT == kEmitField only)
+  long long *__restrict__ facc;      // per-particle fixed-point force / torque sums (EMIT != kEmitNone)
   int64_t N;
   int nx, ny, nz;
   int bcx, bcy, bcz;
@@ -32,15 +32,35 @@ struct StepArgs {
 
 constexpr int kStepThreads = 128;
 enum { kLayoutPull = 0, kLayoutNatural = 1, kLayoutSwapped = 2 };
+// what a step leaves behind for a3: nothing (not the last step of a call), the per-particle force / torque
+// sums, or those plus the per-node exchange vectors (LBMIMB_FLAG_EXCHANGE_FIELD)
+enum { kEmitNone = 0, kEmitForces = 1, kEmitField = 2 };
+
+// Tail of both step kernels on warps that hold a covered node: eq. (3) summed in the kernel.
+template <int D, int EMIT>
+__device__ __forceinline__ void emit_exchange(const StepArgs &a, int64_t x, bool covered, int pe, double beta, double rho,
+                                              double ux, double uy, double uz, double vx, double vy, double vz,
+                                              double rx, double ry, double rz) {
+  const double br = beta * rho;
+  const double sx = br * (vx - ux), sy = br * (vy - uy), sz = br * (vz - uz);   // s = beta rho (V_S - u)  (P6)
+  if (EMIT == kEmitField && covered) store_exchange<D>(a.s, x, sx, sy, sz);
+  if (D == 2) {
+    double v[3] = {-sx, -sy, -(rx * sy - ry * sx)};
+    accumulate_runs<3>(covered ? pe : -1, v, a.facc);
+  } else {
+    double v[6] = {-sx, -sy, -sz, -(ry * sz - rz * sy), -(rz * sx - rx * sz), -(rx * sy - ry * sx)};
+    accumulate_runs<6>(covered ? pe : -1, v, a.facc);
+  }
+}
 
 // ---------------------------------------------------------------------------
 // a2: fused collide-and-stream, one thread per node, one block per row segment.
-// IMB = particles present, EMIT = also store the exchange vector s.
+// IMB = particles present, EMIT = what is left for a3 (kEmit*).
 // The y/z part of every source address is block-uniform; per thread only the three
 // x indices i-1, i, i+1 (wrapped) differ.  A warp takes the IMB path as a whole when
 // any of its nodes is covered (beta = 0 on the others), else the cheaper LBGK path.
 // ---------------------------------------------------------------------------
-template <int D, bool IMB, bool EMIT, int MINB>
+template <int D, bool IMB, int EMIT, int MINB>
 __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(const StepArgs a) {
   using L = Lat<D>;
   constexpr int Q = L::Q;
@@ -61,8 +81,9 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
   // on covered nodes instead of three: C4 7.00 -> 6.46 ms).
   int cnt = 0, pe = 0;
   if (IMB) {
-    cnt = a.eps_cnt[x];
-    pe = a.pid[x];
+    const uint32_t tg = a.tag[x];
+    cnt = tag_cnt(tg);
+    pe = (int)(tg >> kTagPidShift);
   }
 
   // ---- gather (streaming) ----
@@ -94,30 +115,26 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
     }
   }
 
-  double beta = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
+  double beta = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, rx = 0.0, ry = 0.0, rz = 0.0;
   if (IMB && cnt > 0) {
     beta = __ldg(a.beta_tab + cnt);
     solid_velocity<D>(a.prec + (int64_t)pe * prec_stride(D), i, j, k, a.nx, a.ny, a.nz, a.bcx, a.bcy, a.bcz, vx, vy,
-                      vz);
+                      vz, rx, ry, rz);
   }
 
   double rho, ux, uy, uz;
   moments<D>(f, rho, ux, uy, uz);
 
-  if (!IMB || !__any_sync(0xffffffffu, cnt > 0)) {
-    collide_fluid<D>(f, a.cp, rho, ux, uy, uz);
-  } else {
-    collide_imb<D>(f, a.cp, rho, ux, uy, uz, beta, vx, vy, vz);
-    if (EMIT && cnt > 0 && live) {
-      const double br = beta * rho;
-      store_exchange<D>(a.s, x, br * (vx - ux), br * (vy - uy), br * (vz - uz));
-    }
-  }
+  const bool solid_warp = IMB && __any_sync(0xffffffffu, cnt > 0);
+  if (!solid_warp) collide_fluid<D>(f, a.cp, rho, ux, uy, uz);
+  else collide_imb<D>(f, a.cp, rho, ux, uy, uz, beta, vx, vy, vz);
 
   if (live) {
 #pragma unroll
     for (int q = 0; q < Q; ++q) a.fout[(int64_t)q * a.N + x] = f[q];
   }
+  if (EMIT != kEmitNone && solid_warp)
+    emit_exchange<D, EMIT>(a, x, cnt > 0 && live, pe, beta, rho, ux, uy, uz, vx, vy, vz, rx, ry, rz);
 }
 
 // ---------------------------------------------------------------------------
@@ -136,7 +153,7 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
 // address per direction: a block-uniform 64-bit offset (slot and row, looked up in a table of the 9
 // neighbouring rows (dy,dz) with their wall flags) plus one of the three wrapped x indices.
 // XW = walls in x, where the end nodes of a row bounce per thread.
-template <int D, bool IMB, bool EMIT, bool ODD, bool XW, int MINB>
+template <int D, bool IMB, int EMIT, bool ODD, bool XW, int MINB>
 __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_aa_kernel(const StepArgs a) {
   using L = Lat<D>;
   constexpr int Q = L::Q;
@@ -153,8 +170,9 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_aa_kernel(c
 
   int cnt = 0, pe = 0;
   if (IMB) {
-    cnt = a.eps_cnt[x];
-    pe = a.pid[x];
+    const uint32_t tg = a.tag[x];
+    cnt = tag_cnt(tg);
+    pe = (int)(tg >> kTagPidShift);
   }
 
   const int im = i == 0 ? a.nx - 1 : i - 1;
@@ -198,37 +216,34 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_aa_kernel(c
     for (int q = 0; q < Q; ++q) f[q] = *slow_ptr(q);
   }
 
-  double beta = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
+  double beta = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, rx = 0.0, ry = 0.0, rz = 0.0;
   if (IMB && cnt > 0) {
     beta = __ldg(a.beta_tab + cnt);
     solid_velocity<D>(a.prec + (int64_t)pe * prec_stride(D), i, j, k, a.nx, a.ny, a.nz, a.bcx, a.bcy, a.bcz, vx, vy,
-                      vz);
+                      vz, rx, ry, rz);
   }
 
   double rho, ux, uy, uz;
   moments<D>(f, rho, ux, uy, uz);
 
-  if (!IMB || !__any_sync(0xffffffffu, cnt > 0)) {
-    collide_fluid<D>(f, a.cp, rho, ux, uy, uz);
-  } else {
-    collide_imb<D>(f, a.cp, rho, ux, uy, uz, beta, vx, vy, vz);
-    if (EMIT && cnt > 0 && live) {
-      const double br = beta * rho;
-      store_exchange<D>(a.s, x, br * (vx - ux), br * (vy - uy), br * (vz - uz));
+  const bool solid_warp = IMB && __any_sync(0xffffffffu, cnt > 0);
+  if (!solid_warp) collide_fluid<D>(f, a.cp, rho, ux, uy, uz);
+  else collide_imb<D>(f, a.cp, rho, ux, uy, uz, beta, vx, vy, vz);
+
+  if (live) {
+    if (!ODD) {
+#pragma unroll
+      for (int q = 0; q < Q; ++q) F[(int64_t)opposite(q) * a.N + x] = f[q];
+    } else if (inner) {
+#pragma unroll
+      for (int q = 0; q < Q; ++q) *fast_ptr(opposite(q)) = f[q];
+    } else {
+#pragma unroll
+      for (int q = 0; q < Q; ++q) *slow_ptr(opposite(q)) = f[q];
     }
   }
-
-  if (!live) return;
-  if (!ODD) {
-#pragma unroll
-    for (int q = 0; q < Q; ++q) F[(int64_t)opposite(q) * a.N + x] = f[q];
-  } else if (inner) {
-#pragma unroll
-    for (int q = 0; q < Q; ++q) *fast_ptr(opposite(q)) = f[q];
-  } else {
-#pragma unroll
-    for (int q = 0; q < Q; ++q) *slow_ptr(opposite(q)) = f[q];
-  }
+  if (EMIT != kEmitNone && solid_warp)
+    emit_exchange<D, EMIT>(a, x, cnt > 0 && live, pe, beta, rho, ux, uy, uz, vx, vy, vz, rx, ry, rz);
 }
 
 // ---------------------------------------------------------------------------
@@ -320,8 +335,7 @@ __global__ void unstream_kernel(const double *__restrict__ fpre, double *__restr
 
 struct FetchArgs {
   const double *fpost;
-  const uint8_t *eps_cnt;
-  const int32_t *pid;
+  const uint32_t *tag;
   const double *s;
   void *dst;
   int lo[3], ext[3];
@@ -343,11 +357,11 @@ __global__ void fetch_kernel(const FetchArgs a, const Geom g) {
     const int i = a.lo[0] + bi, j = a.lo[1] + bj, k = a.lo[2] + bk;
     const int64_t x = ((int64_t)k * g.ny + j) * g.nx + i;
     if (a.what == LBMIMB_FIELD_EPS_CNT) {
-      ((uint8_t *)a.dst)[b] = a.eps_cnt[x];
+      ((uint8_t *)a.dst)[b] = (uint8_t)tag_cnt(a.tag[x]);
     } else if (a.what == LBMIMB_FIELD_PID) {
-      ((int32_t *)a.dst)[b] = a.pid[x];
+      ((int32_t *)a.dst)[b] = tag_pid(a.tag[x]);
     } else if (a.what == LBMIMB_FIELD_S) {
-      const bool cov = a.have_particles && a.eps_cnt[x] > 0;
+      const bool cov = a.have_particles && tag_cnt(a.tag[x]) > 0;
       for (int c = 0; c < D; ++c) ((double *)a.dst)[(int64_t)c * a.box + b] = cov ? a.s[x * exchange_stride(D) + c] : 0.0;
     } else {
       double f[L::Q];
@@ -398,7 +412,7 @@ __device__ __forceinline__ double diag_block_sum(double v, double *sh) {
 }
 
 template <int D>
-__global__ void __launch_bounds__(kDiagThreads) diag_nodes_kernel(const double *__restrict__ fst, const uint8_t *__restrict__ eps_cnt,
+__global__ void __launch_bounds__(kDiagThreads) diag_nodes_kernel(const double *__restrict__ fst, const uint32_t *__restrict__ tag,
                                                                   const Geom g, int layout, int have_particles,
                                                                   double eps_den, double *__restrict__ partial) {
   using L = Lat<D>;
@@ -422,7 +436,7 @@ __global__ void __launch_bounds__(kDiagThreads) diag_nodes_kernel(const double *
       m[1] += L::cy(q) * f[q];
       m[2] += L::cz(q) * f[q];
     }
-    const double gas = have_particles ? 1.0 - (double)eps_cnt[x] / eps_den : 1.0;
+    const double gas = have_particles ? 1.0 - (double)tag_cnt(tag[x]) / eps_den : 1.0;
     acc[0] += gas;
     acc[1] += rho;
 #pragma unroll
@@ -511,18 +525,20 @@ lbmimb_status launch_init_rest(lbmimb_lattice *h) {
 // One instantiation per (D, IMB, EMIT).  Occupancy targets from the round-1 sweep:
 // 3D 80 registers / 6 blocks per SM, 2D 56 registers / 9 blocks per SM.
 template <int D>
-static void launch_cs(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, bool imb, bool emit) {
+static void launch_cs(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, bool imb, int emit) {
   constexpr int MINB = D == 3 ? 6 : 9;
   if (!imb)
-    collide_stream_kernel<D, false, false, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
-  else if (!emit)
-    collide_stream_kernel<D, true, false, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
+    collide_stream_kernel<D, false, kEmitNone, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
+  else if (emit == kEmitNone)
+    collide_stream_kernel<D, true, kEmitNone, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
+  else if (emit == kEmitForces)
+    collide_stream_kernel<D, true, kEmitForces, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
   else
-    collide_stream_kernel<D, true, true, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
+    collide_stream_kernel<D, true, kEmitField, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a);
 }
 
 template <int D, int MINB>
-static void launch_aa(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, bool imb, bool emit, bool odd) {
+static void launch_aa(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, bool imb, int emit, bool odd) {
 #define LBMIMB_AA(I, E, O, X) collide_stream_aa_kernel<D, I, E, O, X, MINB><<<blocks, kStepThreads, 0, h->stream>>>(a)
 #define LBMIMB_AA_ODD(I, E)                       \
   do {                                            \
@@ -530,27 +546,30 @@ static void launch_aa(lbmimb_lattice *h, const StepArgs &a, unsigned blocks, boo
     else LBMIMB_AA(I, E, true, false);            \
   } while (0)
   if (!odd) {   // the even step touches the own node only: walls do not matter
-    if (!imb) LBMIMB_AA(false, false, false, false);
-    else if (!emit) LBMIMB_AA(true, false, false, false);
-    else LBMIMB_AA(true, true, false, false);
+    if (!imb) LBMIMB_AA(false, kEmitNone, false, false);
+    else if (emit == kEmitNone) LBMIMB_AA(true, kEmitNone, false, false);
+    else if (emit == kEmitForces) LBMIMB_AA(true, kEmitForces, false, false);
+    else LBMIMB_AA(true, kEmitField, false, false);
   } else {
-    if (!imb) LBMIMB_AA_ODD(false, false);
-    else if (!emit) LBMIMB_AA_ODD(true, false);
-    else LBMIMB_AA_ODD(true, true);
+    if (!imb) LBMIMB_AA_ODD(false, kEmitNone);
+    else if (emit == kEmitNone) LBMIMB_AA_ODD(true, kEmitNone);
+    else if (emit == kEmitForces) LBMIMB_AA_ODD(true, kEmitForces);
+    else LBMIMB_AA_ODD(true, kEmitField);
   }
 #undef LBMIMB_AA_ODD
 #undef LBMIMB_AA
 }
 
-lbmimb_status launch_collide_stream(lbmimb_lattice *h, bool emit) {
+lbmimb_status launch_collide_stream(lbmimb_lattice *h, bool emit_last) {
+  const int emit = !emit_last ? kEmitNone : (h->keep_s ? kEmitField : kEmitForces);
   StepArgs a;
   a.fin = h->f[h->cur];
   a.fout = h->f[h->cur ^ 1];
-  a.eps_cnt = h->eps_cnt;
-  a.pid = h->pid;
+  a.tag = h->tag;
   a.prec = h->prec;
   a.beta_tab = h->beta_tab;
   a.s = h->s;
+  a.facc = h->facc;
   a.N = h->g.N;
   a.nx = h->g.nx;
   a.ny = h->g.ny;
@@ -595,8 +614,7 @@ lbmimb_status launch_unstream(lbmimb_lattice *h, const double *f_pre, double *f_
 lbmimb_status launch_fetch(lbmimb_lattice *h, int what, const int64_t lo[3], const int64_t hi[3], void *dst_dev) {
   FetchArgs a;
   a.fpost = h->f[h->cur];
-  a.eps_cnt = h->eps_cnt;
-  a.pid = h->pid;
+  a.tag = h->tag;
   a.s = h->s;
   a.dst = dst_dev;
   a.box = 1;
@@ -622,12 +640,12 @@ lbmimb_status launch_diagnostics(lbmimb_lattice *h, double eps_den) {
   const double *fst = h->f[h->cur];
   const int hp = h->P > 0;
   if (h->g.dim == 2) {
-    diag_nodes_kernel<2><<<nb, kDiagThreads, 0, h->stream>>>(fst, h->eps_cnt, h->g, layout, hp, eps_den, h->diag_partial);
+    diag_nodes_kernel<2><<<nb, kDiagThreads, 0, h->stream>>>(fst, h->tag, h->g, layout, hp, eps_den, h->diag_partial);
     LBMIMB_LAUNCH_CHECK(h, "diag_nodes_kernel");
     diag_final_kernel<2><<<1, kDiagThreads, 0, h->stream>>>(h->diag_partial, nb, h->P, h->vel, h->radius, h->mass,
                                                            h->force, h->diag_out);
   } else {
-    diag_nodes_kernel<3><<<nb, kDiagThreads, 0, h->stream>>>(fst, h->eps_cnt, h->g, layout, hp, eps_den, h->diag_partial);
+    diag_nodes_kernel<3><<<nb, kDiagThreads, 0, h->stream>>>(fst, h->tag, h->g, layout, hp, eps_den, h->diag_partial);
     LBMIMB_LAUNCH_CHECK(h, "diag_nodes_kernel");
     diag_final_kernel<3><<<1, kDiagThreads, 0, h->stream>>>(h->diag_partial, nb, h->P, h->vel, h->radius, h->mass,
                                                            h->force, h->diag_out);

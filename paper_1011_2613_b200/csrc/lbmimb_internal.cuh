@@ -59,8 +59,25 @@ __host__ __device__ constexpr int opposite(int q) { return q == 0 ? 0 : ((q & 1)
 //   3D: x y z vx vy vz wx wy wz R   (10 doubles)      2D: x y vx vy w R (6 doubles)
 __host__ __device__ constexpr int prec_stride(int dim) { return dim == 3 ? 10 : 6; }
 
-// Exchange vectors s are stored as one record per node: [N][2] in 2D, [N][4] in 3D (4th slot unused).
+// Exchange vectors s (kept per node only with LBMIMB_FLAG_EXCHANGE_FIELD) are stored as one record per
+// node: [N][2] in 2D, [N][4] in 3D (4th slot unused).
 __host__ __device__ constexpr int exchange_stride(int dim) { return dim == 3 ? 4 : 2; }
+
+// Node tag: one 32-bit word per node = (covering particle << 8) | inside-sample count (or table code).
+// 0 = uncovered (the particle bits are meaningless when the count is 0), so one memset clears the map and
+// the fused kernel reads one word per node.  Particle indices are 24 bits: max_particles <= 2^24.
+constexpr int kTagPidShift = 8;
+constexpr int64_t kMaxParticles = (int64_t)1 << 24;
+__host__ __device__ constexpr uint32_t make_tag(int32_t p, int cnt) {
+  return cnt > 0 ? ((uint32_t)p << kTagPidShift) | (uint32_t)cnt : 0u;
+}
+__host__ __device__ constexpr int tag_cnt(uint32_t t) { return (int)(t & 0xffu); }
+__host__ __device__ constexpr int32_t tag_pid(uint32_t t) { return (t & 0xffu) ? (int32_t)(t >> kTagPidShift) : -1; }
+
+// Per-particle force / torque accumulators of the fused step: NV = 3 (2D: Fx Fy Tz) or 6 (3D: F, T) values,
+// each a pair of 64-bit fixed-point words (value = hi 2^-40 + lo 2^-92), added with integer atomics: the
+// sum does not depend on the order in which warps arrive (collide.cuh: accumulate_runs).
+__host__ __device__ constexpr int force_values(int dim) { return dim == 3 ? 6 : 3; }
 
 struct Geom {
   int dim;
@@ -135,13 +152,17 @@ struct lbmimb_lattice {
   double *f[2];
   int cur;
   bool aa, aa_swapped;
-  uint8_t *eps_cnt;   // [N]
-  int32_t *pid;       // [N]
-  double *s;          // [N][exchange_stride] exchange vectors of the last step
+  uint32_t *tag;      // [N] node tags (make_tag)
+  double *s;          // [N][exchange_stride] exchange vectors of the last step; NULL unless keep_s
+  bool keep_s;        // LBMIMB_FLAG_EXCHANGE_FIELD
+  long long *facc;    // [Pmax][force_values][2] fixed-point force / torque sums of the last emitting step
+  bool acc_dirty;     // facc holds sums that have not been folded into force / torque (or discarded) yet
   double *beta_tab;   // [256] beta(n_s / S^D, tau)
   int64_t *contested; // mapping fix-up list
   int64_t contested_cap;
-  int32_t *counters;  // [0] contested count, [1] overflow flag, [2] bad-particle flag
+  int32_t *counters;  // [16]: [0] shared-node count, [1] its overflow flag, [8..13] result of validate_particles_dev
+  void *fetch_stage;     // AA mode: grow-only staging buffer of fetch_fields (library-allocated)
+  size_t fetch_stage_bytes;
   double *diag_partial;  // [kDiagBlocksMax][8] stage-1 sums of lbmimb_diagnostics
   double *diag_out;      // [20]
 
@@ -160,7 +181,7 @@ struct lbmimb_lattice {
   bool cg_broken;               // a capture failed once: keep to plain launches
 
   bool map_valid;     // eps_cnt/pid match the particle positions
-  bool s_valid;       // s holds the exchange vectors of the last step under the current map
+  bool s_valid;       // the last step ran under the current map and left its force sums (and s, if kept)
   bool forces_valid;  // force/torque hold the reduction of s
   int64_t t;
   int64_t launches;
@@ -190,11 +211,13 @@ lbmimb_status launch_collide_stream(lbmimb_lattice *h, bool emit);
 lbmimb_status launch_unstream(lbmimb_lattice *h, const double *f_pre, double *f_post);
 lbmimb_status launch_fetch(lbmimb_lattice *h, int what, const int64_t lo[3], const int64_t hi[3], void *dst_dev);
 lbmimb_status launch_pack_records(lbmimb_lattice *h);
+lbmimb_status validate_particles_dev(lbmimb_lattice *h, int64_t P, const double *pos_dev, const double *radius_dev,
+                                     const double *mass_dev, double *rmax, double *rmin);
 lbmimb_status build_cell_list(lbmimb_lattice *h);
 lbmimb_status launch_map(lbmimb_lattice *h);
 lbmimb_status ensure_eps_table(lbmimb_lattice *h);
 int64_t eps_table_entries(int dim);
-lbmimb_status launch_reduce(lbmimb_lattice *h);
+lbmimb_status launch_finish_forces(lbmimb_lattice *h);   // facc -> force / torque, clears facc
 lbmimb_status launch_dem(lbmimb_lattice *h, const lbmimb_dem_params *dem);
 lbmimb_status neighbor_list_prepare(lbmimb_lattice *h);   // (re)allocates the list storage for the current radii
 void neighbor_list_release(lbmimb_lattice *h);

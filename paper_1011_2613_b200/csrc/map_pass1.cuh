@@ -10,7 +10,7 @@
 //            or two additions and a compare each.  Every operation is the same IEEE operation on
 //            the same operands as in the definition (include/lbmimb.h a1), so the counts are
 //            bit-exact; only the order in which samples are visited differs.
-// Nodes reached by more than one particle are detected with an atomic exchange on pid and
+// Nodes reached by more than one particle are detected with an atomic exchange on the node tag and
 // queued for pass 2 (map_contested_kernel), which recomputes them from the definition.
 // (Measured and dropped: one thread per ROW that writes the full columns itself and lists only the
 //  shell -- no per-node classification, but serial commits per thread: C3 0.325 -> 0.369 ms, C4 1.50 -> 1.73 ms.)
@@ -241,12 +241,12 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
     if (wy) j = wrap_i(j, a.g.ny);
     if (D == 3 && wz) k = wrap_i(k, a.g.nz);
   };
-  // The exchange on pid tells whether another particle reached the node first.  Its result is looked at
-  // one commit later (or at the end), so that the round trip of the atomic is off the critical path.
+  // The exchange on the node tag tells whether another particle reached the node first.  Its result is
+  // looked at one commit later (or at the end), so that the round trip of the atomic is off the critical path.
   int64_t pend_x = -1;
-  int32_t pend_old = -1;
+  uint32_t pend_old = 0;
   auto settle = [&]() {
-    if (pend_x >= 0 && pend_old != -1 && pend_old != (int32_t)p) {
+    if (pend_x >= 0 && pend_old != 0u && tag_pid(pend_old) != (int32_t)p) {
       const int slot = atomicAdd(a.counters, 1);
       if (slot < a.contested_cap) a.contested[slot] = pend_x;
       else a.counters[1] = 1;
@@ -256,9 +256,8 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
   auto commit = [&](int i, int j, int k, int cnt) {
     const int64_t x = ((int64_t)k * a.g.ny + j) * a.g.nx + i;
     settle();
-    pend_old = atomicExch(a.pid + x, (int32_t)p);
+    pend_old = atomicExch(a.tag + x, make_tag((int32_t)p, cnt));
     pend_x = x;
-    a.eps_cnt[x] = (uint8_t)cnt;
   };
 
   for (int row0 = 0; row0 < nrows_u; row0 += G) {

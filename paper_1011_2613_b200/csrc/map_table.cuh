@@ -106,7 +106,7 @@ __device__ __forceinline__ int table_code(const TableGeom &t, double dx, double 
 // box (map_pass1.cuh): a node can have a non-zero code only if d^2 <= none2, so every row (j,k) contributes
 // the columns with |dx| <= sqrt(none2 - dy^2 - dz^2) (+ margin: a superset) and the group walks the
 // concatenated intervals.  The look-up itself is unchanged.  Shared nodes are detected like in the sampled
-// map (exchange on pid, examined one commit later).
+// map (exchange on the node tag, examined one commit later).
 // ---------------------------------------------------------------------------
 template <int D, int G>
 __global__ void __launch_bounds__(128) map_table_kernel(const MapArgs a, const TableGeom t) {
@@ -149,9 +149,9 @@ __global__ void __launch_bounds__(128) map_table_kernel(const MapArgs a, const T
     if (D == 3 && wz) k = wrap_i(k, a.g.nz);
   };
   int64_t pend_x = -1;
-  int32_t pend_old = -1;
+  uint32_t pend_old = 0;
   auto settle = [&]() {
-    if (pend_x >= 0 && pend_old != -1 && pend_old != (int32_t)p) {
+    if (pend_x >= 0 && pend_old != 0u && tag_pid(pend_old) != (int32_t)p) {
       const int slot = atomicAdd(a.counters, 1);
       if (slot < a.contested_cap) a.contested[slot] = pend_x;
       else a.counters[1] = 1;
@@ -186,9 +186,8 @@ __global__ void __launch_bounds__(128) map_table_kernel(const MapArgs a, const T
       if (code > 0) {
         const int64_t x = ((int64_t)k * a.g.ny + j) * a.g.nx + i;
         settle();
-        pend_old = atomicExch(a.pid + x, (int32_t)p);
+        pend_old = atomicExch(a.tag + x, make_tag((int32_t)p, code));
         pend_x = x;
-        a.eps_cnt[x] = (uint8_t)code;
       }
     }
     group_sync<G>();
@@ -264,9 +263,6 @@ __global__ void __launch_bounds__(128) map_table_contested_kernel(const MapArgs 
         best_p = op;
       }
     }
-    if (lane == 0) {
-      a.eps_cnt[x] = (uint8_t)(sum > 255 ? 255 : sum);
-      a.pid[x] = best_p;
-    }
+    if (lane == 0) a.tag[x] = make_tag(best_p, sum > 255 ? 255 : sum);
   }
 }

@@ -1,7 +1,9 @@
 // Particle-side kernels: packed records, cell list (counting sort), the particle ->
 // lattice mapping (a1), the force/torque reduction (a3) and the soft-sphere DEM (a4).
 #include <cmath>
+#include <cstring>
 
+#include "collide.cuh"
 #include "lbmimb_internal.cuh"
 
 namespace lbmimb {
@@ -56,6 +58,57 @@ __global__ void pack_records_kernel(int dim, int64_t P, const double *__restrict
     r[8] = omega[2 * P + p];
     r[9] = radius[p];
   }
+}
+
+// ---------------------------------------------------------------------------
+// set_particles_dev: the checks the host variant does on its host arrays, done on the device BEFORE anything
+// is committed to the handle: radius and mass positive and finite, centres inside [-1/2, n) per axis;
+// also the largest / smallest radius (the cell-list geometry needs them on the host).
+// res: [0] number of bad particles, [1] lowest bad index + 1 (as a negative max), [2..3] rmax bits, [4..5] rmin bits
+// ---------------------------------------------------------------------------
+__global__ void validate_particles_kernel(int dim, int64_t P, int nx, int ny, int nz, const double *__restrict__ pos,
+                                          const double *__restrict__ radius, const double *__restrict__ mass,
+                                          int32_t *__restrict__ res) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  const double R = radius[p], m = mass[p];
+  bool ok = R > 0.0 && m > 0.0 && isfinite(R) && isfinite(m);
+  const int n[3] = {nx, ny, nz};
+  for (int a = 0; a < dim; ++a) {
+    const double x = pos[(int64_t)a * P + p];
+    ok = ok && x >= -0.5 && x < (double)n[a];
+  }
+  if (!ok) {
+    atomicAdd(res, 1);
+    atomicMax(res + 1, (int32_t)(0x7fffffff - (p > 0x7ffffffe ? 0x7ffffffe : p)));
+    return;
+  }
+  // positive finite doubles order like their bit patterns
+  atomicMax(reinterpret_cast<unsigned long long *>(res + 2), (unsigned long long)__double_as_longlong(R));
+  atomicMin(reinterpret_cast<unsigned long long *>(res + 4), (unsigned long long)__double_as_longlong(R));
+}
+
+lbmimb_status validate_particles_dev(lbmimb_lattice *h, int64_t P, const double *pos_dev, const double *radius_dev,
+                                     const double *mass_dev, double *rmax, double *rmin) {
+  int32_t *res = h->counters + 8;   // words 8..13 of the 16-word counter block
+  const unsigned long long init[3] = {0ull, 0ull, ~0ull};
+  LBMIMB_CUDA(cudaMemcpyAsync(res, init, sizeof(init), cudaMemcpyHostToDevice, h->stream));
+  validate_particles_kernel<<<blocks_for(P, 256), 256, 0, h->stream>>>(h->g.dim, P, h->g.nx, h->g.ny, h->g.nz, pos_dev,
+                                                                       radius_dev, mass_dev, res);
+  LBMIMB_LAUNCH_CHECK(h, "validate_particles_kernel");
+  unsigned long long out[3];
+  LBMIMB_CUDA(cudaMemcpyAsync(out, res, sizeof(out), cudaMemcpyDeviceToHost, h->stream));
+  LBMIMB_CUDA(cudaStreamSynchronize(h->stream));
+  const int32_t nbad = (int32_t)(out[0] & 0xffffffffu), enc = (int32_t)(out[0] >> 32);
+  if (nbad != 0)
+    return fail(LBMIMB_EINVAL, "%d particle(s) with a non-positive / non-finite radius or mass or a centre outside "
+                               "[-1/2, n); the first is particle %d", nbad, 0x7fffffff - enc);
+  long long b;
+  b = (long long)out[1];
+  memcpy(rmax, &b, 8);
+  b = (long long)out[2];
+  memcpy(rmin, &b, 8);
+  return LBMIMB_OK;
 }
 
 lbmimb_status launch_pack_records(lbmimb_lattice *h) {
@@ -265,8 +318,7 @@ struct MapArgs {
   int64_t P;
   const double *pos;
   const double *radius;
-  uint8_t *eps_cnt;
-  int32_t *pid;
+  uint32_t *tag;       // [N] node tags, make_tag(covering particle, count)
   int64_t *contested;
   int64_t contested_cap;
   int32_t *counters;
@@ -454,10 +506,7 @@ __global__ void __launch_bounds__(128) map_contested_kernel(const MapArgs a, con
     }
     int ucnt = 0;
     for (int m = 0; m * 32 < a.SD; ++m) ucnt += __popc(__ballot_sync(0xffffffffu, (ubits >> m) & 1u));
-    if (lane == 0) {
-      a.eps_cnt[x] = (uint8_t)ucnt;
-      a.pid[x] = best_p;
-    }
+    if (lane == 0) a.tag[x] = make_tag(best_p, ucnt);
   }
 }
 
@@ -525,9 +574,8 @@ static lbmimb_status launch_map_table(lbmimb_lattice *h, const MapArgs &a) {
 lbmimb_status launch_map(lbmimb_lattice *h) {
   lbmimb_status st;
   if (!h->cl_valid && (st = build_cell_list(h)) != LBMIMB_OK) return st;
-  LBMIMB_CUDA(cudaMemsetAsync(h->eps_cnt, 0, (size_t)h->g.N, h->stream));
-  LBMIMB_CUDA(cudaMemsetAsync(h->pid, 0xFF, (size_t)h->g.N * 4, h->stream));
-  LBMIMB_CUDA(cudaMemsetAsync(h->counters, 0, 4, h->stream));
+  LBMIMB_CUDA(cudaMemsetAsync(h->tag, 0, (size_t)h->g.N * 4, h->stream));
+  LBMIMB_CUDA(cudaMemsetAsync(h->counters, 0, 8, h->stream));   // shared-node count and its overflow flag
   MapArgs a;
   a.g = h->g;
   a.S = h->prm.subsamples;
@@ -535,8 +583,7 @@ lbmimb_status launch_map(lbmimb_lattice *h) {
   a.P = h->P;
   a.pos = h->pos;
   a.radius = h->radius;
-  a.eps_cnt = h->eps_cnt;
-  a.pid = h->pid;
+  a.tag = h->tag;
   a.contested = h->contested;
   a.contested_cap = h->contested_cap;
   a.counters = h->counters;
@@ -567,177 +614,41 @@ lbmimb_status launch_map(lbmimb_lattice *h) {
 }
 
 // ---------------------------------------------------------------------------
-// a3: force / torque reduction, eq. (3) with the sign of R6.  One group of G threads per particle.
-// A node can only belong to the particle if its centre is within R + h_out of the particle centre
-// (the map's own classification).  A whole-box walk spends most of its lane-slots on bounding-box
-// nodes that cannot belong to the particle (a sphere fills a third of its box, and a row of 11 nodes
-// occupies 16 lanes: C3 0.275 ms against 0.196 ms for the walk below).  Here every row (j,k) of the
-// box first gets the interval of columns that can hold a candidate, |i - cx| <= sqrt(rout^2 - ry^2 - rz^2) (+ margin: a superset), the interval lengths of a
-// chunk of G rows are scanned, and the threads then walk the concatenated intervals, so that nearly every
-// load that is issued is a node of the particle.  The per-node candidate test and the ownership test are
-// unchanged, so the same nodes are summed; traversal and tree order are fixed => bitwise reproducible.
-template <int D, int G>
-__global__ void __launch_bounds__(128) reduce_forces_dense_kernel(Geom g, int64_t P, double h_out,
-                                                                  const double *__restrict__ pos,
-                                                                  const double *__restrict__ radius,
-                                                                  const int32_t *__restrict__ pid,
-                                                                  const double *__restrict__ s,
-                                                                  double *__restrict__ force,
-                                                                  double *__restrict__ torque) {
-  constexpr int groups = 128 / G;
-  constexpr int NW = G >= 32 ? G / 32 : 1;
-  constexpr int SW = G < 32 ? G : 32;   // shuffle width of a group (two groups share a warp when G = 16)
+// a3: the per-particle sums of eq. (3) are formed inside the fused step (collide.cuh: accumulate_runs) as
+// fixed-point integers; this kernel turns them into force / torque and clears the accumulators for the
+// next emitting step.  (Round 1 wrote a 32-byte exchange record per covered node and gathered the records
+// per particle in a second pass over the bounding boxes: C3 0.38 GB written + 0.72 GB read, 0.18 ms.)
+// ---------------------------------------------------------------------------
+template <int D>
+__global__ void finish_forces_kernel(int64_t P, long long *__restrict__ facc, double *__restrict__ force,
+                                     double *__restrict__ torque) {
   constexpr int NV = D == 2 ? 3 : 6;
-  constexpr int U = 4;
-  __shared__ double sh[groups][NW][NV];
-  __shared__ int pre[groups][G + 1];   // exclusive prefix of the interval lengths of this chunk of rows
-  __shared__ int beg[groups][G];       // first box column of each row's interval
-  __shared__ int wtot[groups][NW];
-  const int grp = threadIdx.x / G, gl = threadIdx.x % G, lane = gl % SW, wid = gl >> 5;
-  const int64_t p = (int64_t)blockIdx.x * groups + grp;
-  double acc[NV];
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  longlong2 *acc = reinterpret_cast<longlong2 *>(facc + p * (2 * NV));
+  double v[NV];
 #pragma unroll
-  for (int v = 0; v < NV; ++v) acc[v] = 0.0;
-  double cx = 0.0, cy = 0.0, cz = 0.0, rout2 = 0.0;
-  int lo[3] = {0, 0, 0}, ext[3] = {0, 0, 1};
-  bool wx = false, wy = false, wz = false;
-  if (p < P) {
-    cx = pos[p];
-    cy = pos[P + p];
-    cz = D == 3 ? pos[2 * P + p] : 0.0;
-    const double R = radius[p];
-    bbox_axis(cx, R, g.nx, g.bcx, lo[0], ext[0]);
-    bbox_axis(cy, R, g.ny, g.bcy, lo[1], ext[1]);
-    if (D == 3) bbox_axis(cz, R, g.nz, g.bcz, lo[2], ext[2]);
-    rout2 = (R + h_out) * (R + h_out);
-    wx = crosses_seam(cx, R, g.nx, g.bcx);
-    wy = crosses_seam(cy, R, g.ny, g.bcy);
-    wz = D == 3 && crosses_seam(cz, R, g.nz, g.bcz);
-  }
-  auto wrap1 = [](int v, int n) { return v < 0 ? v + n : (v >= n ? v - n : v); };
-  const int nrows = (p < P && ext[0] > 0) ? ext[1] * ext[2] : 0;
-  // groups that share a warp synchronise with __syncwarp: they run the same number of passes
-  const int nrows_u = group_uniform_max<G>(nrows);
-  const float inv_e1 = 1.0f / (float)(ext[1] > 0 ? ext[1] : 1);
-  // G == 128: one group per block, so nrows is block-uniform and the block barrier is safe
-  for (int row0 = 0; row0 < nrows_u; row0 += G) {
-    int b0 = 0, len = 0;
-    {
-      const int row = row0 + gl;
-      if (row < nrows) {
-        int bk = 0, bj = row;
-        if (D == 3) fast_divmod(row, ext[1], inv_e1, bk, bj);
-        int j = lo[1] + bj, k = lo[2] + bk;
-        if (wy) j = wrap1(j, g.ny);
-        if (D == 3 && wz) k = wrap1(k, g.nz);
-        double ry = (double)j - cy, rz = D == 3 ? (double)k - cz : 0.0;
-        if (wy) ry = min_image_d(ry, g.ny);
-        if (D == 3 && wz) rz = min_image_d(rz, g.nz);
-        const double hw2 = rout2 - ry * ry - rz * rz;
-        if (hw2 > -1e-6) {
-          if (wx) {
-            len = ext[0];
-          } else {
-            clip_interval(cx, sqrt(fmax(hw2, 0.0) + 1e-6), lo[0], ext[0], b0, len);
-          }
-        }
-      }
-    }
-    const int total = scan_row_intervals<G>(len, b0, gl, pre[grp], beg[grp], wtot[grp]);
-    const int total_u = group_uniform_max<G>(total);
-    for (int t0 = gl; t0 < total_u; t0 += U * G) {
-      int32_t owner[U];
-      double2 s01[U], s23[U];
-      double rx[U], ry[U], rz[U];
-#pragma unroll
-      for (int u = 0; u < U; ++u) {
-        const int t = t0 + u * G;
-        owner[u] = -1;
-        s01[u] = s23[u] = make_double2(0.0, 0.0);
-        rx[u] = ry[u] = rz[u] = 0.0;
-        if (t < total) {
-          const int r = interval_row<G>(pre[grp], t);
-          const int bi = beg[grp][r] + (t - pre[grp][r]);
-          const int row = row0 + r;
-          int bk = 0, bj = row;
-          if (D == 3) fast_divmod(row, ext[1], inv_e1, bk, bj);
-          int i = lo[0] + bi, j = lo[1] + bj, k = lo[2] + bk;
-          if (wx) i = wrap1(i, g.nx);
-          if (wy) j = wrap1(j, g.ny);
-          if (D == 3 && wz) k = wrap1(k, g.nz);
-          rx[u] = (double)i - cx;
-          ry[u] = (double)j - cy;
-          rz[u] = D == 3 ? (double)k - cz : 0.0;
-          if (wx) rx[u] = min_image_d(rx[u], g.nx);
-          if (wy) ry[u] = min_image_d(ry[u], g.ny);
-          if (D == 3 && wz) rz[u] = min_image_d(rz[u], g.nz);
-          if (rx[u] * rx[u] + ry[u] * ry[u] + rz[u] * rz[u] <= rout2) {
-            const int64_t x = ((int64_t)k * g.ny + j) * g.nx + i;
-            const double2 *sr = reinterpret_cast<const double2 *>(s) + x * (exchange_stride(D) / 2);
-            owner[u] = __ldg(pid + x);
-            s01[u] = __ldg(sr);
-            if (D == 3) s23[u] = __ldg(sr + 1);
-          }
-        }
-      }
-#pragma unroll
-      for (int u = 0; u < U; ++u) {
-        if (owner[u] != (int32_t)p) continue;
-        const double sx = s01[u].x, sy = s01[u].y;
-        if (D == 2) {
-          acc[0] -= sx;
-          acc[1] -= sy;
-          acc[2] -= rx[u] * sy - ry[u] * sx;
-        } else {
-          const double sz = s23[u].x;
-          acc[0] -= sx;
-          acc[1] -= sy;
-          acc[2] -= sz;
-          acc[3] -= ry[u] * sz - rz[u] * sy;
-          acc[4] -= rz[u] * sx - rx[u] * sz;
-          acc[5] -= rx[u] * sy - ry[u] * sx;
-        }
-      }
-    }
-    group_sync<G>();
+  for (int c = 0; c < NV; ++c) {
+    const longlong2 w = acc[c];
+    v[c] = fixed_value(w.x, w.y);
+    acc[c] = make_longlong2(0, 0);
   }
 #pragma unroll
-  for (int v = 0; v < NV; ++v)
-    for (int o = SW / 2; o > 0; o >>= 1) acc[v] += __shfl_down_sync(0xffffffffu, acc[v], o, SW);
-  if (lane == 0)
-    for (int v = 0; v < NV; ++v) sh[grp][wid][v] = acc[v];
-  __syncthreads();
-  if (gl == 0 && p < P) {
-    double tot[NV];
-    for (int v = 0; v < NV; ++v) {
-      tot[v] = 0.0;
-      for (int w = 0; w < NW; ++w) tot[v] += sh[grp][w][v];
-    }
-    for (int c = 0; c < D; ++c) force[(int64_t)c * P + p] = tot[c];
-    if (D == 2) {
-      torque[p] = tot[2];
-    } else {
-      for (int c = 0; c < 3; ++c) torque[(int64_t)c * P + p] = tot[3 + c];
-    }
+  for (int c = 0; c < D; ++c) force[(int64_t)c * P + p] = v[c];
+  if (D == 2) {
+    torque[p] = v[2];
+  } else {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) torque[(int64_t)c * P + p] = v[3 + c];
   }
 }
 
-// half extent of a node's sample cloud plus a safety margin: a node whose centre is farther than
-// R + h from a particle centre has no sample inside that particle
-static double sample_cloud_radius(const lbmimb_lattice *h) {
-  if (h->map_mode == LBMIMB_MAP_TABLE) return 0.5 * sqrt((double)h->g.dim) + 1e-6;  // whole cell (R17)
-  return sqrt((double)h->g.dim) * (0.5 - 0.5 / (double)h->prm.subsamples) + 1e-6;
-}
-
-lbmimb_status launch_reduce(lbmimb_lattice *h) {
-  const double ho = sample_cloud_radius(h);
+lbmimb_status launch_finish_forces(lbmimb_lattice *h) {
   if (h->g.dim == 2)
-    reduce_forces_dense_kernel<2, 16><<<blocks_for(h->P, 8), 128, 0, h->stream>>>(h->g, h->P, ho, h->pos, h->radius,
-                                                                                  h->pid, h->s, h->force, h->torque);
+    finish_forces_kernel<2><<<blocks_for(h->P, 256), 256, 0, h->stream>>>(h->P, h->facc, h->force, h->torque);
   else
-    reduce_forces_dense_kernel<3, 128><<<blocks_for(h->P, 1), 128, 0, h->stream>>>(h->g, h->P, ho, h->pos, h->radius,
-                                                                                   h->pid, h->s, h->force, h->torque);
-  LBMIMB_LAUNCH_CHECK(h, "reduce_forces_dense_kernel");
+    finish_forces_kernel<3><<<blocks_for(h->P, 256), 256, 0, h->stream>>>(h->P, h->facc, h->force, h->torque);
+  LBMIMB_LAUNCH_CHECK(h, "finish_forces_kernel");
   return LBMIMB_OK;
 }
 
@@ -928,8 +839,12 @@ void neighbor_list_release(lbmimb_lattice *h) {
   h->nl.x_ref = nullptr;
 }
 
+// positions were replaced: no valid list, and the overflow flags of the old particle set are history
 lbmimb_status neighbor_list_invalidate(lbmimb_lattice *h) {
-  if (h->nl.mem) LBMIMB_CUDA(cudaMemsetAsync(h->nl.state + NL_VALID, 0, 4, h->stream));
+  if (h->nl.mem) {
+    LBMIMB_CUDA(cudaMemsetAsync(h->nl.state + NL_VALID, 0, 4, h->stream));
+    LBMIMB_CUDA(cudaMemsetAsync(h->nl.state + NL_OVF_LIST, 0, 8, h->stream));
+  }
   return LBMIMB_OK;
 }
 

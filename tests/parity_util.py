@@ -97,10 +97,12 @@ def assert_forces_close(gF, gT, ref, tol=FORCE_TOL, floor=True):
     return ForceCheck(rF, rT, (nfF, nfT), (nfF > 1.0, nfT > 1.0), rel)
 
 
-def gpu_run(lb, w, steps, f0=None, streaming=0):
+def gpu_run(lb, w, steps, f0=None, streaming=0, exchange_field=True):
     """Fixed-particle CUDA run through the C-ABI binding; returns (lattice, dict).
-    streaming: lb.STREAM_AB (0) or lb.STREAM_AA (1)."""
-    lat = lb.from_workload(w, streaming=streaming)
+    streaming: lb.STREAM_AB (0) or lb.STREAM_AA (1).  exchange_field: create the lattice with
+    LBMIMB_FLAG_EXCHANGE_FIELD so that the per-node exchange vectors can be fetched and compared
+    (the full-size runs switch it off: it is a diagnostic output, the forces do not need it)."""
+    lat = lb.from_workload(w, streaming=streaming, flags=lb.FLAG_EXCHANGE_FIELD if exchange_field else 0)
     if f0 is not None:
         lat.set_distributions(f0)
     if w.P:
@@ -111,7 +113,8 @@ def gpu_run(lb, w, steps, f0=None, streaming=0):
     if w.P:
         out["eps"] = lat.fetch_fields(lb.FIELD_EPS_CNT)
         out["pid"] = lat.fetch_fields(lb.FIELD_PID)
-        out["s"] = lat.fetch_fields(lb.FIELD_S)
+        if exchange_field:
+            out["s"] = lat.fetch_fields(lb.FIELD_S)
         out["force"], out["torque"] = lat.reduce_particle_forces()
     lat.synchronize()
     return lat, out

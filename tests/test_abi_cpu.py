@@ -72,8 +72,12 @@ def test_workspace_bytes_and_parameter_validation(lb):
     p = lb.make_params(3, (256, 1008, 256), (0, 1, 0), 0.7, (0, -1e-6, 0), 4)
     need = lb.workspace_bytes(p, 24600)
     N = 256 * 1008 * 256
-    assert need >= 2 * 19 * N * 8 + 5 * N + 3 * N * 8          # two f buffers + eps + pid + s
-    assert need < 2 * 19 * N * 8 * 1.25                        # and not much more
+    assert need >= 2 * 19 * N * 8 + 4 * N                      # two f buffers + one tag word per node
+    assert need < 2 * 19 * N * 8 * 1.05                        # and not much more
+    ps = lb.make_params(3, (256, 1008, 256), (0, 1, 0), 0.7, (0, -1e-6, 0), 4, flags=lb.FLAG_EXCHANGE_FIELD)
+    assert lb.workspace_bytes(ps, 24600) - need == 4 * N * 8   # the optional per-node exchange records
+    assert lb.workspace_bytes(lb.make_params(2, (16, 16), (0, 0), 0.8, (0, 0), 8, flags=2), 0) == 0   # unknown flag
+    assert lb.workspace_bytes(p, (1 << 24) + 1) == 0           # tags hold 24-bit particle indices
     p2 = lb.make_params(2, (8192, 32768), (0, 1), 0.55, (0, -1e-6), 8)
     assert lb.workspace_bytes(p2, 1166400) > 2 * 9 * 8192 * 32768 * 8     # > 2^31 elements per buffer
     for bad in (lb.make_params(2, (16, 16), (0, 0), 0.5, (0, 0), 8),      # tau

@@ -365,3 +365,88 @@ def test_error_behaviour(lb):
     assert F.shape == (2, 1) and T.shape == (1, 1)
     assert lat.launch_count() > 3
     lat.close()
+
+
+# ----------------------------------------------------------------------------- in-kernel force sums
+def test_in_kernel_force_sums_reproducible_and_independent_of_the_exchange_field(orc, lb):
+    """a3 is summed inside the fused step with fixed-point integer atomics: two lattices give bit-identical
+    forces, with or without the per-node exchange field, in either streaming mode; FIELD_S needs the flag;
+    sums of a step that was never reduced do not leak into the next one."""
+    w = inputs.reduced("C3")
+    rng = np.random.default_rng(3)
+    w.omega = rng.uniform(-2e-3, 2e-3, size=(3, w.P))
+    ref = oracle_run(orc, w, 5)
+    res = []
+    for streaming in (lb.STREAM_AB, lb.STREAM_AA):
+        for flags in (0, lb.FLAG_EXCHANGE_FIELD, 0):
+            lat = lb.from_workload(w, streaming=streaming, flags=flags)
+            lat.map_particles()
+            lat.step(3)
+            lat.step(1)                          # emits sums nobody reduces ...
+            lat.step(1)                          # ... which must not be added to these
+            res.append(lat.reduce_particle_forces())
+            if not flags:
+                with pytest.raises(lb.LbmimbError) as ei:
+                    lat.fetch_fields(lb.FIELD_S)
+                assert ei.value.status == lb.ESTATE
+            lat.close()
+    for F, T in res[1:]:
+        assert np.array_equal(F, res[0][0]) and np.array_equal(T, res[0][1])
+    assert_forces_close(res[0][0], res[0][1], ref)
+
+
+def test_particle_limit_is_24_bits(lb):
+    with pytest.raises(lb.LbmimbError) as ei:
+        lb.Lattice(2, (16, 16), (0, 0), 0.8, (0, 0), 8, max_particles=(1 << 24) + 1)
+    assert ei.value.status == lb.EINVAL
+
+
+def test_device_side_overflow_surfaces_in_every_synchronous_call_and_clears(orc, lb):
+    """12 coincident disks of radius 110 put ~11 x 38,000 entries on the list of shared nodes of a 1024 x 1024
+    lattice (capacity N/4 + 65536): the overflow is raised by the map kernel and must come back as ESTATE from
+    the calls that synchronise, not as a wrong map; a valid particle set afterwards clears it."""
+    n, P = (1024, 1024), 12
+    lat = lb.Lattice(2, n, (0, 0), 0.8, (0, 0), 8, max_particles=P)
+    pos = np.full((2, P), 500.25)
+    lat.set_particles(pos, np.zeros((2, P)), None, np.full(P, 110.0), np.ones(P))
+    lat.map_particles()
+    for call in (lambda: lat.fetch_fields(lb.FIELD_EPS_CNT, (0, 0, 0), (8, 8, 1)), lat.get_particles, lat.synchronize,
+                 lat.diagnostics):
+        with pytest.raises(lb.LbmimbError) as ei:
+            call()
+        assert ei.value.status == lb.ESTATE and "overflow" in str(ei.value)
+    lat.step(1)
+    with pytest.raises(lb.LbmimbError) as ei:
+        lat.reduce_particle_forces()
+    assert ei.value.status == lb.ESTATE
+    pos2 = np.array([[100.5, 400.25], [300.0, 700.75]])
+    rad2 = np.array([20.0, 30.5])
+    lat.set_particles(pos2, np.zeros((2, 2)), None, rad2, np.ones(2))
+    lat.map_particles()
+    eo, po = orc.map_particles(2, n, (0, 0), 8, pos2, rad2)
+    assert np.array_equal(lat.fetch_fields(lb.FIELD_EPS_CNT)[0], eo[0])
+    assert np.array_equal(lat.fetch_fields(lb.FIELD_PID)[0], po[0])
+    lat.synchronize()
+    lat.close()
+
+
+def test_set_particles_dev_rejects_bad_input_without_touching_the_handle(orc, lb):
+    import torch
+    w = inputs.reduced("C2")
+    lat = lb.from_workload(w)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    bad_pos = w.pos.copy()
+    bad_pos[1, 7] = w.n[1] + 3.0                                   # outside the domain
+    bad_mass = w.mass.copy()
+    bad_mass[3] = 0.0
+    for p_, m_ in ((bad_pos, w.mass), (w.pos, bad_mass)):
+        tp, tv, to, tr, tm = dev(p_), dev(w.vel), dev(w.omega), dev(w.radius), dev(m_)
+        with pytest.raises(lb.LbmimbError) as ei:
+            lat.set_particles_dev(w.P, tp.data_ptr(), tv.data_ptr(), to.data_ptr(), tr.data_ptr(), tm.data_ptr())
+        assert ei.value.status == lb.EINVAL
+    pg, vg, og = lat.get_particles()                              # still the set from_workload installed
+    assert np.array_equal(pg, w.pos) and np.array_equal(vg, w.vel)
+    lat.map_particles()
+    eo, po = orc.map_particles(w.dim, w.n, w.bc, w.subsamples, w.pos, w.radius)
+    assert np.array_equal(lat.fetch_fields(lb.FIELD_EPS_CNT), eo)
+    lat.close()

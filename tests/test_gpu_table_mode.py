@@ -90,7 +90,7 @@ def test_reduced_configs_in_table_mode(orc, lb, name):
         f, s = orc.step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, eps_cnt=eps, pid=pid, pos=w.pos,
                         vel=w.vel, omega=w.omega, want_s=True, eps_den=orc.TABLE_DEN)
     F, T, aF, aT = orc.forces(w.dim, w.n, w.bc, s, pid, w.pos)
-    lat = lb.from_workload(w, map_mode=lb.MAP_TABLE)
+    lat = lb.from_workload(w, map_mode=lb.MAP_TABLE, flags=lb.FLAG_EXCHANGE_FIELD)
     lat.map_particles()
     lat.step(steps)
     assert np.array_equal(lat.fetch_fields(lb.FIELD_EPS_CNT), eps)
