@@ -74,7 +74,33 @@ typedef struct {
   uint64_t workspace_bytes; /* size of workspace_dev; must be >= lbmimb_workspace_bytes() */
   int32_t streaming;  /* LBMIMB_STREAM_AB (0, default) or LBMIMB_STREAM_AA: how step() propagates, see below */
   int32_t flags;      /* 0, or LBMIMB_FLAG_EXCHANGE_FIELD */
+  int64_t slab_y0;    /* slab lattices only: global index of this lattice's first owned row */
+  int64_t slab_ny;    /* rows of the GLOBAL lattice; 0 (default) = this lattice is the whole one */
 } lbmimb_params;
+
+/*
+ * Slabs: domain decomposition along y ("Parallel implementation", Fig. 2).
+ * A lattice with slab_ny > 0 owns the rows [slab_y0, slab_y0 + n[1]) of a global lattice of slab_ny rows
+ * (x and z whole).  bc[1] is the boundary of the GLOBAL lattice; an end of the slab that is not such a wall gets
+ * one ghost row (lbmimb_slab_ghost_rows).  One time step of the decomposed lattice:
+ *     every slab:  lbmimb_map_particles, lbmimb_step(h, 1)
+ *     every slab, every end with a ghost row:  lbmimb_pack_halo(h, side, buf)  ->  transport to the neighbour
+ *                  ->  lbmimb_unpack_halo(neighbour, 1 - side, buf)            (before the neighbour's next step)
+ *     particles cut by a slab face: lbmimb_export_force_sums_dev on every slab, integer SUM over the slabs (any
+ *                  order: the sums are fixed-point integers), lbmimb_import_force_sums_dev, then
+ *                  lbmimb_reduce_particle_forces / lbmimb_dem_step on every slab (the particles are replicated).
+ * What crosses a face per step: the 5 (D3Q19) / 3 (D2Q9) populations that stream through it, n[0]*n[2] nodes
+ * each (lbmimb_halo_count doubles), and 12 (6) 64-bit words per particle.  The transport (peer copies, NCCL,
+ * MPI) is the caller's: the library only packs and unpacks device buffers.
+ * Particles keep GLOBAL coordinates and every slab is given ALL of them, so the map, V_S, the lever arms and the
+ * DEM step are the same arithmetic as on the undivided lattice: maps and force sums agree with it bit for bit,
+ * distributions to rounding order (none changes: bit for bit as well).  Ownership rule for a particle cut by a
+ * face: every covered node adds to the sums of the slab that OWNS the node; ghost rows add nothing.
+ * fetch_fields addresses the owned rows (row 0 = first owned row); set_distributions takes the STORED rows
+ * (ghost rows included, i.e. global rows slab_y0 - ghost_lo ... , wrapped on a periodic axis).
+ * lbmimb_diagnostics sums over the owned rows only.  Slab lattices stream with two arrays (LBMIMB_STREAM_AB);
+ * lbmimb_run_coupled is not available on them (the force sums must cross slabs inside the step).
+ */
 
 /*
  * flags.  EXCHANGE_FIELD: keep the exchange vector s of every covered node of the last step in device memory
@@ -300,6 +326,30 @@ lbmimb_status lbmimb_set_particles_dev(lbmimb_lattice *h, int64_t P, const doubl
                                        const double *vel_dev, const double *omega_dev,
                                        const double *radius_dev, const double *mass_dev);
 lbmimb_status lbmimb_reduce_particle_forces_dev(lbmimb_lattice *h, double *force_dev, double *torque_dev);
+
+/*
+ * Slab lattices (see "Slabs" above).  side: 0 = lower (y-) end, 1 = upper (y+) end.
+ * pack_halo copies the populations LEAVING through that end (c_y = -1 for side 0, +1 for side 1) of the
+ * first / last owned row of the current (post-collision) state into dst_dev, laid out [slot][k][i] with the
+ * slots in ascending direction index (D2Q9: 4,6,7 | 3,5,8; D3Q19: 4,8,9,16,18 | 3,7,10,15,17);
+ * unpack_halo stores such a buffer, packed by the neighbour across that end with the opposite side, in the
+ * ghost row of that end.  lbmimb_halo_count doubles per buffer.  Asynchronous on the handle's stream.
+ * ESTATE: not a slab, or that end is a wall of the global lattice.
+ */
+int64_t lbmimb_halo_count(const lbmimb_lattice *h);
+int32_t lbmimb_slab_ghost_rows(const lbmimb_lattice *h, int32_t side); /* 0 or 1; -1 on bad arguments */
+lbmimb_status lbmimb_pack_halo(lbmimb_lattice *h, int32_t side, double *dst_dev);
+lbmimb_status lbmimb_unpack_halo(lbmimb_lattice *h, int32_t side, const double *src_dev);
+/*
+ * The per-particle force / torque sums of the last step as the integers the fused kernel accumulated:
+ * lbmimb_force_sums_count(h) = P * (3 | 6) * 2 int64 words ([P][value][hi, lo], value = hi 2^-40 + lo 2^-92).
+ * Adding the arrays of all slabs word by word gives the sums of the undivided lattice exactly.  export copies
+ * them out, import replaces them (both asynchronous).  ESTATE unless a step has run since the last map and
+ * reduce_particle_forces has not consumed the sums yet.
+ */
+int64_t lbmimb_force_sums_count(const lbmimb_lattice *h);
+lbmimb_status lbmimb_export_force_sums_dev(lbmimb_lattice *h, int64_t *dst_dev);
+lbmimb_status lbmimb_import_force_sums_dev(lbmimb_lattice *h, const int64_t *src_dev);
 
 /* Blocks until all work queued on the handle's stream has finished. */
 lbmimb_status lbmimb_synchronize(lbmimb_lattice *h);

@@ -31,6 +31,8 @@ EXPORTS = [
     "lbmimb_synchronize", "lbmimb_time", "lbmimb_launch_count", "lbmimb_last_error", "lbmimb_version",
     "lbmimb_set_mapping_mode", "lbmimb_fetch_eps_table", "lbmimb_diagnostics",
     "lbmimb_set_neighbor_mode", "lbmimb_fetch_neighbor_list", "lbmimb_run_coupled",
+    "lbmimb_halo_count", "lbmimb_slab_ghost_rows", "lbmimb_pack_halo", "lbmimb_unpack_halo",
+    "lbmimb_force_sums_count", "lbmimb_export_force_sums_dev", "lbmimb_import_force_sums_dev",
 ]
 DIAG_LEN = 20
 
@@ -39,7 +41,7 @@ class Params(C.Structure):
     _fields_ = [("dim", C.c_int32), ("subsamples", C.c_int32), ("n", C.c_int64 * 3), ("bc", C.c_int32 * 3),
                 ("device", C.c_int32), ("tau", C.c_double), ("g_fluid", C.c_double * 3), ("stream", C.c_void_p),
                 ("workspace_dev", C.c_void_p), ("workspace_bytes", C.c_uint64), ("streaming", C.c_int32),
-                ("flags", C.c_int32)]
+                ("flags", C.c_int32), ("slab_y0", C.c_int64), ("slab_ny", C.c_int64)]
 
 
 class DemParams(C.Structure):
@@ -89,6 +91,16 @@ def load():
     lib.lbmimb_fetch_fields.argtypes = [vp, i32, C.POINTER(i64), C.POINTER(i64), vp]
     lib.lbmimb_set_distributions.argtypes = [vp, vp]
     lib.lbmimb_diagnostics.argtypes = [vp, vp]
+    lib.lbmimb_halo_count.restype = i64
+    lib.lbmimb_halo_count.argtypes = [vp]
+    lib.lbmimb_slab_ghost_rows.restype = i32
+    lib.lbmimb_slab_ghost_rows.argtypes = [vp, i32]
+    lib.lbmimb_pack_halo.argtypes = [vp, i32, vp]
+    lib.lbmimb_unpack_halo.argtypes = [vp, i32, vp]
+    lib.lbmimb_force_sums_count.restype = i64
+    lib.lbmimb_force_sums_count.argtypes = [vp]
+    lib.lbmimb_export_force_sums_dev.argtypes = [vp, vp]
+    lib.lbmimb_import_force_sums_dev.argtypes = [vp, vp]
     lib.lbmimb_synchronize.argtypes = [vp]
     lib.lbmimb_time.restype = i64
     lib.lbmimb_time.argtypes = [vp]
@@ -122,7 +134,8 @@ def version():
 
 
 def make_params(dim, n, bc, tau, g_fluid, subsamples, device=0, stream=0, workspace_dev=0, workspace_bytes=0,
-                streaming=STREAM_AB, flags=0):
+                streaming=STREAM_AB, flags=0, slab=None):
+    """slab = (y0, global_ny): this lattice owns rows [y0, y0 + n[1]) of a global lattice of global_ny rows."""
     p = Params()
     p.dim = dim
     p.subsamples = subsamples
@@ -140,6 +153,7 @@ def make_params(dim, n, bc, tau, g_fluid, subsamples, device=0, stream=0, worksp
     p.workspace_bytes = workspace_bytes
     p.streaming = streaming
     p.flags = flags
+    p.slab_y0, p.slab_ny = (int(slab[0]), int(slab[1])) if slab else (0, 0)
     return p
 
 
@@ -151,7 +165,7 @@ class Lattice:
     """Owner of one lbmimb_lattice handle.  Method names = C entry points without the prefix."""
 
     def __init__(self, dim, n, bc, tau, g_fluid, subsamples, max_particles=0, device=0, use_torch=True,
-                 streaming=STREAM_AB, flags=0):
+                 streaming=STREAM_AB, flags=0, slab=None):
         self.lib = load()
         self.dim = dim
         self.n = tuple(int(v) for v in n) + (1,) * (3 - len(n))
@@ -160,7 +174,7 @@ class Lattice:
         self._ws = None
         stream = 0
         ws_ptr, ws_bytes = 0, 0
-        probe = make_params(dim, n, bc, tau, g_fluid, subsamples, device, streaming=streaming, flags=flags)
+        probe = make_params(dim, n, bc, tau, g_fluid, subsamples, device, streaming=streaming, flags=flags, slab=slab)
         if use_torch:
             import torch
             if not torch.cuda.is_available():
@@ -173,7 +187,8 @@ class Lattice:
                 self._ws = torch.empty(need + 256, dtype=torch.uint8, device="cuda:%d" % device)
             ws_ptr = (self._ws.data_ptr() + 255) & ~255
             ws_bytes = need
-        self.params = make_params(dim, n, bc, tau, g_fluid, subsamples, device, stream, ws_ptr, ws_bytes, streaming, flags)
+        self.params = make_params(dim, n, bc, tau, g_fluid, subsamples, device, stream, ws_ptr, ws_bytes, streaming, flags,
+                                  slab)
         h = C.c_void_p()
         _check(self.lib.lbmimb_create_lattice(C.byref(self.params), max_particles, C.byref(h)))
         self.h = h
@@ -297,7 +312,8 @@ class Lattice:
 
     def set_distributions(self, f):
         f = _f64(f)
-        assert f.size == self.Q * self.n[0] * self.n[1] * self.n[2]
+        rows = self.n[1] + (self.slab_ghost_rows(0) + self.slab_ghost_rows(1) if self.params.slab_ny else 0)
+        assert f.size == self.Q * self.n[0] * rows * self.n[2]      # a slab takes its STORED rows (ghosts included)
         _check(self.lib.lbmimb_set_distributions(self.h, _hp(f)))
 
     def diagnostics(self):
@@ -308,6 +324,28 @@ class Lattice:
         return {"gas_area": out[0], "mass": out[1], "gas_velocity": out[2:2 + D], "solid_velocity": out[5:5 + D],
                 "slip": out[8:8 + D], "drag": out[11:11 + D], "fluid_momentum": out[14:14 + D],
                 "solid_momentum": out[17:17 + D], "vector": out}
+
+    # -- slabs (NEXT-4): device pointers in, device pointers out ------------------------------------
+    def halo_count(self):
+        return int(self.lib.lbmimb_halo_count(self.h))
+
+    def slab_ghost_rows(self, side):
+        return int(self.lib.lbmimb_slab_ghost_rows(self.h, side))
+
+    def pack_halo(self, side, dst_ptr):
+        _check(self.lib.lbmimb_pack_halo(self.h, side, dst_ptr))
+
+    def unpack_halo(self, side, src_ptr):
+        _check(self.lib.lbmimb_unpack_halo(self.h, side, src_ptr))
+
+    def force_sums_count(self):
+        return int(self.lib.lbmimb_force_sums_count(self.h))
+
+    def export_force_sums_dev(self, dst_ptr):
+        _check(self.lib.lbmimb_export_force_sums_dev(self.h, dst_ptr))
+
+    def import_force_sums_dev(self, src_ptr):
+        _check(self.lib.lbmimb_import_force_sums_dev(self.h, src_ptr))
 
     def synchronize(self):
         _check(self.lib.lbmimb_synchronize(self.h))

@@ -50,11 +50,43 @@ static bool valid_params(const lbmimb_params *p, int64_t maxp) {
   if (p->streaming != LBMIMB_STREAM_AB && p->streaming != LBMIMB_STREAM_AA)
     return fail(LBMIMB_EINVAL, "streaming must be LBMIMB_STREAM_AB or LBMIMB_STREAM_AA"), false;
   if ((p->flags & ~LBMIMB_FLAG_EXCHANGE_FIELD) != 0) return fail(LBMIMB_EINVAL, "unknown bit in flags"), false;
+  if (p->slab_ny != 0) {
+    if (p->slab_ny < 0 || p->slab_ny > 0x7fffffff || p->slab_y0 < 0 || p->slab_y0 + p->n[1] > p->slab_ny)
+      return fail(LBMIMB_EINVAL, "slab rows [%lld, %lld) do not fit a lattice of %lld rows", (long long)p->slab_y0,
+                  (long long)(p->slab_y0 + p->n[1]), (long long)p->slab_ny), false;
+    if (p->streaming != LBMIMB_STREAM_AB)
+      return fail(LBMIMB_EINVAL, "slab lattices stream with two arrays (LBMIMB_STREAM_AB)"), false;
+  } else if (p->slab_y0 != 0) {
+    return fail(LBMIMB_EINVAL, "slab_y0 without slab_ny"), false;
+  }
   if (maxp < 0 || maxp > kMaxParticles)
     return fail(LBMIMB_EINVAL, "max_particles out of range (node tags hold 24-bit particle indices)"), false;
   double nn = (double)p->n[0] * (double)p->n[1] * (double)p->n[2];
   if (nn > 4.0e12) return fail(LBMIMB_EINVAL, "lattice too large"), false;
   return true;
+}
+
+// Rows a lattice stores and how they map to the global lattice (lbmimb_internal.cuh: SlabRows).
+static SlabRows slab_rows(const lbmimb_params *p) {
+  SlabRows s;
+  if (p->slab_ny == 0) {
+    s.ny_stored = s.gny = (int)p->n[1];
+    s.oy = 0;
+    s.own_lo = 0;
+    s.own_hi = (int)p->n[1];
+    s.wall_lo = s.wall_hi = p->bc[1];
+    return s;
+  }
+  const int ghost_lo = !(p->bc[1] == 1 && p->slab_y0 == 0);
+  const int ghost_hi = !(p->bc[1] == 1 && p->slab_y0 + p->n[1] == p->slab_ny);
+  s.ny_stored = (int)p->n[1] + ghost_lo + ghost_hi;
+  s.gny = (int)p->slab_ny;
+  s.oy = (int)p->slab_y0 - ghost_lo;
+  s.own_lo = ghost_lo;
+  s.own_hi = ghost_lo + (int)p->n[1];
+  s.wall_lo = !ghost_lo;
+  s.wall_hi = !ghost_hi;
+  return s;
 }
 
 // One place that decides the device memory layout; used for sizing and for carving.
@@ -70,11 +102,15 @@ static Layout make_layout(const lbmimb_params *p, int64_t maxp) {
   Layout L;
   memset(&L, 0, sizeof(L));
   int Q = p->dim == 2 ? 9 : 19;
-  L.N = p->n[0] * p->n[1] * p->n[2];
+  const SlabRows sr = slab_rows(p);
+  L.N = p->n[0] * (int64_t)sr.ny_stored * p->n[2];
   int64_t pm = maxp > 0 ? maxp : 1;
   L.contested_cap = L.N / 4 + 65536;
   L.ncells_max = 1;
-  for (int a = 0; a < p->dim; ++a) L.ncells_max *= (p->n[a] / 2 > 0 ? p->n[a] / 2 : 1);
+  for (int a = 0; a < p->dim; ++a) {   // the particles live in the GLOBAL lattice
+    const int64_t na = a == 1 ? sr.gny : p->n[a];
+    L.ncells_max *= (na / 2 > 0 ? na / 2 : 1);
+  }
   uint64_t o = 0;
   auto take = [&](uint64_t bytes) {
     uint64_t r = o;
@@ -84,11 +120,11 @@ static Layout make_layout(const lbmimb_params *p, int64_t maxp) {
   L.off_f[0] = take((uint64_t)Q * L.N * 8);
   L.off_f[1] = p->streaming == LBMIMB_STREAM_AA ? L.off_f[0] : take((uint64_t)Q * L.N * 8);
   L.off_tag = take((uint64_t)L.N * 4);
+  L.off_counters = take(64);   // directly behind the tags: one memset clears the map and its counters
   L.off_s = (p->flags & LBMIMB_FLAG_EXCHANGE_FIELD) ? take((uint64_t)exchange_stride(p->dim) * L.N * 8) : 0;
   L.off_facc = take((uint64_t)pm * force_values(p->dim) * 16);
   L.off_beta = take(256 * 8);
   L.off_contested = take((uint64_t)L.contested_cap * 8);
-  L.off_counters = take(64);
   L.off_table = take((uint64_t)eps_table_entries(p->dim));
   L.off_diag = take((uint64_t)(kDiagBlocksMax * 8 + 32) * 8);
   L.off_pos = take((uint64_t)3 * pm * 8);
@@ -159,14 +195,19 @@ lbmimb_status lbmimb_create_lattice(const lbmimb_params *params, int64_t max_par
   if (!h) return fail(LBMIMB_ENOMEM, "host allocation failed");
   memset(h, 0, sizeof(*h));
   h->prm = *params;
+  h->sl = slab_rows(params);
+  h->is_slab = params->slab_ny != 0;
   h->g.dim = params->dim;
   h->g.nx = (int)params->n[0];
-  h->g.ny = (int)params->n[1];
+  h->g.ny = h->sl.ny_stored;
   h->g.nz = (int)params->n[2];
   h->g.bcx = params->bc[0];
   h->g.bcy = params->bc[1];
   h->g.bcz = params->dim == 3 ? params->bc[2] : 0;
-  h->g.N = params->n[0] * params->n[1] * params->n[2];
+  h->g.N = params->n[0] * (int64_t)h->sl.ny_stored * params->n[2];
+  h->gp = h->g;
+  h->gp.ny = h->sl.gny;
+  h->gp.N = params->n[0] * (int64_t)h->sl.gny * params->n[2];
   h->Q = params->dim == 2 ? 9 : 19;
   h->SD = 1;
   for (int a = 0; a < params->dim; ++a) h->SD *= params->subsamples;
@@ -305,7 +346,8 @@ lbmimb_status lbmimb_set_particles(lbmimb_lattice *h, int64_t P, const double *p
       return fail(LBMIMB_EINVAL, "particle %lld: radius and mass must be positive and finite", (long long)p);
     for (int a = 0; a < D; ++a) {
       double x = pos[(int64_t)a * P + p];
-      if (!(x >= -0.5) || !(x < (double)h->prm.n[a] - 0.5 + 0.5))  // [ -1/2, n ) accepted (DEM wraps into [0,n))
+      const double na = a == 1 ? (double)h->gp.ny : (double)h->prm.n[a];
+      if (!(x >= -0.5) || !(x < na))  // [ -1/2, n ) accepted (DEM wraps into [0,n))
         return fail(LBMIMB_EINVAL, "particle %lld: centre outside the domain on axis %d", (long long)p, a);
     }
     if (radius[p] > rmax) rmax = radius[p];
@@ -561,15 +603,16 @@ static lbmimb_status check_dem_params(const lbmimb_dem_params *dem) {
   return LBMIMB_OK;
 }
 
-static lbmimb_status dem_body(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
+static lbmimb_status dem_body(lbmimb_lattice *h, const lbmimb_dem_params *dem, bool finish) {
   if (h->P == 0) return LBMIMB_OK;
   lbmimb_status st;
-  if ((st = launch_dem(h, dem)) != LBMIMB_OK) return st;
+  const bool small = dem_small_path(h);
+  if ((st = launch_dem(h, dem, finish)) != LBMIMB_OK) return st;
   // positions moved: the map and the exchange vectors are stale; the cell list was rebuilt at
   // the new positions inside the step and stays valid; force/torque stay "the last reduction"
   h->map_valid = false;
   h->s_valid = false;
-  return launch_pack_records(h);
+  return small ? LBMIMB_OK : launch_pack_records(h);   // the single-block step packs the records itself
 }
 
 lbmimb_status lbmimb_dem_step(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
@@ -578,7 +621,7 @@ lbmimb_status lbmimb_dem_step(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
   if (st != LBMIMB_OK) return st;
   if (h->P == 0) return LBMIMB_OK;
   if ((st = use_device(h)) != LBMIMB_OK) return st;
-  return dem_body(h, dem);
+  return dem_body(h, dem, false);
 }
 
 // ---- lbmimb_run_coupled: the coupled loop with its launches replayed from a CUDA graph ----
@@ -586,8 +629,13 @@ static lbmimb_status coupled_step_body(lbmimb_lattice *h, const lbmimb_dem_param
   lbmimb_status st;
   if ((st = map_body(h)) != LBMIMB_OK) return st;
   if ((st = step_body(h, 1)) != LBMIMB_OK) return st;
+  if (h->P > 0 && dem_small_path(h)) {   // a3's conversion of the sums rides in the single-block DEM kernel
+    h->forces_valid = true;
+    h->acc_dirty = false;
+    return dem_body(h, dem, true);
+  }
   if ((st = reduce_body(h)) != LBMIMB_OK) return st;
-  return dem_body(h, dem);
+  return dem_body(h, dem, false);
 }
 
 static bool coupled_graph_matches(const lbmimb_lattice *h, const CoupledGraph &g, const lbmimb_dem_params *dem) {
@@ -677,6 +725,8 @@ lbmimb_status lbmimb_run_coupled(lbmimb_lattice *h, const lbmimb_dem_params *dem
   lbmimb_status st = check_dem_params(dem);
   if (st != LBMIMB_OK) return st;
   if (nsteps < 0) return fail(LBMIMB_EINVAL, "nsteps < 0");
+  if (h->is_slab)
+    return fail(LBMIMB_ESTATE, "run_coupled is not available on a slab lattice: the force sums cross slabs inside the step");
   if ((st = use_device(h)) != LBMIMB_OK) return st;
   if (h->P == 0) return step_body(h, nsteps);   // no particles: the other three calls are no-ops
   int32_t left = nsteps;
@@ -768,7 +818,7 @@ lbmimb_status lbmimb_fetch_fields(lbmimb_lattice *h, int32_t what, const int64_t
   if (!lo || !hi || !dst) return fail(LBMIMB_EINVAL, "NULL argument");
   int64_t box = 1;
   for (int a = 0; a < 3; ++a) {
-    int64_t na = a == 0 ? h->g.nx : (a == 1 ? h->g.ny : h->g.nz);
+    int64_t na = a == 0 ? h->g.nx : (a == 1 ? h->sl.own_hi - h->sl.own_lo : h->g.nz);   // rows: the owned ones
     if (lo[a] < 0 || hi[a] > na || lo[a] >= hi[a]) return fail(LBMIMB_EINVAL, "box out of range on axis %d", a);
     box *= hi[a] - lo[a];
   }
@@ -821,6 +871,59 @@ lbmimb_status lbmimb_diagnostics(lbmimb_lattice *h, double *out) {
   if ((st = launch_diagnostics(h, den)) != LBMIMB_OK) return st;
   LBMIMB_CUDA(cudaMemcpyAsync(out, h->diag_out, LBMIMB_DIAG_LEN * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
   return sync_and_check(h);
+}
+
+// ---- slab decomposition (NEXT-4): halo pack / unpack and the per-slab force sums ----
+int64_t lbmimb_halo_count(const lbmimb_lattice *h) { return h ? halo_doubles(h) : -1; }
+
+int32_t lbmimb_slab_ghost_rows(const lbmimb_lattice *h, int32_t side) {
+  if (!h || (side != 0 && side != 1)) return -1;
+  return side == 0 ? h->sl.own_lo : h->sl.ny_stored - h->sl.own_hi;
+}
+
+static lbmimb_status halo_common(lbmimb_lattice *h, int32_t side, double *buf_dev, bool pack) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (side != 0 && side != 1) return fail(LBMIMB_EINVAL, "side must be 0 (lower y end) or 1 (upper y end)");
+  if (!buf_dev) return fail(LBMIMB_EINVAL, "buffer is NULL");
+  if (!h->is_slab) return fail(LBMIMB_ESTATE, "not a slab lattice (params.slab_ny = 0)");
+  if (lbmimb_slab_ghost_rows(h, side) == 0)
+    return fail(LBMIMB_ESTATE, "the %s end of this slab is a wall of the global lattice: nothing crosses it",
+                side == 0 ? "lower" : "upper");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  return launch_halo(h, side, buf_dev, pack);
+}
+
+lbmimb_status lbmimb_pack_halo(lbmimb_lattice *h, int32_t side, double *dst_dev) {
+  return halo_common(h, side, dst_dev, true);
+}
+
+lbmimb_status lbmimb_unpack_halo(lbmimb_lattice *h, int32_t side, const double *src_dev) {
+  return halo_common(h, side, const_cast<double *>(src_dev), false);
+}
+
+int64_t lbmimb_force_sums_count(const lbmimb_lattice *h) { return h ? h->P * force_values(h->g.dim) * 2 : -1; }
+
+lbmimb_status lbmimb_export_force_sums_dev(lbmimb_lattice *h, int64_t *dst_dev) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (!dst_dev) return fail(LBMIMB_EINVAL, "dst_dev is NULL");
+  if (h->P > 0 && (!h->s_valid || h->forces_valid))
+    return fail(LBMIMB_ESTATE, "no unreduced force sums: call after lbmimb_step and before lbmimb_reduce_particle_forces");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  LBMIMB_CUDA(cudaMemcpyAsync(dst_dev, h->facc, (size_t)lbmimb_force_sums_count(h) * 8, cudaMemcpyDeviceToDevice, h->stream));
+  return LBMIMB_OK;
+}
+
+lbmimb_status lbmimb_import_force_sums_dev(lbmimb_lattice *h, const int64_t *src_dev) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (!src_dev) return fail(LBMIMB_EINVAL, "src_dev is NULL");
+  if (h->P > 0 && (!h->s_valid || h->forces_valid))
+    return fail(LBMIMB_ESTATE, "no unreduced force sums: call after lbmimb_step and before lbmimb_reduce_particle_forces");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  LBMIMB_CUDA(cudaMemcpyAsync(h->facc, src_dev, (size_t)lbmimb_force_sums_count(h) * 8, cudaMemcpyDeviceToDevice, h->stream));
+  return LBMIMB_OK;
 }
 
 lbmimb_status lbmimb_set_distributions(lbmimb_lattice *h, const double *f) {

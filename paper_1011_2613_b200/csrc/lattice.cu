@@ -24,6 +24,7 @@ struct StepArgs {
   int nx, ny, nz;
   int bcx, bcy, bcz;
   unsigned tiles;      // blocks per lattice row
+  SlabRows sl;         // stored rows <-> global rows, wall flags of the two y ends, owned rows
   CollideParams cp;
   // AA odd step, rows away from walls and seams: f_q(x) lives koff[q] bytes behind element x - cx_q
   // of the array (koff[q] = 8 (opposite(q) * N - cy_q * nx - cz_q * nx * ny))
@@ -94,8 +95,8 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
     bool bounce = false;
     int js = j - cy, ks = k - cz;
     if (cy != 0 && (js < 0 || js >= a.ny)) {
-      if (a.bcy) bounce = true;
-      else js = js < 0 ? js + a.ny : js - a.ny;
+      if (js < 0 ? a.sl.wall_lo : a.sl.wall_hi) bounce = true;
+      else js = js < 0 ? js + a.ny : js - a.ny;   // periodic, or a ghost row pulling garbage nobody reads
     }
     if (D == 3 && cz != 0 && (ks < 0 || ks >= a.nz)) {
       if (a.bcz) bounce = true;
@@ -118,8 +119,8 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
   double beta = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, rx = 0.0, ry = 0.0, rz = 0.0;
   if (IMB && cnt > 0) {
     beta = __ldg(a.beta_tab + cnt);
-    solid_velocity<D>(a.prec + (int64_t)pe * prec_stride(D), i, j, k, a.nx, a.ny, a.nz, a.bcx, a.bcy, a.bcz, vx, vy,
-                      vz, rx, ry, rz);
+    solid_velocity<D>(a.prec + (int64_t)pe * prec_stride(D), i, slab_global_row(a.sl, j), k, a.nx, a.sl.gny, a.nz, a.bcx,
+                      a.bcy, a.bcz, vx, vy, vz, rx, ry, rz);
   }
 
   double rho, ux, uy, uz;
@@ -134,7 +135,8 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
     for (int q = 0; q < Q; ++q) a.fout[(int64_t)q * a.N + x] = f[q];
   }
   if (EMIT != kEmitNone && solid_warp)
-    emit_exchange<D, EMIT>(a, x, cnt > 0 && live, pe, beta, rho, ux, uy, uz, vx, vy, vz, rx, ry, rz);
+    emit_exchange<D, EMIT>(a, x, cnt > 0 && live && j >= a.sl.own_lo && j < a.sl.own_hi, pe, beta, rho, ux, uy, uz, vx,
+                           vy, vz, rx, ry, rz);
 }
 
 // ---------------------------------------------------------------------------
@@ -191,7 +193,7 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_aa_kernel(c
     int jj = j - cy, kk = k - cz;
     bool bounce = false;
     if (cy != 0 && (jj < 0 || jj >= a.ny)) {
-      if (a.bcy) bounce = true;
+      if (jj < 0 ? a.sl.wall_lo : a.sl.wall_hi) bounce = true;
       else jj = jj < 0 ? jj + a.ny : jj - a.ny;
     }
     if (D == 3 && cz != 0 && (kk < 0 || kk >= a.nz)) {
@@ -219,8 +221,8 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_aa_kernel(c
   double beta = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, rx = 0.0, ry = 0.0, rz = 0.0;
   if (IMB && cnt > 0) {
     beta = __ldg(a.beta_tab + cnt);
-    solid_velocity<D>(a.prec + (int64_t)pe * prec_stride(D), i, j, k, a.nx, a.ny, a.nz, a.bcx, a.bcy, a.bcz, vx, vy,
-                      vz, rx, ry, rz);
+    solid_velocity<D>(a.prec + (int64_t)pe * prec_stride(D), i, slab_global_row(a.sl, j), k, a.nx, a.sl.gny, a.nz, a.bcx,
+                      a.bcy, a.bcz, vx, vy, vz, rx, ry, rz);
   }
 
   double rho, ux, uy, uz;
@@ -243,7 +245,8 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_aa_kernel(c
     }
   }
   if (EMIT != kEmitNone && solid_warp)
-    emit_exchange<D, EMIT>(a, x, cnt > 0 && live, pe, beta, rho, ux, uy, uz, vx, vy, vz, rx, ry, rz);
+    emit_exchange<D, EMIT>(a, x, cnt > 0 && live && j >= a.sl.own_lo && j < a.sl.own_hi, pe, beta, rho, ux, uy, uz, vx,
+                           vy, vz, rx, ry, rz);
 }
 
 // ---------------------------------------------------------------------------
@@ -264,8 +267,8 @@ __global__ void init_rest_kernel(double *__restrict__ f, int64_t N) {
 // pull (post-collision, A-B scheme), AA natural or AA swapped.
 // ---------------------------------------------------------------------------
 template <int D>
-__device__ __forceinline__ void gather_node(const double *__restrict__ fst, const Geom &g, int layout, int i, int j,
-                                            int k, double *f) {
+__device__ __forceinline__ void gather_node(const double *__restrict__ fst, const Geom &g, const SlabRows &sl, int layout,
+                                            int i, int j, int k, double *f) {
   using L = Lat<D>;
   const int64_t x = ((int64_t)k * g.ny + j) * g.nx + i;
   if (layout == kLayoutNatural) {
@@ -284,7 +287,7 @@ __device__ __forceinline__ void gather_node(const double *__restrict__ fst, cons
       else is = is < 0 ? is + g.nx : is - g.nx;
     }
     if (js < 0 || js >= g.ny) {
-      if (g.bcy) bounce = true;
+      if (js < 0 ? sl.wall_lo : sl.wall_hi) bounce = true;
       else js = js < 0 ? js + g.ny : js - g.ny;
     }
     if (D == 3 && (ks < 0 || ks >= g.nz)) {
@@ -301,7 +304,8 @@ __device__ __forceinline__ void gather_node(const double *__restrict__ fst, cons
 
 // set_distributions: inverse permutation.  f*_q(x) = f_q(x + c_q), or f_{-q}(x) when x + c_q is behind a wall.
 template <int D>
-__global__ void unstream_kernel(const double *__restrict__ fpre, double *__restrict__ fpost, const Geom g) {
+__global__ void unstream_kernel(const double *__restrict__ fpre, double *__restrict__ fpost, const Geom g,
+                                const SlabRows sl) {
   using L = Lat<D>;
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t x = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; x < g.N; x += stride) {
@@ -319,7 +323,7 @@ __global__ void unstream_kernel(const double *__restrict__ fpre, double *__restr
         else it = it < 0 ? it + g.nx : it - g.nx;
       }
       if (jt < 0 || jt >= g.ny) {
-        if (g.bcy) bounce = true;
+        if (jt < 0 ? sl.wall_lo : sl.wall_hi) bounce = true;
         else jt = jt < 0 ? jt + g.ny : jt - g.ny;
       }
       if (D == 3 && (kt < 0 || kt >= g.nz)) {
@@ -346,7 +350,7 @@ struct FetchArgs {
 };
 
 template <int D>
-__global__ void fetch_kernel(const FetchArgs a, const Geom g) {
+__global__ void fetch_kernel(const FetchArgs a, const Geom g, const SlabRows sl) {
   using L = Lat<D>;
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; b < a.box; b += stride) {
@@ -365,7 +369,7 @@ __global__ void fetch_kernel(const FetchArgs a, const Geom g) {
       for (int c = 0; c < D; ++c) ((double *)a.dst)[(int64_t)c * a.box + b] = cov ? a.s[x * exchange_stride(D) + c] : 0.0;
     } else {
       double f[L::Q];
-      gather_node<D>(a.fpost, g, a.layout, i, j, k, f);
+      gather_node<D>(a.fpost, g, sl, a.layout, i, j, k, f);
       if (a.what == LBMIMB_FIELD_F) {
 #pragma unroll
         for (int q = 0; q < L::Q; ++q) ((double *)a.dst)[(int64_t)q * a.box + b] = f[q];
@@ -413,8 +417,9 @@ __device__ __forceinline__ double diag_block_sum(double v, double *sh) {
 
 template <int D>
 __global__ void __launch_bounds__(kDiagThreads) diag_nodes_kernel(const double *__restrict__ fst, const uint32_t *__restrict__ tag,
-                                                                  const Geom g, int layout, int have_particles,
-                                                                  double eps_den, double *__restrict__ partial) {
+                                                                  const Geom g, const SlabRows sl, int layout,
+                                                                  int have_particles, double eps_den,
+                                                                  double *__restrict__ partial) {
   using L = Lat<D>;
   __shared__ double sh[kDiagThreads / 32];
   double acc[kDiagK];
@@ -426,8 +431,9 @@ __global__ void __launch_bounds__(kDiagThreads) diag_nodes_kernel(const double *
     const int64_t r = x / g.nx;
     const int j = (int)(r % g.ny);
     const int k = (int)(r / g.ny);
+    if (j < sl.own_lo || j >= sl.own_hi) continue;   // ghost rows of a slab belong to the neighbour
     double f[L::Q];
-    gather_node<D>(fst, g, layout, i, j, k, f);
+    gather_node<D>(fst, g, sl, layout, i, j, k, f);
     double rho = 0.0, m[3] = {0.0, 0.0, 0.0};
 #pragma unroll
     for (int q = 0; q < L::Q; ++q) {
@@ -577,6 +583,7 @@ lbmimb_status launch_collide_stream(lbmimb_lattice *h, bool emit_last) {
   a.bcx = h->g.bcx;
   a.bcy = h->g.bcy;
   a.bcz = h->g.bcz;
+  a.sl = h->sl;
   a.tiles = (unsigned)((h->g.nx + kStepThreads - 1) / kStepThreads);
   a.cp = make_collide_params(h);
   const int64_t blocks = (int64_t)a.tiles * h->g.ny * h->g.nz;
@@ -604,9 +611,9 @@ lbmimb_status launch_collide_stream(lbmimb_lattice *h, bool emit_last) {
 
 lbmimb_status launch_unstream(lbmimb_lattice *h, const double *f_pre, double *f_post) {
   if (h->g.dim == 2)
-    unstream_kernel<2><<<grid_for(h->g.N, 256), 256, 0, h->stream>>>(f_pre, f_post, h->g);
+    unstream_kernel<2><<<grid_for(h->g.N, 256), 256, 0, h->stream>>>(f_pre, f_post, h->g, h->sl);
   else
-    unstream_kernel<3><<<grid_for(h->g.N, 256), 256, 0, h->stream>>>(f_pre, f_post, h->g);
+    unstream_kernel<3><<<grid_for(h->g.N, 256), 256, 0, h->stream>>>(f_pre, f_post, h->g, h->sl);
   LBMIMB_LAUNCH_CHECK(h, "unstream_kernel");
   return LBMIMB_OK;
 }
@@ -619,7 +626,7 @@ lbmimb_status launch_fetch(lbmimb_lattice *h, int what, const int64_t lo[3], con
   a.dst = dst_dev;
   a.box = 1;
   for (int c = 0; c < 3; ++c) {
-    a.lo[c] = (int)lo[c];
+    a.lo[c] = (int)lo[c] + (c == 1 ? h->sl.own_lo : 0);   // box rows count from the first OWNED row
     a.ext[c] = (int)(hi[c] - lo[c]);
     a.box *= a.ext[c];
   }
@@ -627,9 +634,9 @@ lbmimb_status launch_fetch(lbmimb_lattice *h, int what, const int64_t lo[3], con
   a.have_particles = h->P > 0;
   a.layout = h->aa ? (h->aa_swapped ? kLayoutSwapped : kLayoutNatural) : kLayoutPull;
   if (h->g.dim == 2)
-    fetch_kernel<2><<<grid_for(a.box, 256), 256, 0, h->stream>>>(a, h->g);
+    fetch_kernel<2><<<grid_for(a.box, 256), 256, 0, h->stream>>>(a, h->g, h->sl);
   else
-    fetch_kernel<3><<<grid_for(a.box, 256), 256, 0, h->stream>>>(a, h->g);
+    fetch_kernel<3><<<grid_for(a.box, 256), 256, 0, h->stream>>>(a, h->g, h->sl);
   LBMIMB_LAUNCH_CHECK(h, "fetch_kernel");
   return LBMIMB_OK;
 }
@@ -640,17 +647,62 @@ lbmimb_status launch_diagnostics(lbmimb_lattice *h, double eps_den) {
   const double *fst = h->f[h->cur];
   const int hp = h->P > 0;
   if (h->g.dim == 2) {
-    diag_nodes_kernel<2><<<nb, kDiagThreads, 0, h->stream>>>(fst, h->tag, h->g, layout, hp, eps_den, h->diag_partial);
+    diag_nodes_kernel<2><<<nb, kDiagThreads, 0, h->stream>>>(fst, h->tag, h->g, h->sl, layout, hp, eps_den, h->diag_partial);
     LBMIMB_LAUNCH_CHECK(h, "diag_nodes_kernel");
     diag_final_kernel<2><<<1, kDiagThreads, 0, h->stream>>>(h->diag_partial, nb, h->P, h->vel, h->radius, h->mass,
                                                            h->force, h->diag_out);
   } else {
-    diag_nodes_kernel<3><<<nb, kDiagThreads, 0, h->stream>>>(fst, h->tag, h->g, layout, hp, eps_den, h->diag_partial);
+    diag_nodes_kernel<3><<<nb, kDiagThreads, 0, h->stream>>>(fst, h->tag, h->g, h->sl, layout, hp, eps_den, h->diag_partial);
     LBMIMB_LAUNCH_CHECK(h, "diag_nodes_kernel");
     diag_final_kernel<3><<<1, kDiagThreads, 0, h->stream>>>(h->diag_partial, nb, h->P, h->vel, h->radius, h->mass,
                                                            h->force, h->diag_out);
   }
   LBMIMB_LAUNCH_CHECK(h, "diag_final_kernel");
+  return LBMIMB_OK;
+}
+
+// ---------------------------------------------------------------------------
+// Slab halo ("domain decomposition"; Fig. 2): after a step the stored array holds the
+// post-collision state f*(x, t).  The next step of the neighbouring slab pulls, into its first / last owned
+// row, the populations that move across the cut: the c_y = +1 ones of our LAST owned row, the c_y = -1 ones
+// of our FIRST owned row (5 of 19 / 3 of 9).  pack copies them into a contiguous buffer [n_face][nz][nx];
+// unpack writes a neighbour's buffer into our ghost row.  side 0 = lower (y-) end, 1 = upper (y+) end:
+//   pack(side)   packs the populations LEAVING through that side (c_y = -1 for side 0, +1 for side 1);
+//   unpack(side) stores populations ENTERING through that side (c_y = +1 for side 0, -1 for side 1) in the
+//                ghost row of that side.
+// Transport (peer copy, NCCL send/recv, MPI) is the caller's.
+// ---------------------------------------------------------------------------
+template <int D>
+__global__ void halo_kernel(double *__restrict__ f, double *__restrict__ buf, const Geom g, int row, int want_cy,
+                            int pack) {
+  using L = Lat<D>;
+  const int64_t plane = (int64_t)g.nx * g.nz;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < plane; e += stride) {
+    const int i = (int)(e % g.nx), k = (int)(e / g.nx);
+    const int64_t x = ((int64_t)k * g.ny + row) * g.nx + i;
+    int slot = 0;
+#pragma unroll
+    for (int q = 0; q < L::Q; ++q) {
+      if (L::cy(q) != want_cy) continue;
+      if (pack) buf[(int64_t)slot * plane + e] = f[(int64_t)q * g.N + x];
+      else f[(int64_t)q * g.N + x] = buf[(int64_t)slot * plane + e];
+      ++slot;
+    }
+  }
+}
+
+int64_t halo_doubles(const lbmimb_lattice *h) { return (int64_t)(h->g.dim == 2 ? 3 : 5) * h->g.nx * h->g.nz; }
+
+lbmimb_status launch_halo(lbmimb_lattice *h, int side, double *buf_dev, bool pack) {
+  // pack: first / last owned row; unpack: the ghost row beyond it
+  const int row = pack ? (side == 0 ? h->sl.own_lo : h->sl.own_hi - 1) : (side == 0 ? h->sl.own_lo - 1 : h->sl.own_hi);
+  const int want_cy = pack ? (side == 0 ? -1 : 1) : (side == 0 ? 1 : -1);
+  double *f = h->f[h->cur];
+  const int nb = grid_for((int64_t)h->g.nx * h->g.nz, 256);
+  if (h->g.dim == 2) halo_kernel<2><<<nb, 256, 0, h->stream>>>(f, buf_dev, h->g, row, want_cy, pack ? 1 : 0);
+  else halo_kernel<3><<<nb, 256, 0, h->stream>>>(f, buf_dev, h->g, row, want_cy, pack ? 1 : 0);
+  LBMIMB_LAUNCH_CHECK(h, "halo_kernel");
   return LBMIMB_OK;
 }
 

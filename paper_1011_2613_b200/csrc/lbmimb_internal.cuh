@@ -86,6 +86,35 @@ struct Geom {
   int64_t N;        // nx*ny*nz
 };
 
+// Slab decomposition along y (include/lbmimb.h "Slabs").  A slab lattice stores its owned rows
+// plus one ghost row on every side that is not a wall of the global lattice.  Two geometries describe it:
+//   the STORED lattice (lbmimb_lattice::g): ny = stored rows; what the lattice kernels index;
+//   the GLOBAL lattice (lbmimb_lattice::gp): ny = rows of the whole lattice; what the particle-side
+//   kernels compute in (particle coordinates are global, so every inside test, minimum image and
+//   contact is the same arithmetic as on the undivided lattice).
+// SlabRows connects them: stored row jl <-> global row jg = jl + oy (mod gny).
+struct SlabRows {
+  int ny_stored;      // rows in memory (owned + ghosts)
+  int gny;            // rows of the global lattice
+  int oy;             // global row of stored row 0 (-1 for the lower ghost of the first periodic slab)
+  int own_lo, own_hi; // stored rows [own_lo, own_hi) are owned; the others are ghosts
+  int wall_lo, wall_hi;  // is the lower / upper end of the STORED lattice a wall (else: ghost row or periodic wrap)
+};
+
+__host__ __device__ __forceinline__ int slab_global_row(const SlabRows &s, int jl) {
+  int jg = jl + s.oy;
+  if (jg < 0) jg += s.gny;
+  else if (jg >= s.gny) jg -= s.gny;
+  return jg;
+}
+// stored row of global row jg, or -1 if this slab does not store it
+__host__ __device__ __forceinline__ int slab_stored_row(const SlabRows &s, int jg) {
+  int jl = jg - s.oy;
+  if (jl < 0) jl += s.gny;
+  else if (jl >= s.gny) jl -= s.gny;
+  return jl < s.ny_stored ? jl : -1;
+}
+
 // Cell list over the particles (mapping fix-up pass and DEM contacts).
 struct CellList {
   int ncx, ncy, ncz;     // cells per axis
@@ -137,7 +166,10 @@ struct CoupledGraph {
 
 struct lbmimb_lattice {
   lbmimb_params prm;
-  lbmimb::Geom g;
+  lbmimb::Geom g;      // the STORED lattice (ny = owned rows + ghost rows)
+  lbmimb::Geom gp;     // the GLOBAL lattice the particles live in (= g unless this is a slab)
+  lbmimb::SlabRows sl;
+  bool is_slab;
   int Q;
   int SD;            // S^dim
   cudaStream_t stream;
@@ -218,11 +250,14 @@ lbmimb_status launch_map(lbmimb_lattice *h);
 lbmimb_status ensure_eps_table(lbmimb_lattice *h);
 int64_t eps_table_entries(int dim);
 lbmimb_status launch_finish_forces(lbmimb_lattice *h);   // facc -> force / torque, clears facc
-lbmimb_status launch_dem(lbmimb_lattice *h, const lbmimb_dem_params *dem);
+lbmimb_status launch_dem(lbmimb_lattice *h, const lbmimb_dem_params *dem, bool finish);
+bool dem_small_path(const lbmimb_lattice *h);
 lbmimb_status neighbor_list_prepare(lbmimb_lattice *h);   // (re)allocates the list storage for the current radii
 void neighbor_list_release(lbmimb_lattice *h);
 lbmimb_status neighbor_list_invalidate(lbmimb_lattice *h);  // positions were replaced
 lbmimb_status launch_diagnostics(lbmimb_lattice *h, double eps_den);
+lbmimb_status launch_halo(lbmimb_lattice *h, int side, double *buf_dev, bool pack);
+int64_t halo_doubles(const lbmimb_lattice *h);
 constexpr int kDiagBlocksMax = 148 * 8;
 
 }  // namespace lbmimb

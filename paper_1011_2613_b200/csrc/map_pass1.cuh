@@ -254,7 +254,9 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
     pend_x = -1;
   };
   auto commit = [&](int i, int j, int k, int cnt) {
-    const int64_t x = ((int64_t)k * a.g.ny + j) * a.g.nx + i;
+    const int jl = slab_stored_row(a.sl, j);   // (a slab stores only some rows of the global lattice)
+    if (jl < 0) return;
+    const int64_t x = ((int64_t)k * a.sl.ny_stored + jl) * a.g.nx + i;
     settle();
     pend_old = atomicExch(a.tag + x, make_tag((int32_t)p, cnt));
     pend_x = x;
@@ -271,7 +273,7 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
       if (D == 3 && wz) dz = min_image_d(dz, a.g.nz);
       const double ny_ = fmax(fabs(dy) - hs, 0.0), nz_ = D == 3 ? fmax(fabs(dz) - hs, 0.0) : 0.0;
       const double rad = r2_none - ny_ * ny_ - nz_ * nz_;
-      if (rad > -1e-9) {
+      if (rad > -1e-9 && slab_stored_row(a.sl, j) >= 0) {
         if (wx) {
           len = ext[0];
         } else {

@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(128) map_table_kernel(const MapArgs a, const T
       if (wy) dy = min_image_d(dy, a.g.ny);
       if (D == 3 && wz) dz = min_image_d(dz, a.g.nz);
       const double rad = t.none2 - dy * dy - dz * dz;
-      if (rad > -1e-9) {
+      if (rad > -1e-9 && slab_stored_row(a.sl, j) >= 0) {
         if (wx) len = ext[0];
         else clip_interval(cx, sqrt(fmax(rad, 0.0) + 1e-9) + 1e-9, lo[0], ext[0], b0, len);
       }
@@ -184,7 +184,7 @@ __global__ void __launch_bounds__(128) map_table_kernel(const MapArgs a, const T
       if (D == 3 && wz) dz = min_image_d(dz, a.g.nz);
       const int code = table_code<D>(t, dx, dy, dz);
       if (code > 0) {
-        const int64_t x = ((int64_t)k * a.g.ny + j) * a.g.nx + i;
+        const int64_t x = ((int64_t)k * a.sl.ny_stored + slab_stored_row(a.sl, j)) * a.g.nx + i;
         settle();
         pend_old = atomicExch(a.tag + x, make_tag((int32_t)p, code));
         pend_x = x;
@@ -218,7 +218,7 @@ __global__ void __launch_bounds__(128) map_table_contested_kernel(const MapArgs 
     const int64_t x = a.contested[e];
     const int i = (int)(x % a.g.nx);
     const int64_t r = x / a.g.nx;
-    const int j = (int)(r % a.g.ny), k = (int)(r / a.g.ny);
+    const int j = slab_global_row(a.sl, (int)(r % a.sl.ny_stored)), k = (int)(r / a.sl.ny_stored);
     int b = 0, en = 0;
     if (cell_lane) {
       int cx_ = cell_coord((double)i, cg, 0) + ox, cy_ = cell_coord((double)j, cg, 1) + oy;

@@ -93,7 +93,7 @@ lbmimb_status validate_particles_dev(lbmimb_lattice *h, int64_t P, const double 
   int32_t *res = h->counters + 8;   // words 8..13 of the 16-word counter block
   const unsigned long long init[3] = {0ull, 0ull, ~0ull};
   LBMIMB_CUDA(cudaMemcpyAsync(res, init, sizeof(init), cudaMemcpyHostToDevice, h->stream));
-  validate_particles_kernel<<<blocks_for(P, 256), 256, 0, h->stream>>>(h->g.dim, P, h->g.nx, h->g.ny, h->g.nz, pos_dev,
+  validate_particles_kernel<<<blocks_for(P, 256), 256, 0, h->stream>>>(h->gp.dim, P, h->gp.nx, h->gp.ny, h->gp.nz, pos_dev,
                                                                        radius_dev, mass_dev, res);
   LBMIMB_LAUNCH_CHECK(h, "validate_particles_kernel");
   unsigned long long out[3];
@@ -260,9 +260,9 @@ static CellGeom cell_geom(const lbmimb_lattice *h) {
   cg.inv_e[0] = h->cl.inv_ex;
   cg.inv_e[1] = h->cl.inv_ey;
   cg.inv_e[2] = h->cl.inv_ez;
-  cg.periodic[0] = !h->g.bcx;
-  cg.periodic[1] = !h->g.bcy;
-  cg.periodic[2] = !h->g.bcz;
+  cg.periodic[0] = !h->gp.bcx;
+  cg.periodic[1] = !h->gp.bcy;
+  cg.periodic[2] = !h->gp.bcz;
   return cg;
 }
 
@@ -270,7 +270,7 @@ lbmimb_status build_cell_list(lbmimb_lattice *h) {
   double edge = 2.0 * h->rmax;
   if (edge < h->rmax + 1.0) edge = h->rmax + 1.0;
   if (edge < 2.0) edge = 2.0;
-  int n[3] = {h->g.nx, h->g.ny, h->g.nz};
+  int n[3] = {h->gp.nx, h->gp.ny, h->gp.nz};
   int nc[3] = {1, 1, 1};
   double inv_e[3] = {1.0, 1.0, 1.0};
   for (int a = 0; a < h->g.dim; ++a) {
@@ -313,7 +313,8 @@ lbmimb_status build_cell_list(lbmimb_lattice *h) {
 // definition (include/lbmimb.h a1): every operation is a separate IEEE op, no FMA.
 // ---------------------------------------------------------------------------
 struct MapArgs {
-  Geom g;
+  Geom g;              // the GLOBAL lattice (particle coordinates are global)
+  SlabRows sl;         // which of its rows this handle stores
   int S, SD;
   int64_t P;
   const double *pos;
@@ -429,7 +430,7 @@ __global__ void __launch_bounds__(128) map_contested_kernel(const MapArgs a, con
     const int64_t x = a.contested[e];
     const int i = (int)(x % a.g.nx);
     const int64_t r = x / a.g.nx;
-    const int j = (int)(r % a.g.ny), k = (int)(r / a.g.ny);
+    const int j = slab_global_row(a.sl, (int)(r % a.sl.ny_stored)), k = (int)(r / a.sl.ny_stored);
     int b = 0, en = 0;
     if (cell_lane) {
       int cx_ = cell_coord((double)i, cg, 0) + ox, cy_ = cell_coord((double)j, cg, 1) + oy;
@@ -574,10 +575,11 @@ static lbmimb_status launch_map_table(lbmimb_lattice *h, const MapArgs &a) {
 lbmimb_status launch_map(lbmimb_lattice *h) {
   lbmimb_status st;
   if (!h->cl_valid && (st = build_cell_list(h)) != LBMIMB_OK) return st;
-  LBMIMB_CUDA(cudaMemsetAsync(h->tag, 0, (size_t)h->g.N * 4, h->stream));
-  LBMIMB_CUDA(cudaMemsetAsync(h->counters, 0, 8, h->stream));   // shared-node count and its overflow flag
+  // one memset: the tags and, directly behind them in the workspace, the shared-node count and its overflow flag
+  LBMIMB_CUDA(cudaMemsetAsync(h->tag, 0, (size_t)((char *)(h->counters + 16) - (char *)h->tag), h->stream));
   MapArgs a;
-  a.g = h->g;
+  a.g = h->gp;
+  a.sl = h->sl;
   a.S = h->prm.subsamples;
   a.SD = h->SD;
   a.P = h->P;
@@ -719,10 +721,9 @@ __device__ __forceinline__ void wall_force(const DemArgs &a, const int *n, const
   }
 }
 
+// contact force on particle i: the particles of the 3^D cells around it (ascending index inside a cell), then the walls
 template <int D>
-__global__ void dem_contact_kernel(const DemArgs a) {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= a.P) return;
+__device__ __forceinline__ void dem_contact_one(const DemArgs &a, int64_t i) {
   const int n[3] = {a.g.nx, a.g.ny, a.g.nz};
   double xi[3], vi[3], F[3] = {0.0, 0.0, 0.0};
   for (int c = 0; c < D; ++c) {
@@ -754,6 +755,12 @@ __global__ void dem_contact_kernel(const DemArgs a) {
       }
   wall_force<D>(a, n, xi, vi, Ri, mi, F);
   for (int q = 0; q < D; ++q) a.fc[(int64_t)q * a.P + i] = F[q];
+}
+
+template <int D>
+__global__ void dem_contact_kernel(const DemArgs a) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < a.P) dem_contact_one<D>(a, i);
 }
 
 // the same sums over the neighbour lists (ascending j).  Runs right after the three predicated
@@ -788,9 +795,7 @@ __global__ void dem_contact_list_kernel(const DemArgs a) {
 // the displacement flag of the rebuild rule when this particle is now farther than skin/2 from
 // where it was when the lists were built.
 template <int D>
-__global__ void dem_kick_drift_kernel(const DemArgs a) {
-  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= a.P) return;
+__device__ __forceinline__ void dem_kick_drift_one(const DemArgs &a, int64_t p) {
   const int n[3] = {a.g.nx, a.g.ny, a.g.nz};
   const bool per[3] = {!a.g.bcx, !a.g.bcy, !a.g.bcz};
   const double m = a.mass[p];
@@ -811,12 +816,15 @@ __global__ void dem_kick_drift_kernel(const DemArgs a) {
   if (a.nl_state != nullptr && verlet_disp2<D>(xn, a.nl_xref, a.nl_Pcap, p, n, per) > a.nl_h2) a.nl_state[NL_DISP] = 1;
 }
 
+template <int D>
+__global__ void dem_kick_drift_kernel(const DemArgs a) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p < a.P) dem_kick_drift_one<D>(a, p);
+}
+
 // second half: v += dt/2 a1; omega += dt T_h / I.  Verlet mode: the lists age by one step.
 template <int D>
-__global__ void dem_kick_kernel(const DemArgs a) {
-  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (p == 0 && a.nl_state != nullptr) a.nl_state[NL_AGE] += 1;
-  if (p >= a.P) return;
+__device__ __forceinline__ void dem_kick_one(const DemArgs &a, int64_t p) {
   const double m = a.mass[p], R = a.radius[p];
   for (int q = 0; q < D; ++q) {
     const int64_t id = (int64_t)q * a.P + p;
@@ -828,6 +836,154 @@ __global__ void dem_kick_kernel(const DemArgs a) {
   for (int q = 0; q < nt; ++q) {
     const int64_t id = (int64_t)q * a.P + p;
     a.omega[id] = a.omega[id] + a.dt * a.torque[id] / I;
+  }
+}
+
+template <int D>
+__global__ void dem_kick_kernel(const DemArgs a) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p == 0 && a.nl_state != nullptr) a.nl_state[NL_AGE] += 1;
+  if (p < a.P) dem_kick_one<D>(a, p);
+}
+
+// ---------------------------------------------------------------------------
+// Small particle sets (P <= kDemSmallP, cell mode): the whole DEM step as ONE single-block kernel.  A coupled
+// step of C5 (4,096 spheres) used to spend 10 dependent launches of 3-6 microseconds each on it (contact,
+// kick+drift, a counting-sort cell list of 2 memsets + 6 kernels, contact, kick, record packing) plus the
+// force conversion of a3; block barriers replace the launch boundaries, global memory is the only storage
+// (coherent inside a block after __syncthreads), and every per-particle / per-cell routine is the one the
+// multi-kernel path runs, in the same order: results are bit for bit the same.
+//   FINISH: first turn the fixed-point force sums of the fused step into force / torque (a3's last part).
+// Leaves a cell list of the NEW positions behind (the map of the next step uses it) and the packed records.
+// ---------------------------------------------------------------------------
+constexpr int kDemSmallP = 8192;
+constexpr int kDemSmallCells = 1024 * 64;
+constexpr int kDemSmallThreads = 1024;
+
+struct DemSmallArgs {
+  CellGeom cg_new;     // cell geometry for the list of the new positions (= the old one: same radii)
+  int64_t ncells;
+  int32_t *count, *start, *fill, *items, *cell_of;
+  long long *facc;
+  double *force_w, *torque_w;   // writable views of force / torque (FINISH)
+  double *prec;
+  int dim;
+};
+
+template <int D, bool FINISH>
+__global__ void __launch_bounds__(kDemSmallThreads) dem_small_kernel(const DemArgs a, const DemSmallArgs b) {
+  __shared__ int32_t wsum[kDemSmallThreads / 32];
+  __shared__ int32_t carry_s;
+  const int tid = threadIdx.x;
+  const int64_t P = a.P;
+  if (FINISH) {   // same thread -> same particles in every phase below: no barrier needed before the kicks
+    constexpr int NV = D == 2 ? 3 : 6;
+    for (int64_t p = tid; p < P; p += kDemSmallThreads) {
+      longlong2 *acc = reinterpret_cast<longlong2 *>(b.facc + p * (2 * NV));
+      double v[NV];
+#pragma unroll
+      for (int c = 0; c < NV; ++c) {
+        const longlong2 w = acc[c];
+        v[c] = fixed_value(w.x, w.y);
+        acc[c] = make_longlong2(0, 0);
+      }
+#pragma unroll
+      for (int c = 0; c < D; ++c) b.force_w[(int64_t)c * P + p] = v[c];
+      if (D == 2) {
+        b.torque_w[p] = v[2];
+      } else {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) b.torque_w[(int64_t)c * P + p] = v[3 + c];
+      }
+    }
+  }
+  for (int64_t i = tid; i < P; i += kDemSmallThreads) dem_contact_one<D>(a, i);
+  __syncthreads();   // every contact sum read the OLD positions and velocities
+  for (int64_t p = tid; p < P; p += kDemSmallThreads) dem_kick_drift_one<D>(a, p);
+  for (int64_t c = tid; c <= b.ncells; c += kDemSmallThreads) b.count[c] = 0;
+  for (int64_t c = tid; c < b.ncells; c += kDemSmallThreads) b.fill[c] = 0;
+  __syncthreads();
+  // ---- cell list of the new positions: count, exclusive scan, fill, sort (as build_cell_list)
+  for (int64_t p = tid; p < P; p += kDemSmallThreads) {
+    const int cx = cell_coord(a.pos[p], b.cg_new, 0);
+    const int cy = cell_coord(a.pos[P + p], b.cg_new, 1);
+    const int cz = D == 3 ? cell_coord(a.pos[2 * P + p], b.cg_new, 2) : 0;
+    const int c = (cz * b.cg_new.nc[1] + cy) * b.cg_new.nc[0] + cx;
+    b.cell_of[p] = c;
+    atomicAdd(b.count + c, 1);
+  }
+  if (tid == 0) carry_s = 0;
+  __syncthreads();
+  {
+    const int64_t n1 = b.ncells + 1;
+    const int per = (int)((n1 + kDemSmallThreads - 1) / kDemSmallThreads);
+    const int64_t lo = (int64_t)tid * per;
+    int32_t tot = 0;
+    for (int e = 0; e < per; ++e)
+      if (lo + e < n1) tot += b.count[lo + e];
+    int32_t incl = tot;
+    const int lane = tid & 31, wid = tid >> 5;
+    for (int o = 1; o < 32; o <<= 1) {
+      const int32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += t;
+    }
+    if (lane == 31) wsum[wid] = incl;
+    __syncthreads();
+    int32_t woff = 0;
+    for (int w = 0; w < wid; ++w) woff += wsum[w];
+    int32_t run = woff + incl - tot;
+    for (int e = 0; e < per; ++e)
+      if (lo + e < n1) {
+        b.start[lo + e] = run;
+        run += b.count[lo + e];
+      }
+  }
+  __syncthreads();
+  for (int64_t p = tid; p < P; p += kDemSmallThreads) {
+    const int c = b.cell_of[p];
+    const int slot = atomicAdd(b.fill + c, 1);
+    b.items[b.start[c] + slot] = (int32_t)p;
+  }
+  __syncthreads();
+  for (int64_t c = tid; c < b.ncells; c += kDemSmallThreads) {
+    const int bg = b.start[c], en = b.start[c + 1];
+    for (int q0 = bg + 1; q0 < en; ++q0) {
+      const int32_t v = b.items[q0];
+      int q = q0 - 1;
+      while (q >= bg && b.items[q] > v) {
+        b.items[q + 1] = b.items[q];
+        --q;
+      }
+      b.items[q + 1] = v;
+    }
+  }
+  __syncthreads();
+  DemArgs a2 = a;
+  a2.cg = b.cg_new;
+  for (int64_t i = tid; i < P; i += kDemSmallThreads) dem_contact_one<D>(a2, i);
+  __syncthreads();   // the kicks below change velocities the contact sums above read
+  for (int64_t p = tid; p < P; p += kDemSmallThreads) {
+    dem_kick_one<D>(a, p);
+    double *r = b.prec + p * prec_stride(D);
+    if (D == 2) {
+      r[0] = a.pos[p];
+      r[1] = a.pos[P + p];
+      r[2] = a.vel[p];
+      r[3] = a.vel[P + p];
+      r[4] = a.omega[p];
+      r[5] = a.radius[p];
+    } else {
+      r[0] = a.pos[p];
+      r[1] = a.pos[P + p];
+      r[2] = a.pos[2 * P + p];
+      r[3] = a.vel[p];
+      r[4] = a.vel[P + p];
+      r[5] = a.vel[2 * P + p];
+      r[6] = a.omega[p];
+      r[7] = a.omega[P + p];
+      r[8] = a.omega[2 * P + p];
+      r[9] = a.radius[p];
+    }
   }
 }
 
@@ -853,7 +1009,7 @@ lbmimb_status neighbor_list_prepare(lbmimb_lattice *h) {
   if (nl.mem && nl.rmax == h->rmax && nl.rmin == h->rmin) return LBMIMB_OK;
   neighbor_list_release(h);
   const int D = h->g.dim;
-  const int n[3] = {h->g.nx, h->g.ny, h->g.nz};
+  const int n[3] = {h->gp.nx, h->gp.ny, h->gp.nz};
   const double cutoff = (2.0 * h->rmax + nl.skin) * (1.0 + 1e-9);  // margin: cell binning is rounded
   const double dmin = 1.5 * h->rmin;  // closest centres the sizing allows for (soft spheres overlap)
   double edge_max = 0.0;
@@ -906,15 +1062,15 @@ lbmimb_status neighbor_list_prepare(lbmimb_lattice *h) {
 static VerletArgs verlet_args(const lbmimb_lattice *h) {
   const NeighborList &nl = h->nl;
   VerletArgs v;
-  v.g = h->g;
+  v.g = h->gp;
   v.cg.dim = h->g.dim;
   for (int a = 0; a < 3; ++a) {
     v.cg.nc[a] = nl.nc[a];
     v.cg.inv_e[a] = nl.inv_e[a];
   }
-  v.cg.periodic[0] = !h->g.bcx;
-  v.cg.periodic[1] = !h->g.bcy;
-  v.cg.periodic[2] = !h->g.bcz;
+  v.cg.periodic[0] = !h->gp.bcx;
+  v.cg.periodic[1] = !h->gp.bcy;
+  v.cg.periodic[2] = !h->gp.bcz;
   v.P = h->P;
   v.Pcap = nl.Pcap;
   v.ncells = nl.ncells;
@@ -947,8 +1103,24 @@ static lbmimb_status verlet_ensure(lbmimb_lattice *h, const VerletArgs &v) {
   return LBMIMB_OK;
 }
 
+// can this handle's DEM step run as the single-block kernel (which can also do a3's conversion)?
+bool dem_small_path(const lbmimb_lattice *h) {
+  if (h->nl.mode == LBMIMB_NEIGHBOR_VERLET || h->P > kDemSmallP) return false;
+  // same geometry rule as build_cell_list
+  double edge = 2.0 * h->rmax;
+  if (edge < h->rmax + 1.0) edge = h->rmax + 1.0;
+  if (edge < 2.0) edge = 2.0;
+  const int n[3] = {h->gp.nx, h->gp.ny, h->gp.nz};
+  int64_t nc = 1;
+  for (int a = 0; a < h->g.dim; ++a) {
+    int c = (int)floor((double)n[a] / edge);
+    nc *= c < 1 ? 1 : c;
+  }
+  return nc + 1 <= kDemSmallCells;
+}
+
 template <int D>
-static lbmimb_status dem_impl(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
+static lbmimb_status dem_impl(lbmimb_lattice *h, const lbmimb_dem_params *dem, bool finish) {
   lbmimb_status st;
   const bool verlet = h->nl.mode == LBMIMB_NEIGHBOR_VERLET;
   if (verlet) {
@@ -957,7 +1129,7 @@ static lbmimb_status dem_impl(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
     return st;
   }
   DemArgs a;
-  a.g = h->g;
+  a.g = h->gp;
   a.P = h->P;
   a.pos = h->pos;
   a.vel = h->vel;
@@ -1005,6 +1177,26 @@ static lbmimb_status dem_impl(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
     h->cl_valid = false;   // the particles moved and no cell list was built at the new positions
     return LBMIMB_OK;
   }
+  if (dem_small_path(h)) {
+    DemSmallArgs b;
+    b.cg_new = a.cg;
+    b.ncells = h->cl.ncells;
+    b.count = h->cl.count;
+    b.start = h->cl.start;
+    b.fill = h->cl.fill;
+    b.items = h->cl.items;
+    b.cell_of = h->cl.cell_of;
+    b.facc = h->facc;
+    b.force_w = h->force;
+    b.torque_w = h->torque;
+    b.prec = h->prec;
+    b.dim = D;
+    if (finish) dem_small_kernel<D, true><<<1, kDemSmallThreads, 0, h->stream>>>(a, b);
+    else dem_small_kernel<D, false><<<1, kDemSmallThreads, 0, h->stream>>>(a, b);
+    LBMIMB_LAUNCH_CHECK(h, "dem_small_kernel");
+    return LBMIMB_OK;   // cell list of the new positions and packed records are in place
+  }
+  if (finish) return fail(LBMIMB_EINVAL, "internal: force conversion can only be folded into the single-block DEM step");
   dem_contact_kernel<D><<<nb, 128, 0, h->stream>>>(a);
   LBMIMB_LAUNCH_CHECK(h, "dem_contact_kernel");
   dem_kick_drift_kernel<D><<<nb, 128, 0, h->stream>>>(a);
@@ -1018,8 +1210,10 @@ static lbmimb_status dem_impl(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
   return LBMIMB_OK;
 }
 
-lbmimb_status launch_dem(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
-  return h->g.dim == 2 ? dem_impl<2>(h, dem) : dem_impl<3>(h, dem);
+// finish: also convert the fixed-point force sums of the last step (only with dem_small_path(h)).
+// On return the packed records are current if dem_small_path(h), else the caller packs them.
+lbmimb_status launch_dem(lbmimb_lattice *h, const lbmimb_dem_params *dem, bool finish) {
+  return h->g.dim == 2 ? dem_impl<2>(h, dem, finish) : dem_impl<3>(h, dem, finish);
 }
 
 }  // namespace lbmimb

@@ -1,0 +1,131 @@
+"""NEXT-4 (Fig. 2): the lattice cut into y-slabs, each its own handle, halo rows and
+per-slab force sums exchanged through the C-ABI (include/lbmimb.h "Slabs").  `-m gpu`, ONE GPU: the slabs are
+separate handles on the same device and the transport is a device-to-device copy (paper_1011_2613_b200.slabs.LocalSlabs);
+the inter-rank schedule is covered on CPU by tests/test_slabs_gloo.py.  Reference: the CPU oracle on the UNDIVIDED
+lattice, usual tolerances; plus bitwise equality with the undivided CUDA lattice (the decomposition changes no
+arithmetic and the force sums are order-free integers)."""
+import numpy as np
+import pytest
+
+from paper_1011_2613_b200 import inputs, slabs
+from parity_util import assert_fields_close, assert_forces_close, force_floor, gpu_run, oracle_run
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lb():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1011_2613_b200 import binding
+    binding.load()
+    return binding
+
+
+def _slabs_for(lb, w, nslabs, bc=None):
+    s = slabs.LocalSlabs(lb, w.dim, w.n, bc or w.bc, w.tau, w.g_fluid, w.subsamples, nslabs, max_particles=w.P)
+    s.set_particles(w.pos, w.vel, w.omega, w.radius, w.mass)
+    return s
+
+
+@pytest.mark.parametrize("name,nslabs,periodic_y", [("C3", 2, False), ("C3", 3, False), ("C2", 3, False), ("C4", 2, False),
+                                                    ("P3D", 2, True), ("P3D", 1, True), ("P2D", 4, True)])
+def test_fixed_particles_slabs_against_the_undivided_lattice(orc, lb, name, nslabs, periodic_y):
+    """Reduced cuts (particles cut by the slab faces, walls or a periodic seam in y): maps bit-exact, f <= 1e-12 and
+    forces <= 1e-10 against the oracle; everything bitwise equal to the undivided CUDA lattice."""
+    w = inputs.reduced(name)
+    rng = np.random.default_rng(11)
+    w.omega = rng.uniform(-1e-3, 1e-3, size=w.omega.shape)
+    assert (w.bc[1] == 0) == periodic_y
+    steps = 12
+    ref = oracle_run(orc, w, steps)
+    one, got1 = gpu_run(lb, w, steps, exchange_field=False)
+    s = _slabs_for(lb, w, nslabs)
+    cut = [y0 for (y0, _) in s.parts[1:]]
+    if cut:                                       # some particle really straddles a face
+        assert any(((w.pos[1] - w.radius < c) & (w.pos[1] + w.radius > c)).any() for c in cut)
+    s.map_particles()
+    s.step(steps)
+    (F, T), every = s.reduce_particle_forces()
+    eps, pid, f = s.fetch_fields(lb.FIELD_EPS_CNT), s.fetch_fields(lb.FIELD_PID), s.fetch_fields(lb.FIELD_F)
+    assert np.array_equal(eps, ref["eps"]) and np.array_equal(pid, ref["pid"])
+    assert_fields_close(f, ref["f"])
+    assert_forces_close(F, T, ref)
+    assert np.array_equal(f, got1["f"])
+    assert np.array_equal(F, got1["force"]) and np.array_equal(T, got1["torque"])
+    for Fk, Tk in every:                          # every slab ends up with the same, complete sums
+        assert np.array_equal(Fk, F) and np.array_equal(Tk, T)
+    assert np.array_equal(s.fetch_fields(lb.FIELD_RHO), got1["rho"])
+    s.close()
+    one.close()
+
+
+@pytest.mark.parametrize("name,nslabs", [("C5", 2), ("P3D", 3)])
+def test_coupled_windows_on_slabs(orc, lb, name, nslabs):
+    """The coupled protocol (oracle.coupled_step leads, shared state at every window start) with the lattice in
+    slabs: map -> step -> halo exchange -> force sums across slabs -> reduce -> DEM on every slab."""
+    w = inputs.reduced(name)
+    d = w.dem
+    dargs = (d["kn"], d["restitution"], d["g_particle"], d["dt"])
+    f = orc.init(w.dim, w.n)
+    pos, vel, om = w.pos.copy(), w.vel.copy(), w.omega.copy()
+    s = slabs.LocalSlabs(lb, w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, nslabs, max_particles=w.P)
+    for k in range(3):
+        s.set_distributions(f)
+        s.set_particles(pos, vel, om, w.radius, w.mass)
+        for it in range(6):
+            f, pos, vel, om, ref = orc.coupled_step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, pos, vel, om,
+                                                    w.radius, w.mass, *dargs)
+            s.map_particles()
+            if it == 0:
+                assert np.array_equal(s.fetch_fields(lb.FIELD_EPS_CNT), ref["eps"])
+                assert np.array_equal(s.fetch_fields(lb.FIELD_PID), ref["pid"])
+            s.step(1)
+            (F, T), _ = s.reduce_particle_forces()
+            ref.update(floor=force_floor(ref["pid"], w.P), radius=w.radius)
+            assert_forces_close(F, T, ref)
+            s.dem_step(*dargs)
+        assert_fields_close(s.fetch_fields(lb.FIELD_F), f)
+        pg, vg, og = s.get_particles()
+        assert np.abs(pg - pos).max() < 1e-10
+        assert np.abs(vg - vel).max() <= 1e-10 * np.abs(vel).max() + 1e-18
+        for l in s.lat[1:]:                       # the replicated particles stay bit-identical on every slab
+            p2, v2, o2 = l.get_particles()
+            assert np.array_equal(p2, pg) and np.array_equal(v2, vg) and np.array_equal(o2, og)
+    s.close()
+
+
+def test_slab_diagnostics_add_up_and_errors(orc, lb):
+    w = inputs.reduced("C3")
+    s = _slabs_for(lb, w, 3)
+    s.map_particles()
+    s.step(5)
+    one, _ = gpu_run(lb, w, 5, exchange_field=False)
+    whole = one.diagnostics()
+    parts = [l.diagnostics() for l in s.lat]
+    assert abs(sum(p["mass"] for p in parts) - whole["mass"]) < 1e-9 * whole["mass"]
+    assert abs(sum(p["gas_area"] for p in parts) - whole["gas_area"]) < 1e-9 * whole["gas_area"]
+    mom = sum(p["fluid_momentum"] for p in parts)
+    assert np.abs(mom - whole["fluid_momentum"]).max() < 1e-12 * w.nodes
+    assert s.lat[0].slab_ghost_rows(0) == 0 and s.lat[0].slab_ghost_rows(1) == 1     # walls in y: no ghost at the wall
+    assert s.lat[1].slab_ghost_rows(0) == 1 and s.lat[2].slab_ghost_rows(1) == 0
+    import torch
+    buf = torch.empty(s.lat[0].halo_count(), dtype=torch.float64, device="cuda")
+    with pytest.raises(lb.LbmimbError) as ei:
+        s.lat[0].pack_halo(0, buf.data_ptr())                    # the lower end of slab 0 is a wall
+    assert ei.value.status == lb.ESTATE
+    with pytest.raises(lb.LbmimbError) as ei:
+        one.pack_halo(1, buf.data_ptr())                         # not a slab
+    assert ei.value.status == lb.ESTATE
+    d = inputs.reduced("C5").dem
+    with pytest.raises(lb.LbmimbError) as ei:
+        s.lat[1].run_coupled(2, d["kn"], d["restitution"], d["g_particle"], d["dt"])
+    assert ei.value.status == lb.ESTATE
+    with pytest.raises(lb.LbmimbError) as ei:
+        lb.Lattice(3, (16, 8, 16), (0, 0, 0), 0.8, (0, 0, 0), 4, streaming=lb.STREAM_AA, slab=(0, 16))
+    assert ei.value.status == lb.EINVAL
+    with pytest.raises(lb.LbmimbError) as ei:
+        lb.Lattice(3, (16, 8, 16), (0, 0, 0), 0.8, (0, 0, 0), 4, slab=(10, 16))      # rows 10..18 of 16
+    assert ei.value.status == lb.EINVAL
+    s.close()
+    one.close()
