@@ -49,7 +49,9 @@ def test_run_coupled_equals_the_explicit_loop(lb, name, streaming, verlet):
     loop(a, d, 9)
     b.run_coupled(9, *args)                                   # 1 plain step + 4 replays of the pair
     same_state(lb, a, b)
-    assert a.launch_count() - l0a == b.launch_count() - l0b   # the launch counter counts replayed kernels too
+    # the launch counter counts replayed kernels too; with the cell list run_coupled folds the conversion of the
+    # force sums into its DEM kernels, which saves the explicit loop's one reduce launch per step
+    assert (a.launch_count() - l0a) - (b.launch_count() - l0b) == (0 if verlet else 9)
     loop(a, d, 4)
     b.run_coupled(4, *args)                                   # starts on the other parity: second graph
     same_state(lb, a, b)

@@ -117,7 +117,7 @@ def test_paper_suspension_coupled_windows(orc, lb, name, streaming):
         lat.map_particles()
         eps, pid = orc.map_particles(w.dim, w.n, w.bc, w.subsamples, pos, w.radius)
         dg = lat.diagnostics()
-        dr = orc.diagnostics(w.dim, f, eps, w.subsamples ** w.dim, vel, w.radius, w.mass, F)
+        dr = orc.diagnostics(w.dim, f, eps, w.subsamples ** w.dim, vel, w.radius, w.mass, ref["force"])
         assert np.abs(dg["slip"] - dr["slip"]).max() <= 1e-10 * np.abs(dr["slip"]).max() + 1e-12 * np.abs(f).max()
-        assert np.abs(dg["drag"] - dr["drag"]).max() <= 1e-10 * np.abs(dr["drag"]).max() + float((1e-10 * 1e-3 * aF + ref["floor"]).mean())
+        assert np.abs(dg["drag"] - dr["drag"]).max() <= 1e-10 * np.abs(dr["drag"]).max() + float((1e-10 * 1e-3 * ref["abs_f"] + ref["floor"]).mean())
     lat.close()
