@@ -229,7 +229,7 @@ lbmimb_status lbmimb_step(lbmimb_lattice *h, int32_t nsteps);
  * eq. (3) with the sign of R6 (force ON the particle):
  *   F_p = - sum_{n: pid=p} s_n,   T_p = - sum_n (x_n - x_p) x s_n   (minimum image), h^D/dt = 1.
  * The sums were formed by the last step (runs of a particle's nodes are pre-summed per warp in a fixed tree
- * and added as 64-bit fixed-point integers, resolution 2^-92, so the result does not depend on the order
+ * and added as 64-bit fixed-point integers, resolution 2^-91, so the result does not depend on the order
  * in which thread blocks ran: bitwise reproducible); this call converts them.  force / torque may be NULL:
  * results stay on the device for dem_step; otherwise they are copied to the host and the call is synchronous.
  * ESTATE if no step has run since the last map_particles.
@@ -342,7 +342,7 @@ lbmimb_status lbmimb_pack_halo(lbmimb_lattice *h, int32_t side, double *dst_dev)
 lbmimb_status lbmimb_unpack_halo(lbmimb_lattice *h, int32_t side, const double *src_dev);
 /*
  * The per-particle force / torque sums of the last step as the integers the fused kernel accumulated:
- * lbmimb_force_sums_count(h) = P * (3 | 6) * 2 int64 words ([P][value][hi, lo], value = hi 2^-40 + lo 2^-92).
+ * lbmimb_force_sums_count(h) = P * (3 | 6) * 2 int64 words ([P][value][hi, lo], value = hi 2^-40 + lo 2^-91).
  * Adding the arrays of all slabs word by word gives the sums of the undivided lattice exactly.  export copies
  * them out, import replaces them (both asynchronous).  ESTATE unless a step has run since the last map and
  * reduce_particle_forces has not consumed the sums yet.

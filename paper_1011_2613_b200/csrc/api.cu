@@ -92,7 +92,7 @@ static SlabRows slab_rows(const lbmimb_params *p) {
 // One place that decides the device memory layout; used for sizing and for carving.
 struct Layout {
   uint64_t off_f[2], off_tag, off_s, off_facc, off_beta, off_contested, off_counters, off_table, off_diag;
-  uint64_t off_pos, off_vel, off_omega, off_radius, off_mass, off_force, off_torque, off_fc, off_prec;
+  uint64_t off_pos, off_vel, off_omega, off_radius, off_mass, off_force, off_torque, off_fc, off_prec, off_pos2, off_vel2;
   uint64_t off_count, off_start, off_fill, off_items, off_cell_of, off_bsums;
   uint64_t total;
   int64_t N, contested_cap, ncells_max;
@@ -136,6 +136,8 @@ static Layout make_layout(const lbmimb_params *p, int64_t maxp) {
   L.off_torque = take((uint64_t)3 * pm * 8);
   L.off_fc = take((uint64_t)3 * pm * 8);
   L.off_prec = take((uint64_t)10 * pm * 8);
+  L.off_pos2 = take((uint64_t)3 * pm * 8);
+  L.off_vel2 = take((uint64_t)3 * pm * 8);
   L.off_count = take((uint64_t)(L.ncells_max + 1) * 4);
   L.off_start = take((uint64_t)(L.ncells_max + 1) * 4);
   L.off_fill = take((uint64_t)(L.ncells_max + 1) * 4);
@@ -258,6 +260,8 @@ lbmimb_status lbmimb_create_lattice(const lbmimb_params *params, int64_t max_par
   h->torque = (double *)(h->ws + L.off_torque);
   h->fc = (double *)(h->ws + L.off_fc);
   h->prec = (double *)(h->ws + L.off_prec);
+  h->pos2 = (double *)(h->ws + L.off_pos2);
+  h->vel2 = (double *)(h->ws + L.off_vel2);
   h->cl.count = (int32_t *)(h->ws + L.off_count);
   h->cl.start = (int32_t *)(h->ws + L.off_start);
   h->cl.fill = (int32_t *)(h->ws + L.off_fill);
@@ -606,13 +610,13 @@ static lbmimb_status check_dem_params(const lbmimb_dem_params *dem) {
 static lbmimb_status dem_body(lbmimb_lattice *h, const lbmimb_dem_params *dem, bool finish) {
   if (h->P == 0) return LBMIMB_OK;
   lbmimb_status st;
-  const bool small = dem_small_path(h);
+  const bool cells = dem_can_finish(h);   // cell-list mode: the second-half kernel packs the records itself
   if ((st = launch_dem(h, dem, finish)) != LBMIMB_OK) return st;
   // positions moved: the map and the exchange vectors are stale; the cell list was rebuilt at
   // the new positions inside the step and stays valid; force/torque stay "the last reduction"
   h->map_valid = false;
   h->s_valid = false;
-  return small ? LBMIMB_OK : launch_pack_records(h);   // the single-block step packs the records itself
+  return cells ? LBMIMB_OK : launch_pack_records(h);
 }
 
 lbmimb_status lbmimb_dem_step(lbmimb_lattice *h, const lbmimb_dem_params *dem) {
@@ -629,7 +633,7 @@ static lbmimb_status coupled_step_body(lbmimb_lattice *h, const lbmimb_dem_param
   lbmimb_status st;
   if ((st = map_body(h)) != LBMIMB_OK) return st;
   if ((st = step_body(h, 1)) != LBMIMB_OK) return st;
-  if (h->P > 0 && dem_small_path(h)) {   // a3's conversion of the sums rides in the single-block DEM kernel
+  if (h->P > 0 && dem_can_finish(h)) {   // a3's conversion of the sums rides in the first DEM kernel
     h->forces_valid = true;
     h->acc_dirty = false;
     return dem_body(h, dem, true);
@@ -666,7 +670,7 @@ static lbmimb_status coupled_graph_capture(lbmimb_lattice *h, const lbmimb_dem_p
   // device, so everything the captured calls toggled is put back
   const int cur0 = h->cur;
   const bool swapped0 = h->aa_swapped, map0 = h->map_valid, s0 = h->s_valid, forces0 = h->forces_valid;
-  const bool cl0 = h->cl_valid, dirty0 = h->acc_dirty;
+  const bool cl0 = h->cl_valid, dirty0 = h->acc_dirty, clean0 = h->cl.count_clean;
   const double table0 = h->table_R;
   LBMIMB_CUDA(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
   h->stream = h->cap_stream;
@@ -688,6 +692,7 @@ static lbmimb_status coupled_graph_capture(lbmimb_lattice *h, const lbmimb_dem_p
     h->forces_valid = forces0;
     h->cl_valid = cl0;
     h->acc_dirty = dirty0;
+    h->cl.count_clean = clean0;
     h->table_R = table0;
     return st != LBMIMB_OK ? st : cuda_fail(e, "cudaStreamEndCapture(coupled steps)");
   }

@@ -180,46 +180,56 @@ __device__ __forceinline__ void solid_velocity(const double *__restrict__ pr, in
 // the run adds the partial sum to the particle's accumulators as 64-bit FIXED-POINT integers: integer
 // addition is associative, so the total does not depend on the order in which warps arrive, and the
 // reduction is bitwise reproducible without a second pass over the lattice.
-//   value = hi 2^-40 + lo 2^-92: hi = rint(v 2^40), lo = rint((v - hi 2^-40) 2^92); the remainder is exact
-//   and |lo| <= 2^51, so runs add without overflow and a sum resolves 2^-92 ~ 2e-28 (|v| < 2^22).
+//   value = hi 2^-40 + lo 2^-91: hi = rint(v 2^40), lo = rint((v - hi 2^-40) 2^91); the remainder is exact
+//   and |lo| <= 2^50, so thousands of runs add without overflow and a sum resolves 2^-91 ~ 4e-28 (|v| < 2^11).
+// A run lies in one lattice row, so the lever arm components r_y, r_z are the same on all its nodes and
+//   sum r x s = (r_y S_z - r_z S_y,  r_z S_x - sum r_x s_z,  sum r_x s_y - r_y S_x),  S = sum s:
+// five sums per run in 3D (three in 2D) instead of six, combined by the head lane.
 // ---------------------------------------------------------------------------
+// double -> integer without the (slow) conversion unit: for |x| < 2^51, x + 1.5 2^52 has the integer nearest to x in
+// its low mantissa bits, and subtracting the constant again gives that integer back as a double, exactly.
+__device__ __forceinline__ long long round_to_ll(double x, double &rounded) {
+  constexpr double kMagic = 6755399441055744.0;   // 1.5 * 2^52
+  const double t = x + kMagic;
+  rounded = t - kMagic;
+  return __double_as_longlong(t) - __double_as_longlong(kMagic);
+}
+
 __device__ __forceinline__ void fixed_add(long long *acc, double v) {
   constexpr double k40 = 1099511627776.0, k52 = 4503599627370496.0;
-  const long long hi = __double2ll_rn(v * k40);
-  const double rem = v - (double)hi * (1.0 / k40);
-  const long long lo = __double2ll_rn((rem * k40) * k52);
+  double hi_d, lo_d;
+  const long long hi = round_to_ll(v * k40, hi_d);          // |v| < 2^11 (a force in lattice units)
+  const double rem = v - hi_d * (1.0 / k40);                // exact, |rem| <= 2^-41
+  const long long lo = round_to_ll((rem * k40) * (k52 * 0.5), lo_d);   // rem 2^91: |.| <= 2^50
   atomicAdd(reinterpret_cast<unsigned long long *>(acc), (unsigned long long)hi);
   if (lo != 0) atomicAdd(reinterpret_cast<unsigned long long *>(acc) + 1, (unsigned long long)lo);
 }
 
 __host__ __device__ __forceinline__ double fixed_value(long long hi, long long lo) {
-  return (double)hi * (1.0 / 1099511627776.0) + ((double)lo * (1.0 / 4503599627370496.0)) * (1.0 / 1099511627776.0);
+  return (double)hi * (1.0 / 1099511627776.0) + ((double)lo * (2.0 / 4503599627370496.0)) * (1.0 / 1099511627776.0);
 }
 
-// Whole warp must call.  key < 0: this lane contributes nothing.  v[NV]: this node's -s and -(r x s).
+// Whole warp must call.  key < 0: this lane contributes nothing.  On return the FIRST lane of every run of equal
+// keys holds the run's sums in v[NV] and the function returns true there (false on all other lanes).
 template <int NV>
-__device__ __forceinline__ void accumulate_runs(int key, double (&v)[NV], long long *__restrict__ facc) {
+__device__ __forceinline__ bool reduce_runs(int key, double (&v)[NV]) {
   const unsigned lane = threadIdx.x & 31u;
   const int prev = __shfl_up_sync(0xffffffffu, key, 1);
   const bool boundary = key < 0 || lane == 0 || prev != key;       // first lane of a run (or an idle lane)
   const unsigned bmask = __ballot_sync(0xffffffffu, boundary);
-  if (__all_sync(0xffffffffu, key < 0)) return;
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) {
     // lanes lane+1 .. lane+d all continue this lane's run?
     const unsigned between = ((1u << d) - 1u) << 1;
     const bool take = lane + d < 32u && ((bmask >> lane) & between) == 0u;
+    if (!__any_sync(0xffffffffu, take)) break;   // no run is longer than d: the remaining steps add nothing
 #pragma unroll
     for (int c = 0; c < NV; ++c) {
       const double o = __shfl_down_sync(0xffffffffu, v[c], d);
       if (take) v[c] += o;
     }
   }
-  if (boundary && key >= 0) {
-    long long *acc = facc + (int64_t)key * (2 * NV);
-#pragma unroll
-    for (int c = 0; c < NV; ++c) fixed_add(acc + 2 * c, v[c]);
-  }
+  return boundary && key >= 0;
 }
 
 }  // namespace lbmimb

@@ -45,12 +45,26 @@ __device__ __forceinline__ void emit_exchange(const StepArgs &a, int64_t x, bool
   const double br = beta * rho;
   const double sx = br * (vx - ux), sy = br * (vy - uy), sz = br * (vz - uz);   // s = beta rho (V_S - u)  (P6)
   if (EMIT == kEmitField && covered) store_exchange<D>(a.s, x, sx, sy, sz);
+  const int key = covered ? pe : -1;
   if (D == 2) {
-    double v[3] = {-sx, -sy, -(rx * sy - ry * sx)};
-    accumulate_runs<3>(covered ? pe : -1, v, a.facc);
+    double v[3] = {sx, sy, rx * sy};
+    if (reduce_runs<3>(key, v)) {
+      long long *acc = a.facc + (int64_t)key * 6;
+      fixed_add(acc + 0, -v[0]);
+      fixed_add(acc + 2, -v[1]);
+      fixed_add(acc + 4, -(v[2] - ry * v[0]));
+    }
   } else {
-    double v[6] = {-sx, -sy, -sz, -(ry * sz - rz * sy), -(rz * sx - rx * sz), -(rx * sy - ry * sx)};
-    accumulate_runs<6>(covered ? pe : -1, v, a.facc);
+    double v[5] = {sx, sy, sz, rx * sy, rx * sz};
+    if (reduce_runs<5>(key, v)) {
+      long long *acc = a.facc + (int64_t)key * 12;
+      fixed_add(acc + 0, -v[0]);
+      fixed_add(acc + 2, -v[1]);
+      fixed_add(acc + 4, -v[2]);
+      fixed_add(acc + 6, -(ry * v[2] - rz * v[1]));
+      fixed_add(acc + 8, -(rz * v[0] - v[4]));
+      fixed_add(acc + 10, -(v[3] - ry * v[0]));
+    }
   }
 }
 

@@ -75,8 +75,8 @@ __host__ __device__ constexpr int tag_cnt(uint32_t t) { return (int)(t & 0xffu);
 __host__ __device__ constexpr int32_t tag_pid(uint32_t t) { return (t & 0xffu) ? (int32_t)(t >> kTagPidShift) : -1; }
 
 // Per-particle force / torque accumulators of the fused step: NV = 3 (2D: Fx Fy Tz) or 6 (3D: F, T) values,
-// each a pair of 64-bit fixed-point words (value = hi 2^-40 + lo 2^-92), added with integer atomics: the
-// sum does not depend on the order in which warps arrive (collide.cuh: accumulate_runs).
+// each a pair of 64-bit fixed-point words (value = hi 2^-40 + lo 2^-91), added with integer atomics: the
+// sum does not depend on the order in which warps arrive (collide.cuh: reduce_runs).
 __host__ __device__ constexpr int force_values(int dim) { return dim == 3 ? 6 : 3; }
 
 struct Geom {
@@ -127,6 +127,7 @@ struct CellList {
   int32_t *cell_of; // [Pmax]
   int32_t *block_sums;  // scan scratch
   int64_t ncells_max;
+  bool count_clean;     // count[] is all zero (the DEM first half adds to it; cl_small_kernel leaves it zeroed)
 };
 
 // Verlet neighbour lists of a4 (R19).  Library-allocated (sized from the radii).
@@ -201,6 +202,7 @@ struct lbmimb_lattice {
   // particles (SoA, device)
   int64_t Pmax, P;
   double *pos, *vel, *omega, *radius, *mass, *force, *torque, *fc, *prec;
+  double *pos2, *vel2;   // state after the first half of a DEM step (double buffer, cell-list mode)
   double rmax, rmin;  // largest / smallest radius of the current set
   int map_mode;       // LBMIMB_MAP_SAMPLING or LBMIMB_MAP_TABLE
   uint8_t *eps_table; // table of map mode TABLE (R17), built for radius table_R
@@ -251,7 +253,7 @@ lbmimb_status ensure_eps_table(lbmimb_lattice *h);
 int64_t eps_table_entries(int dim);
 lbmimb_status launch_finish_forces(lbmimb_lattice *h);   // facc -> force / torque, clears facc
 lbmimb_status launch_dem(lbmimb_lattice *h, const lbmimb_dem_params *dem, bool finish);
-bool dem_small_path(const lbmimb_lattice *h);
+bool dem_can_finish(const lbmimb_lattice *h);
 lbmimb_status neighbor_list_prepare(lbmimb_lattice *h);   // (re)allocates the list storage for the current radii
 void neighbor_list_release(lbmimb_lattice *h);
 lbmimb_status neighbor_list_invalidate(lbmimb_lattice *h);  // positions were replaced

@@ -266,6 +266,8 @@ static CellGeom cell_geom(const lbmimb_lattice *h) {
   return cg;
 }
 
+lbmimb_status finish_cell_list(lbmimb_lattice *h);
+
 lbmimb_status build_cell_list(lbmimb_lattice *h) {
   double edge = 2.0 * h->rmax;
   if (edge < h->rmax + 1.0) edge = h->rmax + 1.0;
@@ -293,6 +295,14 @@ lbmimb_status build_cell_list(lbmimb_lattice *h) {
   CellGeom cg = cell_geom(h);
   cl_count_kernel<<<blocks_for(h->P, 256), 256, 0, h->stream>>>(cg, h->P, h->pos, cl.cell_of, cl.count);
   LBMIMB_LAUNCH_CHECK(h, "cl_count_kernel");
+  return finish_cell_list(h);
+}
+
+// second part of the counting sort: count[] and cell_of[] are filled (fill[] zeroed) -> start[], items[]
+lbmimb_status finish_cell_list(lbmimb_lattice *h) {
+  CellList &cl = h->cl;
+  const int64_t n1 = cl.ncells + 1;
+  cl.count_clean = false;
   const int nb = (int)((n1 + kScanChunk - 1) / kScanChunk);
   scan_reduce_kernel<<<nb, 256, 0, h->stream>>>(cl.count, n1, cl.block_sums);
   LBMIMB_LAUNCH_CHECK(h, "scan_reduce_kernel");
@@ -616,7 +626,7 @@ lbmimb_status launch_map(lbmimb_lattice *h) {
 }
 
 // ---------------------------------------------------------------------------
-// a3: the per-particle sums of eq. (3) are formed inside the fused step (collide.cuh: accumulate_runs) as
+// a3: the per-particle sums of eq. (3) are formed inside the fused step (collide.cuh: reduce_runs) as
 // fixed-point integers; this kernel turns them into force / torque and clears the accumulators for the
 // next emitting step.  (Round 1 wrote a 32-byte exchange record per covered node and gathered the records
 // per particle in a second pass over the bounding boxes: C3 0.38 GB written + 0.72 GB read, 0.18 ms.)
@@ -723,9 +733,10 @@ __device__ __forceinline__ void wall_force(const DemArgs &a, const int *n, const
 
 // contact force on particle i: the particles of the 3^D cells around it (ascending index inside a cell), then the walls
 template <int D>
-__device__ __forceinline__ void dem_contact_one(const DemArgs &a, int64_t i) {
+__device__ __forceinline__ void dem_contact_sum(const DemArgs &a, int64_t i, double *F) {
   const int n[3] = {a.g.nx, a.g.ny, a.g.nz};
-  double xi[3], vi[3], F[3] = {0.0, 0.0, 0.0};
+  double xi[3], vi[3];
+  F[0] = F[1] = F[2] = 0.0;
   for (int c = 0; c < D; ++c) {
     xi[c] = a.pos[(int64_t)c * a.P + i];
     vi[c] = a.vel[(int64_t)c * a.P + i];
@@ -754,13 +765,6 @@ __device__ __forceinline__ void dem_contact_one(const DemArgs &a, int64_t i) {
         }
       }
   wall_force<D>(a, n, xi, vi, Ri, mi, F);
-  for (int q = 0; q < D; ++q) a.fc[(int64_t)q * a.P + i] = F[q];
-}
-
-template <int D>
-__global__ void dem_contact_kernel(const DemArgs a) {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < a.P) dem_contact_one<D>(a, i);
 }
 
 // the same sums over the neighbour lists (ascending j).  Runs right after the three predicated
@@ -847,143 +851,191 @@ __global__ void dem_kick_kernel(const DemArgs a) {
 }
 
 // ---------------------------------------------------------------------------
-// Small particle sets (P <= kDemSmallP, cell mode): the whole DEM step as ONE single-block kernel.  A coupled
-// step of C5 (4,096 spheres) used to spend 10 dependent launches of 3-6 microseconds each on it (contact,
-// kick+drift, a counting-sort cell list of 2 memsets + 6 kernels, contact, kick, record packing) plus the
-// force conversion of a3; block barriers replace the launch boundaries, global memory is the only storage
-// (coherent inside a block after __syncthreads), and every per-particle / per-cell routine is the one the
-// multi-kernel path runs, in the same order: results are bit for bit the same.
-//   FINISH: first turn the fixed-point force sums of the fused step into force / torque (a3's last part).
-// Leaves a cell list of the NEW positions behind (the map of the next step uses it) and the packed records.
+// Cell-list mode: the DEM step in two kernels around the rebuild of the cell list.  Positions and velocities
+// are double-buffered (pos2 / vel2), so that a particle can take its half step while its neighbours' contact
+// sums still read the old state: no kernel boundary is needed between the contact sum and the kick.
+//   first half : [a3: fixed-point force sums -> force / torque]  F_c(x, v) -> v2 = v + dt/2 a0, x2 = x + dt v2
+//                (wrapped), cell of x2 counted
+//   cell list of x2 (one single-block kernel for small sets, else the counting sort of build_cell_list)
+//   second half: F_c(x2, v2) -> v = v2 + dt/2 a1, x = x2, omega += dt T_h / I, packed record
+// Same per-particle arithmetic and summation order as the one-kernel-per-phase sequence of round 1 (and as the
+// neighbour-list path below): bit for bit the same trajectories.  C5: 10 launches + 2 memsets -> 3 launches.
 // ---------------------------------------------------------------------------
-constexpr int kDemSmallP = 8192;
-constexpr int kDemSmallCells = 1024 * 64;
-constexpr int kDemSmallThreads = 1024;
-
-struct DemSmallArgs {
-  CellGeom cg_new;     // cell geometry for the list of the new positions (= the old one: same radii)
-  int64_t ncells;
-  int32_t *count, *start, *fill, *items, *cell_of;
+struct DemCellArgs {
+  double *pos2, *vel2;          // state after the first half step
+  double *pos_out, *vel_out;    // final state (the handle's pos / vel)
+  int32_t *count, *cell_of;     // cell list under construction
   long long *facc;
   double *force_w, *torque_w;   // writable views of force / torque (FINISH)
   double *prec;
-  int dim;
 };
 
 template <int D, bool FINISH>
-__global__ void __launch_bounds__(kDemSmallThreads) dem_small_kernel(const DemArgs a, const DemSmallArgs b) {
-  __shared__ int32_t wsum[kDemSmallThreads / 32];
-  __shared__ int32_t carry_s;
-  const int tid = threadIdx.x;
+__global__ void __launch_bounds__(128) dem_first_half_kernel(const DemArgs a, const DemCellArgs b) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= a.P) return;
   const int64_t P = a.P;
-  if (FINISH) {   // same thread -> same particles in every phase below: no barrier needed before the kicks
+  double Fh[3] = {0.0, 0.0, 0.0};
+  if (FINISH) {
     constexpr int NV = D == 2 ? 3 : 6;
-    for (int64_t p = tid; p < P; p += kDemSmallThreads) {
-      longlong2 *acc = reinterpret_cast<longlong2 *>(b.facc + p * (2 * NV));
-      double v[NV];
+    longlong2 *acc = reinterpret_cast<longlong2 *>(b.facc + p * (2 * NV));
+    double v[NV];
 #pragma unroll
-      for (int c = 0; c < NV; ++c) {
-        const longlong2 w = acc[c];
-        v[c] = fixed_value(w.x, w.y);
-        acc[c] = make_longlong2(0, 0);
-      }
+    for (int c = 0; c < NV; ++c) {
+      const longlong2 w = acc[c];
+      v[c] = fixed_value(w.x, w.y);
+      acc[c] = make_longlong2(0, 0);
+    }
 #pragma unroll
-      for (int c = 0; c < D; ++c) b.force_w[(int64_t)c * P + p] = v[c];
-      if (D == 2) {
-        b.torque_w[p] = v[2];
-      } else {
+    for (int c = 0; c < D; ++c) {
+      b.force_w[(int64_t)c * P + p] = v[c];
+      Fh[c] = v[c];
+    }
+    if (D == 2) {
+      b.torque_w[p] = v[2];
+    } else {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) b.torque_w[(int64_t)c * P + p] = v[3 + c];
+      for (int c = 0; c < 3; ++c) b.torque_w[(int64_t)c * P + p] = v[3 + c];
+    }
+  } else {
+#pragma unroll
+    for (int c = 0; c < D; ++c) Fh[c] = a.force[(int64_t)c * P + p];
+  }
+  double Fc[3];
+  dem_contact_sum<D>(a, p, Fc);
+  const int n[3] = {a.g.nx, a.g.ny, a.g.nz};
+  const bool per[3] = {!a.g.bcx, !a.g.bcy, !a.g.bcz};
+  const double m = a.mass[p];
+  double xn[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+  for (int q = 0; q < D; ++q) {
+    const int64_t id = (int64_t)q * P + p;
+    const double a0 = (Fh[q] + Fc[q]) / m + a.gp[q];
+    const double v = a.vel[id] + 0.5 * a.dt * a0;
+    b.vel2[id] = v;
+    double x = a.pos[id] + a.dt * v;
+    if (per[q]) {
+      if (x >= (double)n[q]) x -= (double)n[q];
+      if (x < 0.0) x += (double)n[q];
+    }
+    b.pos2[id] = x;
+    xn[q] = x;
+  }
+  const int cx = cell_coord(xn[0], a.cg, 0), cy = cell_coord(xn[1], a.cg, 1);
+  const int cz = D == 3 ? cell_coord(xn[2], a.cg, 2) : 0;
+  const int c = (cz * a.cg.nc[1] + cy) * a.cg.nc[0] + cx;
+  b.cell_of[p] = c;
+  atomicAdd(b.count + c, 1);
+}
+
+// a.pos / a.vel = the half-step state (pos2 / vel2), a.start / a.items = the cell list of pos2
+template <int D>
+__global__ void __launch_bounds__(128) dem_second_half_kernel(const DemArgs a, const DemCellArgs b) {
+  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= a.P) return;
+  const int64_t P = a.P;
+  double Fc[3];
+  dem_contact_sum<D>(a, p, Fc);
+  const double m = a.mass[p], R = a.radius[p];
+  double x[3] = {0.0, 0.0, 0.0}, v[3] = {0.0, 0.0, 0.0}, w[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+  for (int q = 0; q < D; ++q) {
+    const int64_t id = (int64_t)q * P + p;
+    const double a1 = (a.force[id] + Fc[q]) / m + a.gp[q];
+    v[q] = a.vel[id] + 0.5 * a.dt * a1;
+    x[q] = a.pos[id];
+    b.vel_out[id] = v[q];
+    b.pos_out[id] = x[q];
+  }
+  const double I = (D == 3 ? 0.4 : 0.5) * m * R * R;
+  constexpr int nt = D == 2 ? 1 : 3;
+#pragma unroll
+  for (int q = 0; q < nt; ++q) {
+    const int64_t id = (int64_t)q * P + p;
+    w[q] = a.omega[id] + a.dt * a.torque[id] / I;
+    a.omega[id] = w[q];
+  }
+  double *r = b.prec + p * prec_stride(D);
+  if (D == 2) {
+    r[0] = x[0];
+    r[1] = x[1];
+    r[2] = v[0];
+    r[3] = v[1];
+    r[4] = w[0];
+    r[5] = R;
+  } else {
+    r[0] = x[0];
+    r[1] = x[1];
+    r[2] = x[2];
+    r[3] = v[0];
+    r[4] = v[1];
+    r[5] = v[2];
+    r[6] = w[0];
+    r[7] = w[1];
+    r[8] = w[2];
+    r[9] = R;
+  }
+}
+
+// Cell list of a small set from the counts the first half left: exclusive scan, fill, sort -- one block, so
+// that block barriers stand where the counting sort of build_cell_list has five kernel boundaries.  Leaves
+// count and fill zeroed for the next step.
+constexpr int kListSmallP = 65536;
+constexpr int kListSmallCells = 1024 * 64;
+constexpr int kListSmallThreads = 1024;
+
+__global__ void __launch_bounds__(kListSmallThreads) cl_small_kernel(int64_t P, int64_t ncells, int32_t *__restrict__ count,
+                                                                   int32_t *__restrict__ start,
+                                                                   int32_t *__restrict__ fill,
+                                                                   int32_t *__restrict__ items,
+                                                                   const int32_t *__restrict__ cell_of) {
+  __shared__ int32_t wsum[kListSmallThreads / 32];
+  const int tid = threadIdx.x;
+  const int64_t n1 = ncells + 1;
+  const int per = (int)((n1 + kListSmallThreads - 1) / kListSmallThreads);
+  const int64_t lo = (int64_t)tid * per;
+  int32_t tot = 0;
+  for (int e = 0; e < per; ++e)
+    if (lo + e < ncells) tot += count[lo + e];
+  int32_t incl = tot;
+  const int lane = tid & 31, wid = tid >> 5;
+  for (int o = 1; o < 32; o <<= 1) {
+    const int32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += t;
+  }
+  if (lane == 31) wsum[wid] = incl;
+  __syncthreads();
+  int32_t woff = 0;
+  for (int w = 0; w < wid; ++w) woff += wsum[w];
+  int32_t run = woff + incl - tot;
+  for (int e = 0; e < per; ++e)
+    if (lo + e < n1) {
+      start[lo + e] = run;
+      if (lo + e < ncells) {
+        run += count[lo + e];
+        count[lo + e] = 0;
+        fill[lo + e] = 0;
       }
     }
-  }
-  for (int64_t i = tid; i < P; i += kDemSmallThreads) dem_contact_one<D>(a, i);
-  __syncthreads();   // every contact sum read the OLD positions and velocities
-  for (int64_t p = tid; p < P; p += kDemSmallThreads) dem_kick_drift_one<D>(a, p);
-  for (int64_t c = tid; c <= b.ncells; c += kDemSmallThreads) b.count[c] = 0;
-  for (int64_t c = tid; c < b.ncells; c += kDemSmallThreads) b.fill[c] = 0;
   __syncthreads();
-  // ---- cell list of the new positions: count, exclusive scan, fill, sort (as build_cell_list)
-  for (int64_t p = tid; p < P; p += kDemSmallThreads) {
-    const int cx = cell_coord(a.pos[p], b.cg_new, 0);
-    const int cy = cell_coord(a.pos[P + p], b.cg_new, 1);
-    const int cz = D == 3 ? cell_coord(a.pos[2 * P + p], b.cg_new, 2) : 0;
-    const int c = (cz * b.cg_new.nc[1] + cy) * b.cg_new.nc[0] + cx;
-    b.cell_of[p] = c;
-    atomicAdd(b.count + c, 1);
-  }
-  if (tid == 0) carry_s = 0;
-  __syncthreads();
-  {
-    const int64_t n1 = b.ncells + 1;
-    const int per = (int)((n1 + kDemSmallThreads - 1) / kDemSmallThreads);
-    const int64_t lo = (int64_t)tid * per;
-    int32_t tot = 0;
-    for (int e = 0; e < per; ++e)
-      if (lo + e < n1) tot += b.count[lo + e];
-    int32_t incl = tot;
-    const int lane = tid & 31, wid = tid >> 5;
-    for (int o = 1; o < 32; o <<= 1) {
-      const int32_t t = __shfl_up_sync(0xffffffffu, incl, o);
-      if (lane >= o) incl += t;
-    }
-    if (lane == 31) wsum[wid] = incl;
-    __syncthreads();
-    int32_t woff = 0;
-    for (int w = 0; w < wid; ++w) woff += wsum[w];
-    int32_t run = woff + incl - tot;
-    for (int e = 0; e < per; ++e)
-      if (lo + e < n1) {
-        b.start[lo + e] = run;
-        run += b.count[lo + e];
-      }
+  for (int64_t p = tid; p < P; p += kListSmallThreads) {
+    const int c = cell_of[p];
+    const int slot = atomicAdd(fill + c, 1);
+    items[start[c] + slot] = (int32_t)p;
   }
   __syncthreads();
-  for (int64_t p = tid; p < P; p += kDemSmallThreads) {
-    const int c = b.cell_of[p];
-    const int slot = atomicAdd(b.fill + c, 1);
-    b.items[b.start[c] + slot] = (int32_t)p;
-  }
-  __syncthreads();
-  for (int64_t c = tid; c < b.ncells; c += kDemSmallThreads) {
-    const int bg = b.start[c], en = b.start[c + 1];
+  for (int64_t c = tid; c < ncells; c += kListSmallThreads) {
+    const int bg = start[c], en = start[c + 1];
     for (int q0 = bg + 1; q0 < en; ++q0) {
-      const int32_t v = b.items[q0];
+      const int32_t v = items[q0];
       int q = q0 - 1;
-      while (q >= bg && b.items[q] > v) {
-        b.items[q + 1] = b.items[q];
+      while (q >= bg && items[q] > v) {
+        items[q + 1] = items[q];
         --q;
       }
-      b.items[q + 1] = v;
+      items[q + 1] = v;
     }
-  }
-  __syncthreads();
-  DemArgs a2 = a;
-  a2.cg = b.cg_new;
-  for (int64_t i = tid; i < P; i += kDemSmallThreads) dem_contact_one<D>(a2, i);
-  __syncthreads();   // the kicks below change velocities the contact sums above read
-  for (int64_t p = tid; p < P; p += kDemSmallThreads) {
-    dem_kick_one<D>(a, p);
-    double *r = b.prec + p * prec_stride(D);
-    if (D == 2) {
-      r[0] = a.pos[p];
-      r[1] = a.pos[P + p];
-      r[2] = a.vel[p];
-      r[3] = a.vel[P + p];
-      r[4] = a.omega[p];
-      r[5] = a.radius[p];
-    } else {
-      r[0] = a.pos[p];
-      r[1] = a.pos[P + p];
-      r[2] = a.pos[2 * P + p];
-      r[3] = a.vel[p];
-      r[4] = a.vel[P + p];
-      r[5] = a.vel[2 * P + p];
-      r[6] = a.omega[p];
-      r[7] = a.omega[P + p];
-      r[8] = a.omega[2 * P + p];
-      r[9] = a.radius[p];
-    }
+    fill[c] = 0;
   }
 }
 
@@ -1103,21 +1155,8 @@ static lbmimb_status verlet_ensure(lbmimb_lattice *h, const VerletArgs &v) {
   return LBMIMB_OK;
 }
 
-// can this handle's DEM step run as the single-block kernel (which can also do a3's conversion)?
-bool dem_small_path(const lbmimb_lattice *h) {
-  if (h->nl.mode == LBMIMB_NEIGHBOR_VERLET || h->P > kDemSmallP) return false;
-  // same geometry rule as build_cell_list
-  double edge = 2.0 * h->rmax;
-  if (edge < h->rmax + 1.0) edge = h->rmax + 1.0;
-  if (edge < 2.0) edge = 2.0;
-  const int n[3] = {h->gp.nx, h->gp.ny, h->gp.nz};
-  int64_t nc = 1;
-  for (int a = 0; a < h->g.dim; ++a) {
-    int c = (int)floor((double)n[a] / edge);
-    nc *= c < 1 ? 1 : c;
-  }
-  return nc + 1 <= kDemSmallCells;
-}
+// In cell-list mode the first-half kernel can also convert the fixed-point force sums (a3's last part).
+bool dem_can_finish(const lbmimb_lattice *h) { return h->nl.mode != LBMIMB_NEIGHBOR_VERLET; }
 
 template <int D>
 static lbmimb_status dem_impl(lbmimb_lattice *h, const lbmimb_dem_params *dem, bool finish) {
@@ -1177,41 +1216,44 @@ static lbmimb_status dem_impl(lbmimb_lattice *h, const lbmimb_dem_params *dem, b
     h->cl_valid = false;   // the particles moved and no cell list was built at the new positions
     return LBMIMB_OK;
   }
-  if (dem_small_path(h)) {
-    DemSmallArgs b;
-    b.cg_new = a.cg;
-    b.ncells = h->cl.ncells;
-    b.count = h->cl.count;
-    b.start = h->cl.start;
-    b.fill = h->cl.fill;
-    b.items = h->cl.items;
-    b.cell_of = h->cl.cell_of;
-    b.facc = h->facc;
-    b.force_w = h->force;
-    b.torque_w = h->torque;
-    b.prec = h->prec;
-    b.dim = D;
-    if (finish) dem_small_kernel<D, true><<<1, kDemSmallThreads, 0, h->stream>>>(a, b);
-    else dem_small_kernel<D, false><<<1, kDemSmallThreads, 0, h->stream>>>(a, b);
-    LBMIMB_LAUNCH_CHECK(h, "dem_small_kernel");
-    return LBMIMB_OK;   // cell list of the new positions and packed records are in place
+  // ---- cell-list mode: first half, cell list of the new positions, second half
+  CellList &cl = h->cl;
+  if (!cl.count_clean) {
+    LBMIMB_CUDA(cudaMemsetAsync(cl.count, 0, (size_t)(cl.ncells + 1) * 4, h->stream));
+    cl.count_clean = true;
   }
-  if (finish) return fail(LBMIMB_EINVAL, "internal: force conversion can only be folded into the single-block DEM step");
-  dem_contact_kernel<D><<<nb, 128, 0, h->stream>>>(a);
-  LBMIMB_LAUNCH_CHECK(h, "dem_contact_kernel");
-  dem_kick_drift_kernel<D><<<nb, 128, 0, h->stream>>>(a);
-  LBMIMB_LAUNCH_CHECK(h, "dem_kick_drift_kernel");
-  if ((st = build_cell_list(h)) != LBMIMB_OK) return st;
-  a.cg = cell_geom(h);
-  dem_contact_kernel<D><<<nb, 128, 0, h->stream>>>(a);
-  LBMIMB_LAUNCH_CHECK(h, "dem_contact_kernel");
-  dem_kick_kernel<D><<<nb, 128, 0, h->stream>>>(a);
-  LBMIMB_LAUNCH_CHECK(h, "dem_kick_kernel");
-  return LBMIMB_OK;
+  DemCellArgs b;
+  b.pos2 = h->pos2;
+  b.vel2 = h->vel2;
+  b.pos_out = h->pos;
+  b.vel_out = h->vel;
+  b.count = cl.count;
+  b.cell_of = cl.cell_of;
+  b.facc = h->facc;
+  b.force_w = h->force;
+  b.torque_w = h->torque;
+  b.prec = h->prec;
+  if (finish) dem_first_half_kernel<D, true><<<nb, 128, 0, h->stream>>>(a, b);
+  else dem_first_half_kernel<D, false><<<nb, 128, 0, h->stream>>>(a, b);
+  LBMIMB_LAUNCH_CHECK(h, "dem_first_half_kernel");
+  if (h->P <= kListSmallP && cl.ncells + 1 <= kListSmallCells) {
+    cl_small_kernel<<<1, kListSmallThreads, 0, h->stream>>>(h->P, cl.ncells, cl.count, cl.start, cl.fill, cl.items,
+                                                           cl.cell_of);
+    LBMIMB_LAUNCH_CHECK(h, "cl_small_kernel");
+  } else {
+    LBMIMB_CUDA(cudaMemsetAsync(cl.fill, 0, (size_t)cl.ncells * 4, h->stream));
+    if ((st = finish_cell_list(h)) != LBMIMB_OK) return st;   // scan, fill, sort of build_cell_list (count stays dirty)
+  }
+  h->cl_valid = true;
+  a.pos = h->pos2;
+  a.vel = h->vel2;
+  dem_second_half_kernel<D><<<nb, 128, 0, h->stream>>>(a, b);
+  LBMIMB_LAUNCH_CHECK(h, "dem_second_half_kernel");
+  return LBMIMB_OK;   // cell list of the new positions and packed records are in place
 }
 
-// finish: also convert the fixed-point force sums of the last step (only with dem_small_path(h)).
-// On return the packed records are current if dem_small_path(h), else the caller packs them.
+// finish: also convert the fixed-point force sums of the last step (cell-list mode only, dem_can_finish).
+// On return the packed records are current in cell-list mode; in neighbour-list mode the caller packs them.
 lbmimb_status launch_dem(lbmimb_lattice *h, const lbmimb_dem_params *dem, bool finish) {
   return h->g.dim == 2 ? dem_impl<2>(h, dem, finish) : dem_impl<3>(h, dem, finish);
 }

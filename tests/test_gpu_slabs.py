@@ -28,8 +28,8 @@ def _slabs_for(lb, w, nslabs, bc=None):
     return s
 
 
-@pytest.mark.parametrize("name,nslabs,periodic_y", [("C3", 2, False), ("C3", 3, False), ("C2", 3, False), ("C4", 2, False),
-                                                    ("P3D", 2, True), ("P3D", 1, True), ("P2D", 4, True)])
+@pytest.mark.parametrize("name,nslabs,periodic_y", [("C3", 2, False), ("C3", 3, False), ("C2", 3, False), ("C4", 3, False),
+                                                    ("P3D", 4, True), ("P3D", 1, True), ("P2D", 4, True)])
 def test_fixed_particles_slabs_against_the_undivided_lattice(orc, lb, name, nslabs, periodic_y):
     """Reduced cuts (particles cut by the slab faces, walls or a periodic seam in y): maps bit-exact, f <= 1e-12 and
     forces <= 1e-10 against the oracle; everything bitwise equal to the undivided CUDA lattice."""
@@ -60,7 +60,7 @@ def test_fixed_particles_slabs_against_the_undivided_lattice(orc, lb, name, nsla
     one.close()
 
 
-@pytest.mark.parametrize("name,nslabs", [("C5", 2), ("P3D", 3)])
+@pytest.mark.parametrize("name,nslabs", [("C5", 2), ("P3D", 4)])
 def test_coupled_windows_on_slabs(orc, lb, name, nslabs):
     """The coupled protocol (oracle.coupled_step leads, shared state at every window start) with the lattice in
     slabs: map -> step -> halo exchange -> force sums across slabs -> reduce -> DEM on every slab."""
