@@ -26,8 +26,8 @@ struct StepArgs {
   unsigned tiles;      // blocks per lattice row
   SlabRows sl;         // stored rows <-> global rows, wall flags of the two y ends, owned rows
   CollideParams cp;
-  // AA odd step, rows away from walls and seams: f_q(x) lives koff[q] bytes behind element x - cx_q
-  // of the array (koff[q] = 8 (opposite(q) * N - cy_q * nx - cz_q * nx * ny))
+  // Rows away from walls and seams: f_q(x) is read koff[q] bytes behind element x - cx_q of the array.
+  //   pull (A-B):  koff[q] = 8 (q N - cy_q nx - cz_q nx ny);   AA odd step: the same with slot opposite(q)
   int64_t koff[19];
 };
 
@@ -92,17 +92,27 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
   const int ip = i == a.nx - 1 ? 0 : i + 1;
 
   // The node tag (sample count, covering particle) is requested before the populations so that the
-  // dependent gather of the particle record overlaps the population loads (two dependent round trips
-  // on covered nodes instead of three: C4 7.00 -> 6.46 ms).
-  int cnt = 0, pe = 0;
-  if (IMB) {
-    const uint32_t tg = a.tag[x];
-    cnt = tag_cnt(tg);
-    pe = (int)(tg >> kTagPidShift);
-  }
+  // dependent gather of the particle record overlaps the population loads (C4 7.00 -> 6.46 ms in round 1).
+  uint32_t tg = 0;
+  if (IMB) tg = a.tag[x];
 
   // ---- gather (streaming) ----
+  // Rows whose 9 neighbouring rows all lie inside the stored lattice (block-uniform test; all but the first and
+  // last row of each axis): the source of direction q is a constant byte offset koff[q] = 8 (q N - cy nx -
+  // cz nx ny) behind one of three per-thread pointers (x-1, x, x+1 wrapped).  The general path below costs
+  // ~15 integer instructions per direction; with it the kernel executed 1.86 G warp instructions against
+  // 1.29-1.36 G of the in-place kernels for the same collision.
   double f[Q];
+  const bool inner = j >= 1 && j <= a.ny - 2 && (D == 2 || (k >= 1 && k <= a.nz - 2));
+  if (inner) {
+    const char *const p0 = (const char *)(a.fin + x), *const pm = (const char *)(a.fin + (rowoff + im)),
+                      *const pp = (const char *)(a.fin + (rowoff + ip));
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+      const int cx = L::cx(q);
+      f[q] = *(const double *)((cx == 0 ? p0 : (cx == 1 ? pm : pp)) + a.koff[q]);
+    }
+  } else {
 #pragma unroll
   for (int q = 0; q < Q; ++q) {
     const int cx = L::cx(q), cy = L::cy(q), cz = L::cz(q);
@@ -121,6 +131,7 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
     const int xs = (bounce || cx == 0) ? i : (cx == 1 ? im : ip);
     f[q] = base[xs];
   }
+  }
   if (a.bcx && (i == 0 || i == a.nx - 1)) {
     // x walls: the end nodes of a row bounce their own opposite population back (R15)
 #pragma unroll
@@ -130,6 +141,15 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_kernel(cons
     }
   }
 
+  // The tag is looked at only now: a warp issues in order, so decoding it earlier holds back the population
+  // loads behind the tag's round trip (21 % of the stall samples with the round-1 ordering).  Here all Q loads
+  // are in flight when the dependent gather of the particle record starts.
+  int cnt = 0, pe = 0;
+  if (IMB) {
+    asm volatile("" : "+r"(tg) : : "memory");
+    cnt = tag_cnt(tg);
+    pe = (int)(tg >> kTagPidShift);
+  }
   double beta = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, rx = 0.0, ry = 0.0, rz = 0.0;
   if (IMB && cnt > 0) {
     beta = __ldg(a.beta_tab + cnt);
@@ -184,12 +204,8 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_aa_kernel(c
   const int64_t x = rowoff + i;
   double *__restrict__ F = a.fout;   // the one array (fin == fout)
 
-  int cnt = 0, pe = 0;
-  if (IMB) {
-    const uint32_t tg = a.tag[x];
-    cnt = tag_cnt(tg);
-    pe = (int)(tg >> kTagPidShift);
-  }
+  uint32_t tg = 0;
+  if (IMB) tg = a.tag[x];
 
   const int im = i == 0 ? a.nx - 1 : i - 1;
   const int ip = i == a.nx - 1 ? 0 : i + 1;
@@ -232,6 +248,15 @@ __global__ void __launch_bounds__(kStepThreads, MINB) collide_stream_aa_kernel(c
     for (int q = 0; q < Q; ++q) f[q] = *slow_ptr(q);
   }
 
+  // The tag is looked at only now: a warp issues in order, so decoding it earlier holds back the population
+  // loads behind the tag's round trip (21 % of the stall samples with the round-1 ordering).  Here all Q loads
+  // are in flight when the dependent gather of the particle record starts.
+  int cnt = 0, pe = 0;
+  if (IMB) {
+    asm volatile("" : "+r"(tg) : : "memory");
+    cnt = tag_cnt(tg);
+    pe = (int)(tg >> kTagPidShift);
+  }
   double beta = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, rx = 0.0, ry = 0.0, rz = 0.0;
   if (IMB && cnt > 0) {
     beta = __ldg(a.beta_tab + cnt);
@@ -614,6 +639,11 @@ lbmimb_status launch_collide_stream(lbmimb_lattice *h, bool emit_last) {
     else launch_aa<3, 5>(h, a, (unsigned)blocks, imb, emit, h->aa_swapped);
     LBMIMB_LAUNCH_CHECK(h, "collide_stream_aa_kernel");
     return LBMIMB_OK;
+  }
+  for (int q = 0; q < h->Q; ++q) {
+    const int cy = h->g.dim == 2 ? Lat<2>::cy(q) : Lat<3>::cy(q);
+    const int cz = h->g.dim == 2 ? 0 : Lat<3>::cz(q);
+    a.koff[q] = 8 * ((int64_t)q * a.N - (int64_t)cy * a.nx - (int64_t)cz * a.nx * a.ny);
   }
   if (h->g.dim == 2)
     launch_cs<2>(h, a, (unsigned)blocks, imb, emit);

@@ -731,10 +731,16 @@ __device__ __forceinline__ void wall_force(const DemArgs &a, const int *n, const
   }
 }
 
-// contact force on particle i: the particles of the 3^D cells around it (ascending index inside a cell), then the walls
+// Contact force on particle i by ONE WARP: lane t takes the t-th of the 3^D cells around the particle (lanes
+// beyond 3^D idle), sums the pair forces of that cell's particles in ascending index, and the lanes' partial
+// sums are added in a fixed butterfly, so the result is reproducible.  A thread per particle walks the 27
+// cells one after the other and pays two dependent memory latencies per neighbour candidate, ~70 times in a
+// row (C5: 55 us per contact evaluation for 4,096 spheres); a warp per particle pays them two or three times.
+// Every lane returns the total (walls included).
 template <int D>
 __device__ __forceinline__ void dem_contact_sum(const DemArgs &a, int64_t i, double *F) {
   const int n[3] = {a.g.nx, a.g.ny, a.g.nz};
+  const int t = threadIdx.x & 31;
   double xi[3], vi[3];
   F[0] = F[1] = F[2] = 0.0;
   for (int c = 0; c < D; ++c) {
@@ -745,25 +751,35 @@ __device__ __forceinline__ void dem_contact_sum(const DemArgs &a, int64_t i, dou
   int cc[3] = {0, 0, 0};
   for (int c = 0; c < D; ++c) cc[c] = cell_coord(xi[c], a.cg, c);
   const int nc0 = a.cg.nc[0], nc1 = a.cg.nc[1], nc2 = D == 3 ? a.cg.nc[2] : 1;
-  for (int oz = D == 3 ? off_lo(nc2, a.cg.periodic[2]) : 0; oz <= (D == 3 ? off_hi(nc2, a.cg.periodic[2]) : 0); ++oz)
-    for (int oy = off_lo(nc1, a.cg.periodic[1]); oy <= off_hi(nc1, a.cg.periodic[1]); ++oy)
-      for (int ox = off_lo(nc0, a.cg.periodic[0]); ox <= off_hi(nc0, a.cg.periodic[0]); ++ox) {
-        int ex = cc[0] + ox, ey = cc[1] + oy, ez = cc[2] + oz;
-        if (a.cg.periodic[0]) ex = wrap_i(ex, nc0);
-        else if (ex < 0 || ex >= nc0) continue;
-        if (a.cg.periodic[1]) ey = wrap_i(ey, nc1);
-        else if (ey < 0 || ey >= nc1) continue;
-        if (D == 3) {
-          if (a.cg.periodic[2]) ez = wrap_i(ez, nc2);
-          else if (ez < 0 || ez >= nc2) continue;
-        }
-        const int c = (ez * nc1 + ey) * nc0 + ex;
-        for (int it = a.start[c]; it < a.start[c + 1]; ++it) {
-          const int j = a.items[it];
-          if (j == (int)i) continue;
-          pair_force<D>(a, n, xi, vi, Ri, mi, j, F);
-        }
+  constexpr int NC = D == 3 ? 27 : 9;
+  if (t < NC) {
+    const int ox = t % 3 - 1, oy = (t / 3) % 3 - 1, oz = D == 3 ? t / 9 - 1 : 0;
+    int ex = cc[0] + ox, ey = cc[1] + oy, ez = cc[2] + oz;
+    bool ok = ox >= off_lo(nc0, a.cg.periodic[0]) && ox <= off_hi(nc0, a.cg.periodic[0]) &&
+              oy >= off_lo(nc1, a.cg.periodic[1]) && oy <= off_hi(nc1, a.cg.periodic[1]);
+    if (D == 3) ok = ok && oz >= off_lo(nc2, a.cg.periodic[2]) && oz <= off_hi(nc2, a.cg.periodic[2]);
+    if (a.cg.periodic[0]) ex = wrap_i(ex, nc0);
+    else ok = ok && ex >= 0 && ex < nc0;
+    if (a.cg.periodic[1]) ey = wrap_i(ey, nc1);
+    else ok = ok && ey >= 0 && ey < nc1;
+    if (D == 3) {
+      if (a.cg.periodic[2]) ez = wrap_i(ez, nc2);
+      else ok = ok && ez >= 0 && ez < nc2;
+    }
+    if (ok) {
+      const int c = (ez * nc1 + ey) * nc0 + ex;
+      const int bg = a.start[c], en = a.start[c + 1];
+      for (int it = bg; it < en; ++it) {
+        const int j = a.items[it];
+        if (j == (int)i) continue;
+        pair_force<D>(a, n, xi, vi, Ri, mi, j, F);
       }
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < D; ++q)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) F[q] += __shfl_xor_sync(0xffffffffu, F[q], o);
   wall_force<D>(a, n, xi, vi, Ri, mi, F);
 }
 
@@ -872,9 +888,12 @@ struct DemCellArgs {
 
 template <int D, bool FINISH>
 __global__ void __launch_bounds__(128) dem_first_half_kernel(const DemArgs a, const DemCellArgs b) {
-  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;   // one warp per particle
   if (p >= a.P) return;
   const int64_t P = a.P;
+  double Fc[3];
+  dem_contact_sum<D>(a, p, Fc);
+  if ((threadIdx.x & 31) != 0) return;
   double Fh[3] = {0.0, 0.0, 0.0};
   if (FINISH) {
     constexpr int NV = D == 2 ? 3 : 6;
@@ -901,8 +920,6 @@ __global__ void __launch_bounds__(128) dem_first_half_kernel(const DemArgs a, co
 #pragma unroll
     for (int c = 0; c < D; ++c) Fh[c] = a.force[(int64_t)c * P + p];
   }
-  double Fc[3];
-  dem_contact_sum<D>(a, p, Fc);
   const int n[3] = {a.g.nx, a.g.ny, a.g.nz};
   const bool per[3] = {!a.g.bcx, !a.g.bcy, !a.g.bcz};
   const double m = a.mass[p];
@@ -931,11 +948,12 @@ __global__ void __launch_bounds__(128) dem_first_half_kernel(const DemArgs a, co
 // a.pos / a.vel = the half-step state (pos2 / vel2), a.start / a.items = the cell list of pos2
 template <int D>
 __global__ void __launch_bounds__(128) dem_second_half_kernel(const DemArgs a, const DemCellArgs b) {
-  const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;   // one warp per particle
   if (p >= a.P) return;
   const int64_t P = a.P;
   double Fc[3];
   dem_contact_sum<D>(a, p, Fc);
+  if ((threadIdx.x & 31) != 0) return;
   const double m = a.mass[p], R = a.radius[p];
   double x[3] = {0.0, 0.0, 0.0}, v[3] = {0.0, 0.0, 0.0}, w[3] = {0.0, 0.0, 0.0};
 #pragma unroll
@@ -1024,6 +1042,7 @@ __global__ void __launch_bounds__(kListSmallThreads) cl_small_kernel(int64_t P, 
     items[start[c] + slot] = (int32_t)p;
   }
   __syncthreads();
+#pragma unroll 4
   for (int64_t c = tid; c < ncells; c += kListSmallThreads) {
     const int bg = start[c], en = start[c + 1];
     for (int q0 = bg + 1; q0 < en; ++q0) {
@@ -1233,8 +1252,9 @@ static lbmimb_status dem_impl(lbmimb_lattice *h, const lbmimb_dem_params *dem, b
   b.force_w = h->force;
   b.torque_w = h->torque;
   b.prec = h->prec;
-  if (finish) dem_first_half_kernel<D, true><<<nb, 128, 0, h->stream>>>(a, b);
-  else dem_first_half_kernel<D, false><<<nb, 128, 0, h->stream>>>(a, b);
+  const int nbw = blocks_for(h->P, 4);   // one warp per particle, four per block
+  if (finish) dem_first_half_kernel<D, true><<<nbw, 128, 0, h->stream>>>(a, b);
+  else dem_first_half_kernel<D, false><<<nbw, 128, 0, h->stream>>>(a, b);
   LBMIMB_LAUNCH_CHECK(h, "dem_first_half_kernel");
   if (h->P <= kListSmallP && cl.ncells + 1 <= kListSmallCells) {
     cl_small_kernel<<<1, kListSmallThreads, 0, h->stream>>>(h->P, cl.ncells, cl.count, cl.start, cl.fill, cl.items,
@@ -1247,7 +1267,7 @@ static lbmimb_status dem_impl(lbmimb_lattice *h, const lbmimb_dem_params *dem, b
   h->cl_valid = true;
   a.pos = h->pos2;
   a.vel = h->vel2;
-  dem_second_half_kernel<D><<<nb, 128, 0, h->stream>>>(a, b);
+  dem_second_half_kernel<D><<<nbw, 128, 0, h->stream>>>(a, b);
   LBMIMB_LAUNCH_CHECK(h, "dem_second_half_kernel");
   return LBMIMB_OK;   // cell list of the new positions and packed records are in place
 }

@@ -56,7 +56,7 @@ def _gpu_drag(lb, dim, d, tau=1.0, g=1e-7):
     K = g * dg["mass"] / (nu * u_inf)
     F, _ = lat.reduce_particle_forces()
     lat.close()
-    assert U[0] < U[1] < U[2] < u_inf and u_inf * 2 * a / nu < 0.05              # still accelerating; Stokes regime
+    assert U[0] < U[1] < U[2] < u_inf and u_inf * 2 * a / nu < 0.2               # still accelerating; Re_p <= 0.2 as in Table 1
     return K / _k_ref(dim, a, L) - 1.0, U, float(F[1, 0]), g * dg["mass"]
 
 
