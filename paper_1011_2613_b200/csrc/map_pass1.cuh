@@ -1,9 +1,9 @@
 // a1, pass 1 of the particle -> lattice mapping (included by particles.cu).
 //
 // One group of G threads per particle walks the particle's bounding box.
-//   phase A: the nodes of the row intervals that can hold a covered node (dense walk, below) are classified
-//            by the distance of their centre to the particle centre: surely full (count = S^D), surely
-//            empty, or a boundary cell that must be sampled;
+//   phase A: every row of the box gets the interval of columns that can hold a covered node and, inside it,
+//            the interval of columns that are surely full (count = S^D) -- two square roots per row, no
+//            per-node classification (dense walk, below);
 //   phase B: one THREAD per boundary cell counts the inside samples.  The squared distance is
 //            separable, d2 = (dx^2 + dy^2) + dz^2 with dx depending on (i, ax) only, so the S
 //            values per axis are formed once (S*D subtract/multiply) and the S^D samples cost one
@@ -16,8 +16,6 @@
 //  shell -- no per-node classification, but serial commits per thread: C3 0.325 -> 0.369 ms, C4 1.50 -> 1.73 ms.)
 #pragma once
 // (included inside namespace lbmimb, after MapArgs / bbox_axis / min_image_d / wrap_i / sub_offset)
-
-constexpr int kMapChunk = 1024;
 
 // exact b / d and b % d for 0 <= b < 2^24, d >= 1, without the integer-division sequence
 __device__ __forceinline__ void fast_divmod(int b, int d, float inv_d, int &q, int &r) {
@@ -180,23 +178,27 @@ __device__ __forceinline__ void clip_interval(double c, double half, int lo, int
   len = ih >= il ? ih - il + 1 : 0;
 }
 
-// Dense walk of the bounding box.  A sphere fills a third of its box, so classifying every box node
-// (phase A of map_particles_kernel) spends most of its time on nodes that are plainly empty.  Here every
-// row (j,k) of the box first gets the interval of columns that can pass the "not surely empty" test,
-//   max(|dx| - hs, 0)^2 <= r2_none - ny_^2 - nz_^2   <=>   |dx| <= hs + sqrt(...)   (+ margin: a superset),
-// the interval lengths of a chunk of G rows are scanned, and phase A walks the concatenated intervals with the
-// SAME per-node classification as before; phase B is unchanged.  Rows of a particle whose box crosses the
-// periodic seam in x keep their full length (no unwrapped coordinate to take the interval in).
+// Dense walk of the bounding box.  A sphere fills a third of its box, so classifying every box node spends
+// most of its time on nodes that are plainly empty; and classifying every candidate node one by one (round 1)
+// still costs ~130 instructions per node.  Here every row (j,k) of the box gets TWO column intervals from
+// two square roots:
+//   candidates: nodes that can hold an inside sample,  |dx| <= hs + sqrt(r2_none - ny_^2 - nz_^2)  (+ margin),
+//               ny_ = max(|dy| - hs, 0): the nearest point of the node's sample cloud is not outside;
+//   full      : nodes whose whole sample cloud is inside,  |dx| <= sqrt(r2_full - fy^2 - fz^2) - hs  (- margin),
+//               fy = |dy| + hs: the farthest corner of the cloud is inside.
+// (hs = 1/2 - 1/(2S) is the half edge of the cloud; the margins, relative 1e-9, dwarf the rounding of either
+// side, and erring towards "candidate but not full" only means a node is sampled that needed not be.)
+// The full intervals of a chunk of G rows are concatenated (exclusive scan of their lengths) and committed with
+// count S^D, one node per thread, coalesced along x; the boundary pieces (candidates left and right of the full
+// interval) are concatenated the same way and sampled, one THREAD per boundary cell.  A particle whose box
+// covers a whole periodic x axis has no unwrapped coordinate to take intervals in: all its columns are sampled.
 template <int D, int G, int SFIX>
 __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
   constexpr int groups = 128 / G;
-  constexpr int CH = G >= 64 ? kMapChunk : 8 * G;   // candidate nodes per pass of a group
   constexpr int NW = G >= 32 ? G / 32 : 1;
   __shared__ double sub[256];
-  __shared__ int list[groups][CH];
-  __shared__ int nlist[groups];
-  __shared__ int pre[groups][G + 1];   // exclusive prefix of the interval lengths of this chunk of rows
-  __shared__ int beg[groups][G];       // first box column of each row's interval
+  __shared__ int pre_b[groups][G + 1], pre_f[groups][G + 1];   // exclusive prefixes of the boundary / full lengths
+  __shared__ int cbeg[groups][G], fbeg[groups][G], flen[groups][G], clen[groups][G];
   __shared__ int wtot[groups][NW];
   for (int t = threadIdx.x; t < a.S; t += blockDim.x) sub[t] = sub_offset(t, a.S);
   const int grp = threadIdx.x / G, gl = threadIdx.x % G;
@@ -217,6 +219,7 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
     wy = crosses_seam(cy, R, a.g.ny, a.g.bcy);
     wz = D == 3 && crosses_seam(cz, R, a.g.nz, a.g.bcz);
   }
+  const bool whole_x = wx && ext[0] >= a.g.nx;   // box covers the periodic x axis: no interval arithmetic
   int nrows = 0;
   if (active && ext[0] > 0) {
     const int64_t r64 = (int64_t)ext[1] * ext[2];
@@ -226,9 +229,6 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
   const int nrows_u = group_uniform_max<G>(nrows);
   const float inv1 = 1.0f / (float)(ext[1] > 0 ? ext[1] : 1);
   const double R2 = __dmul_rn(R, R);
-  // Classification of a node by the box [|d| - hs, |d| + hs] per axis that holds its sample cloud
-  // (hs = 1/2 - 1/(2S)): its farthest corner inside the particle => every sample is inside, its nearest
-  // point outside => none is.  The margin (relative 1e-9) dwarfs the rounding of either test.
   const double hs = a.hs;
   const double r2_full = R2 - 1e-9 * (R2 + 1.0), r2_none = R2 + 1e-9 * (R2 + 1.0);
   __syncthreads();
@@ -263,68 +263,62 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
   };
 
   for (int row0 = 0; row0 < nrows_u; row0 += G) {
-    // ---- candidate interval of each row of this chunk
-    int b0 = 0, len = 0;
+    // ---- the two intervals of each row of this chunk
+    int cb = 0, cl = 0, fb = 0, fl = 0;
     if (row0 + gl < nrows) {
       int j, k;
       row_of(row0 + gl, j, k);
       double dy = (double)j - cy, dz = D == 3 ? (double)k - cz : 0.0;
       if (wy) dy = min_image_d(dy, a.g.ny);
       if (D == 3 && wz) dz = min_image_d(dz, a.g.nz);
-      const double ny_ = fmax(fabs(dy) - hs, 0.0), nz_ = D == 3 ? fmax(fabs(dz) - hs, 0.0) : 0.0;
+      const double ay = fabs(dy), az = fabs(dz);
+      const double ny_ = fmax(ay - hs, 0.0), nz_ = D == 3 ? fmax(az - hs, 0.0) : 0.0;
       const double rad = r2_none - ny_ * ny_ - nz_ * nz_;
       if (rad > -1e-9 && slab_stored_row(a.sl, j) >= 0) {
-        if (wx) {
-          len = ext[0];
+        if (whole_x) {
+          cl = ext[0];
         } else {
-          clip_interval(cx, hs + sqrt(fmax(rad, 0.0) + 1e-9) + 1e-9, lo[0], ext[0], b0, len);
+          clip_interval(cx, hs + sqrt(fmax(rad, 0.0) + 1e-9) + 1e-9, lo[0], ext[0], cb, cl);
+          const double fy = ay + hs, fz = D == 3 ? az + hs : 0.0;
+          const double radf = r2_full - fy * fy - fz * fz;
+          if (radf > 0.0 && cl > 0) {
+            const double wf = sqrt(radf) - hs - 1e-9;
+            if (wf >= 0.0) {
+              clip_interval(cx, wf, lo[0] + cb, cl, fb, fl);   // inside the candidate interval
+              fb += cb;
+            }
+          }
         }
       }
     }
-    const int total = scan_row_intervals<G>(len, b0, gl, pre[grp], beg[grp], wtot[grp]);
-    const int total_u = group_uniform_max<G>(total);
+    clen[grp][gl] = cl;
+    flen[grp][gl] = fl;
+    const int totalF = scan_row_intervals<G>(fl, fb, gl, pre_f[grp], fbeg[grp], wtot[grp]);
+    const int totalB = scan_row_intervals<G>(cl - fl, cb, gl, pre_b[grp], cbeg[grp], wtot[grp]);
 
-    for (int tb = 0; tb < total_u; tb += CH) {
-      if (gl == 0) nlist[grp] = 0;
-      group_sync<G>();
-      // ---- phase A: classify the candidate nodes
-      for (int t = tb + gl; t < total && t < tb + CH; t += G) {
-        const int r = interval_row<G>(pre[grp], t);
-        const int bi = beg[grp][r] + (t - pre[grp][r]);
-        int i = lo[0] + bi, j, k;
-        row_of(row0 + r, j, k);
-        if (wx) i = wrap_i(i, a.g.nx);
-        double dx = (double)i - cx, dy = (double)j - cy, dz = D == 3 ? (double)k - cz : 0.0;
-        if (wx) dx = min_image_d(dx, a.g.nx);
-        if (wy) dy = min_image_d(dy, a.g.ny);
-        if (D == 3 && wz) dz = min_image_d(dz, a.g.nz);
-        dx = fabs(dx);
-        dy = fabs(dy);
-        dz = fabs(dz);
-        const double fx = dx + hs, fy = dy + hs, fz = D == 3 ? dz + hs : 0.0;
-        const double nx_ = fmax(dx - hs, 0.0), ny_ = fmax(dy - hs, 0.0), nz_ = D == 3 ? fmax(dz - hs, 0.0) : 0.0;
-        if (fx * fx + fy * fy + fz * fz <= r2_full) {
-          commit(i, j, k, a.SD);
-        } else if (nx_ * nx_ + ny_ * ny_ + nz_ * nz_ <= r2_none) {
-          const int slot = atomicAdd(&nlist[grp], 1);
-          list[grp][slot] = (r << 16) | bi;   // boundary cell: sample it (r < G <= 128, bi < 2^16)
-        }
-      }
-      group_sync<G>();
-      // ---- phase B: one thread per boundary cell
-      const int nl = nlist[grp];
-      for (int e = gl; e < nl; e += G) {
-        const int code = list[grp][e];
-        int i = lo[0] + (code & 0xffff), j, k;
-        row_of(row0 + (code >> 16), j, k);
-        if (wx) i = wrap_i(i, a.g.nx);
-        int cnt;
-        if (SFIX > 0) cnt = thread_count_fixed<D, (SFIX > 0 ? SFIX : 1)>(a.g, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
-        else cnt = thread_count_generic<D>(a.g, a.S, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
-        if (cnt > 0) commit(i, j, k, cnt);
-      }
-      group_sync<G>();
+    // ---- full nodes: commit S^D, consecutive columns of a row on consecutive threads
+    for (int t = gl; t < totalF; t += G) {
+      const int r = interval_row<G>(pre_f[grp], t);
+      int i = lo[0] + fbeg[grp][r] + (t - pre_f[grp][r]), j, k;
+      row_of(row0 + r, j, k);
+      if (wx) i = wrap_i(i, a.g.nx);
+      commit(i, j, k, a.SD);
     }
+    // ---- boundary cells (left and right of the full interval): one thread samples one cell
+    for (int t = gl; t < totalB; t += G) {
+      const int r = interval_row<G>(pre_b[grp], t);
+      const int o = t - pre_b[grp][r];
+      const int cbr = cbeg[grp][r], fbr = fbeg[grp][r], flr = flen[grp][r];
+      const int left = flr > 0 ? fbr - cbr : clen[grp][r];
+      int i = lo[0] + (o < left ? cbr + o : fbr + flr + (o - left)), j, k;
+      row_of(row0 + r, j, k);
+      if (wx) i = wrap_i(i, a.g.nx);
+      int cnt;
+      if (SFIX > 0) cnt = thread_count_fixed<D, (SFIX > 0 ? SFIX : 1)>(a.g, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
+      else cnt = thread_count_generic<D>(a.g, a.S, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
+      if (cnt > 0) commit(i, j, k, cnt);
+    }
+    group_sync<G>();
   }
   settle();
 }
