@@ -189,6 +189,9 @@ def test_c5_coupled_in_full(orc, lb):
             f, pos, vel, om, _ = orc.coupled_step(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, f, pos, vel, om,
                                                   w.radius, w.mass, *dargs)
         record(config="C5", window=k, oracle_only_replay=True, seconds=round(time.time() - t0, 1))
+        np.savez(_ckpt_path(k + 1), f=f, pos=pos, vel=vel, omega=om)             # so that a later call need not replay
+        if os.path.exists(_ckpt_path(k)):
+            os.remove(_ckpt_path(k))
     lat = lb.Lattice(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, max_particles=w.P)
     for k in range(first, last):
         t0 = time.time()
