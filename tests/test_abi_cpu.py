@@ -47,11 +47,13 @@ def test_library_is_built_for_sm_100a(lb):
 def test_struct_layout_matches_the_header(lb, tmp_path):
     prog = tmp_path / "layout.c"
     prog.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "lbmimb.h"\nint main(void){\n'
-                    'printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\\n", sizeof(lbmimb_params),'
+                    'printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\\n", sizeof(lbmimb_params),'
                     'offsetof(lbmimb_params,dim),offsetof(lbmimb_params,subsamples),offsetof(lbmimb_params,n),'
                     'offsetof(lbmimb_params,bc),offsetof(lbmimb_params,device),offsetof(lbmimb_params,tau),'
                     'offsetof(lbmimb_params,g_fluid),offsetof(lbmimb_params,stream),'
-                    'offsetof(lbmimb_params,workspace_dev),offsetof(lbmimb_params,workspace_bytes));\n'
+                    'offsetof(lbmimb_params,workspace_dev),offsetof(lbmimb_params,workspace_bytes),'
+                    'offsetof(lbmimb_params,streaming),offsetof(lbmimb_params,flags),'
+                    'offsetof(lbmimb_params,slab_y0),offsetof(lbmimb_params,slab_ny));\n'
                     'printf("%zu %zu %zu %zu %zu\\n", sizeof(lbmimb_dem_params),offsetof(lbmimb_dem_params,kn),'
                     'offsetof(lbmimb_dem_params,restitution),offsetof(lbmimb_dem_params,g_particle),'
                     'offsetof(lbmimb_dem_params,dt));\nreturn 0;}\n')
@@ -61,7 +63,8 @@ def test_struct_layout_matches_the_header(lb, tmp_path):
     got = [int(v) for v in lines[0].split()]
     P = lb.Params
     want = [C.sizeof(P)] + [getattr(P, k).offset for k in ("dim", "subsamples", "n", "bc", "device", "tau", "g_fluid",
-                                                            "stream", "workspace_dev", "workspace_bytes")]
+                                                            "stream", "workspace_dev", "workspace_bytes", "streaming", "flags",
+                                                            "slab_y0", "slab_ny")]
     assert got == want
     got = [int(v) for v in lines[1].split()]
     D = lb.DemParams
