@@ -163,22 +163,6 @@ __device__ __forceinline__ int interval_row(const int *pre, int t) {
   return r;
 }
 
-// does any thread of the group hold `v`?  (all threads of the block must call when G > 32)
-template <int G>
-__device__ __forceinline__ bool group_any(bool v) {
-  if constexpr (G > 32) {
-    return __syncthreads_or(v ? 1 : 0) != 0;   // G == 128: one group per block
-  } else {
-    const unsigned b = __ballot_sync(0xffffffffu, v);
-    if constexpr (G == 32) {
-      return b != 0u;
-    } else {
-      const unsigned lane = threadIdx.x & 31u;
-      return ((b >> (lane & ~(unsigned)(G - 1))) & ((1u << G) - 1u)) != 0u;
-    }
-  }
-}
-
 // loop bounds of groups that share a warp (G < 32) must agree: they synchronise with __syncwarp
 template <int G>
 __device__ __forceinline__ int group_uniform_max(int v) {
@@ -192,50 +176,6 @@ __device__ __forceinline__ void clip_interval(double c, double half, int lo, int
   if (ih > lo + ext - 1) ih = lo + ext - 1;
   b0 = il - lo;
   len = ih >= il ? ih - il + 1 : 0;
-}
-
-// Can another particle reach a node of particle p?  Only if its centre is closer than R_p + R_q + 2 h_cloud.  The
-// lanes of the group look through the 3^D cells of the particle cell list around the particle.  If nobody is
-// that close (the rule in a suspension: C4 has no such pair at all) the tags are written with plain stores;
-// otherwise with the exchange that detects shared nodes (82 M atomics per map on C4 otherwise).
-// Whole group (G > 32: whole block) must call.
-template <int D, int G>
-__device__ __forceinline__ bool has_close_neighbour(const MapArgs &a, int64_t p, bool active, double cx, double cy,
-                                                    double cz, double R, int gl) {
-  bool close = false;
-  if (active) {
-    constexpr int NC = D == 3 ? 27 : 9;
-    int cc[3] = {cell_coord(cx, a.cg, 0), cell_coord(cy, a.cg, 1), D == 3 ? cell_coord(cz, a.cg, 2) : 0};
-    const int nc0 = a.cg.nc[0], nc1 = a.cg.nc[1], nc2 = D == 3 ? a.cg.nc[2] : 1;
-    for (int t = gl; t < NC; t += G) {
-      const int ox = t % 3 - 1, oy = (t / 3) % 3 - 1, oz = D == 3 ? t / 9 - 1 : 0;
-      int ex = cc[0] + ox, ey = cc[1] + oy, ez = cc[2] + oz;
-      bool ok = ox >= off_lo(nc0, a.cg.periodic[0]) && ox <= off_hi(nc0, a.cg.periodic[0]) &&
-                oy >= off_lo(nc1, a.cg.periodic[1]) && oy <= off_hi(nc1, a.cg.periodic[1]);
-      if (D == 3) ok = ok && oz >= off_lo(nc2, a.cg.periodic[2]) && oz <= off_hi(nc2, a.cg.periodic[2]);
-      if (a.cg.periodic[0]) ex = wrap_i(ex, nc0);
-      else ok = ok && ex >= 0 && ex < nc0;
-      if (a.cg.periodic[1]) ey = wrap_i(ey, nc1);
-      else ok = ok && ey >= 0 && ey < nc1;
-      if (D == 3) {
-        if (a.cg.periodic[2]) ez = wrap_i(ez, nc2);
-        else ok = ok && ez >= 0 && ez < nc2;
-      }
-      if (!ok) continue;
-      const int c = (ez * nc1 + ey) * nc0 + ex;
-      for (int it = a.cl_start[c]; it < a.cl_start[c + 1]; ++it) {
-        const int q = a.cl_items[it];
-        if (q == (int)p) continue;
-        double ex_ = cx - a.pos[q], ey_ = cy - a.pos[a.P + q], ez_ = D == 3 ? cz - a.pos[2 * a.P + q] : 0.0;
-        if (!a.g.bcx) ex_ = min_image_d(ex_, a.g.nx);
-        if (!a.g.bcy) ey_ = min_image_d(ey_, a.g.ny);
-        if (D == 3 && !a.g.bcz) ez_ = min_image_d(ez_, a.g.nz);
-        const double lim = R + a.radius[q] + a.share_margin;
-        if (ex_ * ex_ + ey_ * ey_ + ez_ * ez_ < lim * lim) close = true;
-      }
-    }
-  }
-  return group_any<G>(close);
 }
 
 // Dense walk of the bounding box.  A sphere fills a third of its box, so classifying every box node spends
@@ -280,7 +220,6 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
     wz = D == 3 && crosses_seam(cz, R, a.g.nz, a.g.bcz);
   }
   const bool whole_x = wx && ext[0] >= a.g.nx;   // box covers the periodic x axis: no interval arithmetic
-  const bool shared = has_close_neighbour<D, G>(a, p, active, cx, cy, cz, R, gl);
   int nrows = 0;
   if (active && ext[0] > 0) {
     const int64_t r64 = (int64_t)ext[1] * ext[2];
@@ -318,10 +257,6 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
     const int jl = slab_stored_row(a.sl, j);   // (a slab stores only some rows of the global lattice)
     if (jl < 0) return;
     const int64_t x = ((int64_t)k * a.sl.ny_stored + jl) * a.g.nx + i;
-    if (!shared) {   // nobody else can write this node
-      a.tag[x] = make_tag((int32_t)p, cnt);
-      return;
-    }
     settle();
     pend_old = atomicExch(a.tag + x, make_tag((int32_t)p, cnt));
     pend_x = x;

@@ -133,7 +133,6 @@ __global__ void __launch_bounds__(128) map_table_kernel(const MapArgs a, const T
     wy = crosses_seam(cy, R, a.g.ny, a.g.bcy);
     wz = D == 3 && crosses_seam(cz, R, a.g.nz, a.g.bcz);
   }
-  const bool shared = has_close_neighbour<D, G>(a, p, active, cx, cy, cz, R, gl);   // else: plain stores (map_pass1.cuh)
   int nrows = 0;
   if (active && ext[0] > 0) {
     const int64_t r64 = (int64_t)ext[1] * ext[2];
@@ -186,13 +185,9 @@ __global__ void __launch_bounds__(128) map_table_kernel(const MapArgs a, const T
       const int code = table_code<D>(t, dx, dy, dz);
       if (code > 0) {
         const int64_t x = ((int64_t)k * a.sl.ny_stored + slab_stored_row(a.sl, j)) * a.g.nx + i;
-        if (!shared) {
-          a.tag[x] = make_tag((int32_t)p, code);
-        } else {
-          settle();
-          pend_old = atomicExch(a.tag + x, make_tag((int32_t)p, code));
-          pend_x = x;
-        }
+        settle();
+        pend_old = atomicExch(a.tag + x, make_tag((int32_t)p, code));
+        pend_x = x;
       }
     }
     group_sync<G>();

@@ -119,7 +119,7 @@ lbmimb_status launch_pack_records(lbmimb_lattice *h) {
 }
 
 // ---------------------------------------------------------------------------
-// cell list: counting sort of the particles into cells of edge >= 2 R_max + 2
+// cell list: counting sort of the particles into cells of edge >= max(2 R_max, R_max + 1, 2)
 // ---------------------------------------------------------------------------
 struct CellGeom {
   int dim;
@@ -268,12 +268,10 @@ static CellGeom cell_geom(const lbmimb_lattice *h) {
 
 lbmimb_status finish_cell_list(lbmimb_lattice *h);
 
-// Cell edge: >= 2 R_max (contacts) and >= 2 R_max + 2 h_cloud (two particles that share a lattice node: the map
-// asks the 3^D cells around a particle for such neighbours; h_cloud <= sqrt(3)/2), so 2 R_max + 2.
-static double cell_edge(const lbmimb_lattice *h) { return 2.0 * h->rmax + 2.0; }
-
 lbmimb_status build_cell_list(lbmimb_lattice *h) {
-  const double edge = cell_edge(h);
+  double edge = 2.0 * h->rmax;
+  if (edge < h->rmax + 1.0) edge = h->rmax + 1.0;
+  if (edge < 2.0) edge = 2.0;
   int n[3] = {h->gp.nx, h->gp.ny, h->gp.nz};
   int nc[3] = {1, 1, 1};
   double inv_e[3] = {1.0, 1.0, 1.0};
@@ -337,10 +335,6 @@ struct MapArgs {
   int32_t *counters;
   double h_in, h_out;  // radius of a node's sample cloud + safety margin
   double hs;           // half edge of the sample cloud, 1/2 - 1/(2S)
-  // cell list over the particles (pass 1 asks it whether a particle has a neighbour close enough to share a node)
-  CellGeom cg;
-  const int32_t *cl_start, *cl_items;
-  double share_margin; // two particles can share a node only if |c_p - c_q| < R_p + R_q + share_margin
 };
 
 __device__ __forceinline__ double sub_offset(int a, int S) {
@@ -609,14 +603,7 @@ lbmimb_status launch_map(lbmimb_lattice *h) {
   a.h_in = hs + 1e-6;
   a.h_out = hs + 1e-6;
   a.hs = 0.5 - 0.5 / (double)a.S;
-  a.cg = cell_geom(h);
-  a.cl_start = h->cl.start;
-  a.cl_items = h->cl.items;
-  a.share_margin = 2.0 * a.h_out + 1e-6;
-  if (h->map_mode == LBMIMB_MAP_TABLE) {
-    a.share_margin = sqrt((double)h->g.dim) + 1e-5;   // a node has a non-zero code up to R + sqrt(D)/2 from the centre (R17)
-    return launch_map_table(h, a);
-  }
+  if (h->map_mode == LBMIMB_MAP_TABLE) return launch_map_table(h, a);
   // threads per particle: enough lanes for the boundary shell without leaving most of them idle
   const double edge = 2.0 * h->rmax + 3.0;
   if (h->g.dim == 2) {
@@ -631,9 +618,9 @@ lbmimb_status launch_map(lbmimb_lattice *h) {
   LBMIMB_LAUNCH_CHECK(h, "map_particles_kernel");
   CellGeom cg = cell_geom(h);
   if (h->g.dim == 2)
-    map_contested_kernel<2><<<148 * 16, 128, 0, h->stream>>>(a, cg, h->cl.start, h->cl.items);
+    map_contested_kernel<2><<<148 * 4, 128, 0, h->stream>>>(a, cg, h->cl.start, h->cl.items);
   else
-    map_contested_kernel<3><<<148 * 16, 128, 0, h->stream>>>(a, cg, h->cl.start, h->cl.items);
+    map_contested_kernel<3><<<148 * 4, 128, 0, h->stream>>>(a, cg, h->cl.start, h->cl.items);
   LBMIMB_LAUNCH_CHECK(h, "map_contested_kernel");
   return LBMIMB_OK;
 }
