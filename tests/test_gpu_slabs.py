@@ -129,3 +129,24 @@ def test_slab_diagnostics_add_up_and_errors(orc, lb):
     assert ei.value.status == lb.EINVAL
     s.close()
     one.close()
+
+
+@pytest.mark.parametrize("dim,n,bc,nslabs", [(2, (37, 8), (0, 0), 8), (2, (130, 6), (1, 1), 3), (3, (9, 5, 4), (0, 0, 0), 5),
+                                             (3, (6, 7, 3), (1, 1, 1), 2)])
+def test_degenerate_slabs_random_state_no_particles(orc, lb, dim, n, bc, nslabs):
+    """Slabs of a single owned row (every row is a first AND a last row: both ghosts feed it), walls on every axis,
+    no particles: a random non-equilibrium state stepped on the slabs equals the oracle on the undivided lattice."""
+    rng = np.random.default_rng(21)
+    _, wq, _ = orc.velocity_set(dim)
+    shape = (len(wq),) + tuple(reversed(tuple(n) + (1,) * (3 - len(n))))
+    f0 = wq.reshape((-1, 1, 1, 1)) * (1 + 0.05 * rng.standard_normal(shape))
+    g = (1e-5, -2e-5, 3e-5)[:dim]
+    s = slabs.LocalSlabs(lb, dim, n, bc, 0.63, g, 8 if dim == 2 else 4, nslabs)
+    s.set_distributions(f0)
+    assert np.array_equal(s.fetch_fields(lb.FIELD_F), f0)
+    f = f0
+    for _ in range(9):
+        f = orc.step(dim, n, bc, 0.63, g, 8, f)
+    s.step(9)
+    assert_fields_close(s.fetch_fields(lb.FIELD_F), f)
+    s.close()
