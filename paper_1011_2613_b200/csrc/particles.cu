@@ -618,9 +618,9 @@ lbmimb_status launch_map(lbmimb_lattice *h) {
   LBMIMB_LAUNCH_CHECK(h, "map_particles_kernel");
   CellGeom cg = cell_geom(h);
   if (h->g.dim == 2)
-    map_contested_kernel<2><<<148 * 4, 128, 0, h->stream>>>(a, cg, h->cl.start, h->cl.items);
+    map_contested_kernel<2><<<148 * 16, 128, 0, h->stream>>>(a, cg, h->cl.start, h->cl.items);
   else
-    map_contested_kernel<3><<<148 * 4, 128, 0, h->stream>>>(a, cg, h->cl.start, h->cl.items);
+    map_contested_kernel<3><<<148 * 16, 128, 0, h->stream>>>(a, cg, h->cl.start, h->cl.items);
   LBMIMB_LAUNCH_CHECK(h, "map_contested_kernel");
   return LBMIMB_OK;
 }
