@@ -229,7 +229,8 @@ lbmimb_status lbmimb_step(lbmimb_lattice *h, int32_t nsteps);
  * eq. (3) with the sign of R6 (force ON the particle):
  *   F_p = - sum_{n: pid=p} s_n,   T_p = - sum_n (x_n - x_p) x s_n   (minimum image), h^D/dt = 1.
  * The sums were formed by the last step (runs of a particle's nodes are pre-summed per warp in a fixed tree
- * and added as 64-bit fixed-point integers, resolution 2^-91, so the result does not depend on the order
+ * and added as 64-bit fixed-point integers (resolution 2^-91; a run's partial sum must stay below 2^11 in
+ * lattice units, which any stable simulation does by many orders of magnitude), so the result does not depend on the order
  * in which thread blocks ran: bitwise reproducible); this call converts them.  force / torque may be NULL:
  * results stay on the device for dem_step; otherwise they are copied to the host and the call is synchronous.
  * ESTATE if no step has run since the last map_particles.
