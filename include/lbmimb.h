@@ -317,6 +317,26 @@ lbmimb_status lbmimb_fetch_fields(lbmimb_lattice *h, int32_t what, const int64_t
 #define LBMIMB_DIAG_LEN 20
 lbmimb_status lbmimb_diagnostics(lbmimb_lattice *h, double *out);
 
+/*
+ * lbmimb_diagnostics for callers that cannot call cudaMalloc and must not synchronise (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid allocation): the same 20 quantities, written to out_dev
+ * (DEVICE pointer, LBMIMB_DIAG_LEN doubles), asynchronous on the handle's stream.  It allocates nothing, frees
+ * nothing and calls no allocating routine: its scratch (the per-block partial sums of the two reduction stages) is
+ * a static device array inside the library of lbmimb_diagnostics_static_scratch_bytes() = 403,456 bytes, which
+ * every GPU that loads the library holds until the process exits.  The particle sums are formed by one block per
+ * 256 particles, so the array bounds the particle count: more than
+ * lbmimb_diagnostics_static_max_particles() = 1,048,576 particles -> EINVAL (use lbmimb_diagnostics).
+ * Node sums are bit for bit those of lbmimb_diagnostics; particle sums (V_s, F_d, solid momentum) are added in
+ * a different order and agree to rounding.  All calls on a device share the array, which keeps the last call's
+ * contents; every call overwrites exactly the rows it reads back, so nothing has to be cleared.  Calls that overlap
+ * on the GPU (two handles on two streams) race on it: serialise them.  The device-side error flags (see "Errors")
+ * are not looked at, since that needs a synchronisation.
+ * EINVAL: NULL argument, too many particles; ESTATE if particles are set but not mapped.
+ */
+int64_t lbmimb_diagnostics_static_max_particles(void);
+int64_t lbmimb_diagnostics_static_scratch_bytes(void);
+lbmimb_status lbmimb_diagnostics_static_dev(lbmimb_lattice *h, double *out_dev);
+
 /* Replaces all distributions: f[Q][nz][ny][nx] = f_i(x, t) as LBMIMB_FIELD_F returns them. */
 lbmimb_status lbmimb_set_distributions(lbmimb_lattice *h, const double *f);
 

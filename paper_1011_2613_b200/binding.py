@@ -33,6 +33,8 @@ EXPORTS = [
     "lbmimb_set_neighbor_mode", "lbmimb_fetch_neighbor_list", "lbmimb_run_coupled",
     "lbmimb_halo_count", "lbmimb_slab_ghost_rows", "lbmimb_pack_halo", "lbmimb_unpack_halo",
     "lbmimb_force_sums_count", "lbmimb_export_force_sums_dev", "lbmimb_import_force_sums_dev",
+    "lbmimb_diagnostics_static_dev", "lbmimb_diagnostics_static_max_particles",
+    "lbmimb_diagnostics_static_scratch_bytes",
 ]
 DIAG_LEN = 20
 
@@ -91,6 +93,11 @@ def load():
     lib.lbmimb_fetch_fields.argtypes = [vp, i32, C.POINTER(i64), C.POINTER(i64), vp]
     lib.lbmimb_set_distributions.argtypes = [vp, vp]
     lib.lbmimb_diagnostics.argtypes = [vp, vp]
+    lib.lbmimb_diagnostics_static_dev.argtypes = [vp, vp]
+    lib.lbmimb_diagnostics_static_max_particles.restype = i64
+    lib.lbmimb_diagnostics_static_max_particles.argtypes = []
+    lib.lbmimb_diagnostics_static_scratch_bytes.restype = i64
+    lib.lbmimb_diagnostics_static_scratch_bytes.argtypes = []
     lib.lbmimb_halo_count.restype = i64
     lib.lbmimb_halo_count.argtypes = [vp]
     lib.lbmimb_slab_ghost_rows.restype = i32
@@ -131,6 +138,14 @@ def _f64(a):
 
 def version():
     return load().lbmimb_version().decode()
+
+
+def diagnostics_static_max_particles():
+    return int(load().lbmimb_diagnostics_static_max_particles())
+
+
+def diagnostics_static_scratch_bytes():
+    return int(load().lbmimb_diagnostics_static_scratch_bytes())
 
 
 def make_params(dim, n, bc, tau, g_fluid, subsamples, device=0, stream=0, workspace_dev=0, workspace_bytes=0,
@@ -324,6 +339,10 @@ class Lattice:
         return {"gas_area": out[0], "mass": out[1], "gas_velocity": out[2:2 + D], "solid_velocity": out[5:5 + D],
                 "slip": out[8:8 + D], "drag": out[11:11 + D], "fluid_momentum": out[14:14 + D],
                 "solid_momentum": out[17:17 + D], "vector": out}
+
+    def diagnostics_static_dev(self, out_ptr):
+        """The 20 doubles of lbmimb_diagnostics into a DEVICE buffer; no allocation, no synchronisation."""
+        _check(self.lib.lbmimb_diagnostics_static_dev(self.h, out_ptr))
 
     # -- slabs (NEXT-4): device pointers in, device pointers out ------------------------------------
     def halo_count(self):

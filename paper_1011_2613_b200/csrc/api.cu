@@ -878,6 +878,23 @@ lbmimb_status lbmimb_diagnostics(lbmimb_lattice *h, double *out) {
   return sync_and_check(h);
 }
 
+// The same diagnostics without any allocation or synchronisation: scratch in a static device array (lattice.cu).
+int64_t lbmimb_diagnostics_static_max_particles(void) { return diagnostics_static_max_particles(); }
+int64_t lbmimb_diagnostics_static_scratch_bytes(void) { return diagnostics_static_scratch_bytes(); }
+
+lbmimb_status lbmimb_diagnostics_static_dev(lbmimb_lattice *h, double *out_dev) {
+  if (!h) return fail(LBMIMB_EINVAL, "handle is NULL");
+  if (!out_dev) return fail(LBMIMB_EINVAL, "out_dev is NULL");
+  if (h->P > diagnostics_static_max_particles())
+    return fail(LBMIMB_EINVAL, "lbmimb_diagnostics_static_dev: %lld particles exceed the static scratch (at most %lld); "
+                               "use lbmimb_diagnostics", (long long)h->P, (long long)diagnostics_static_max_particles());
+  if (h->P > 0 && !h->map_valid) return fail(LBMIMB_ESTATE, "particle map is stale: call lbmimb_map_particles first");
+  lbmimb_status st = use_device(h);
+  if (st != LBMIMB_OK) return st;
+  const double den = h->map_mode == LBMIMB_MAP_TABLE ? (double)LBMIMB_TABLE_DEN : (double)h->SD;
+  return launch_diagnostics_static(h, den, out_dev);
+}
+
 // ---- slab decomposition (NEXT-4): halo pack / unpack and the per-slab force sums ----
 int64_t lbmimb_halo_count(const lbmimb_lattice *h) { return h ? halo_doubles(h) : -1; }
 

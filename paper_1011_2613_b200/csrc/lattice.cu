@@ -750,4 +750,141 @@ lbmimb_status launch_halo(lbmimb_lattice *h, int side, double *buf_dev, bool pac
   return LBMIMB_OK;
 }
 
+// ---------------------------------------------------------------------------
+// lbmimb_diagnostics_static_dev: the diagnostics of lbmimb_diagnostics for callers that must not allocate and
+// must not synchronise (code under CUDA graph capture, tight loops).  Same node stage (diag_nodes_kernel, same
+// grid => the same partial sums bit for bit); the particle sums, which lbmimb_diagnostics forms serially in
+// its one final block, are formed by ceil(P / 256) blocks, so this variant needs scratch that grows with P.  That
+// scratch is NOT in the handle's workspace but in the file-scope array below, of a fixed size:
+//   kStaticNodeRows (1184) x 8 + kStaticParticleRows (4096) x 10 doubles = 403,456 bytes,
+// which every GPU that loads the library holds until the process exits.  P beyond 4096 x 256 = 1,048,576 is
+// rejected.  In host code the array's NAME is a host-side stand-in, not a device address: the address is taken
+// once per device with cudaGetSymbolAddress, that device being current, and handed to the kernels.
+// Every call (of every handle on the device) shares the array.  Nothing in it has to start at zero: each call
+// overwrites exactly the rows it reads back (rows [0, nb) and [0, nbp)).  Calls that overlap on the GPU (two
+// streams) race on it.
+// ---------------------------------------------------------------------------
+constexpr int kStaticNodeRows = kDiagBlocksMax;
+constexpr int kStaticParticleRows = 4096;
+constexpr int kStaticParticleK = 10;
+constexpr int64_t kStaticMaxParticles = (int64_t)kStaticParticleRows * kDiagThreads;
+constexpr int kStaticDoubles = kStaticNodeRows * kDiagK + kStaticParticleRows * kStaticParticleK;
+static __device__ __align__(256) double g_diag_static_scratch[kStaticDoubles];
+
+constexpr int kStaticMaxDevices = 64;
+static double *g_diag_static_ptr[kStaticMaxDevices];   // device address of the array, per device ordinal (0 = not taken yet)
+
+// per block: [0] sum vol, [1..3] sum vol v, [4..6] sum m v, [7..9] sum F  (the sums of diag_final_kernel)
+template <int D>
+__global__ void __launch_bounds__(kDiagThreads) diag_particles_static_kernel(int64_t P, const double *__restrict__ vel,
+                                                                             const double *__restrict__ radius,
+                                                                             const double *__restrict__ mass,
+                                                                             const double *__restrict__ force,
+                                                                             double *__restrict__ ppartial) {
+  __shared__ double sh[kDiagThreads / 32];
+  double pa[kStaticParticleK];
+#pragma unroll
+  for (int c = 0; c < kStaticParticleK; ++c) pa[c] = 0.0;
+  const double kPi = 3.14159265358979323846;
+  const int64_t p = (int64_t)blockIdx.x * kDiagThreads + threadIdx.x;
+  if (p < P) {
+    const double R = radius[p];
+    const double vol = D == 2 ? kPi * (R * R) : (4.0 / 3.0 * kPi) * (R * R * R);
+    pa[0] = vol;
+#pragma unroll
+    for (int c = 0; c < D; ++c) {
+      const double v = vel[(int64_t)c * P + p];
+      pa[1 + c] = vol * v;
+      pa[4 + c] = mass[p] * v;
+      pa[7 + c] = force[(int64_t)c * P + p];
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < kStaticParticleK; ++c) {
+    const double t = diag_block_sum(pa[c], sh);
+    if (threadIdx.x == 0) ppartial[(int64_t)blockIdx.x * kStaticParticleK + c] = t;
+  }
+}
+
+// out[20] as diag_final_kernel writes it; node partials summed exactly as there, particle partials in block order
+template <int D>
+__global__ void __launch_bounds__(kDiagThreads) diag_final_static_kernel(const double *__restrict__ partial, int nblocks,
+                                                                         const double *__restrict__ ppartial, int npblocks,
+                                                                         int64_t P, double *__restrict__ out) {
+  __shared__ double sh[kDiagThreads / 32];
+  __shared__ double tot[kDiagK + kStaticParticleK];
+  for (int c = 0; c < kDiagK; ++c) {
+    double v = 0.0;
+    for (int b = threadIdx.x; b < nblocks; b += kDiagThreads) v += partial[(int64_t)b * kDiagK + c];
+    const double t = diag_block_sum(v, sh);
+    if (threadIdx.x == 0) tot[c] = t;
+  }
+  for (int c = 0; c < kStaticParticleK; ++c) {
+    double v = 0.0;
+    for (int b = threadIdx.x; b < npblocks; b += kDiagThreads) v += ppartial[(int64_t)b * kStaticParticleK + c];
+    const double t = diag_block_sum(v, sh);
+    if (threadIdx.x == 0) tot[kDiagK + c] = t;
+  }
+  if (threadIdx.x == 0) {
+    for (int c = 0; c < 20; ++c) out[c] = 0.0;
+    out[0] = tot[0];
+    out[1] = tot[1];
+    for (int c = 0; c < D; ++c) {
+      out[2 + c] = tot[2 + c] / tot[0];
+      out[14 + c] = tot[5 + c];
+      if (P > 0) {
+        out[5 + c] = tot[9 + c] / tot[8];
+        out[11 + c] = tot[15 + c] / (double)P;
+        out[17 + c] = tot[12 + c];
+      }
+      out[8 + c] = out[2 + c] - out[5 + c];
+    }
+  }
+}
+
+int64_t diagnostics_static_max_particles() { return kStaticMaxParticles; }
+int64_t diagnostics_static_scratch_bytes() { return (int64_t)kStaticDoubles * 8; }
+
+// No cudaMalloc / cudaFree / allocating routine, no synchronisation: four launches on the handle's stream.
+// The caller (api.cu) has made the handle's device current.
+lbmimb_status launch_diagnostics_static(lbmimb_lattice *h, double eps_den, double *out_dev) {
+  if (h->P > kStaticMaxParticles)
+    return fail(LBMIMB_EINVAL, "lbmimb_diagnostics_static_dev: %lld particles exceed the static scratch (at most %lld); "
+                               "use lbmimb_diagnostics", (long long)h->P, (long long)kStaticMaxParticles);
+  const int dev = h->prm.device;
+  if (dev < 0 || dev >= kStaticMaxDevices) return fail(LBMIMB_EINVAL, "device ordinal %d beyond %d", dev, kStaticMaxDevices);
+  if (!g_diag_static_ptr[dev]) {   // set-up, once per device, that device being current
+    double *ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void **)&ptr, g_diag_static_scratch);
+    if (e != cudaSuccess || !ptr) return cuda_fail(e, "cudaGetSymbolAddress(g_diag_static_scratch)");
+    g_diag_static_ptr[dev] = ptr;
+  }
+  double *partial = g_diag_static_ptr[dev];
+  double *ppartial = partial + (size_t)kStaticNodeRows * kDiagK;
+  const int layout = h->aa ? (h->aa_swapped ? kLayoutSwapped : kLayoutNatural) : kLayoutPull;
+  const int nb = grid_for(h->g.N, kDiagThreads, kStaticNodeRows);
+  const int nbp = (int)((h->P + kDiagThreads - 1) / kDiagThreads);
+  const double *fst = h->f[h->cur];
+  const int hp = h->P > 0;
+  if (h->g.dim == 2) {
+    diag_nodes_kernel<2><<<nb, kDiagThreads, 0, h->stream>>>(fst, h->tag, h->g, h->sl, layout, hp, eps_den, partial);
+    LBMIMB_LAUNCH_CHECK(h, "diag_nodes_kernel");
+    if (nbp > 0) {
+      diag_particles_static_kernel<2><<<nbp, kDiagThreads, 0, h->stream>>>(h->P, h->vel, h->radius, h->mass, h->force, ppartial);
+      LBMIMB_LAUNCH_CHECK(h, "diag_particles_static_kernel");
+    }
+    diag_final_static_kernel<2><<<1, kDiagThreads, 0, h->stream>>>(partial, nb, ppartial, nbp, h->P, out_dev);
+  } else {
+    diag_nodes_kernel<3><<<nb, kDiagThreads, 0, h->stream>>>(fst, h->tag, h->g, h->sl, layout, hp, eps_den, partial);
+    LBMIMB_LAUNCH_CHECK(h, "diag_nodes_kernel");
+    if (nbp > 0) {
+      diag_particles_static_kernel<3><<<nbp, kDiagThreads, 0, h->stream>>>(h->P, h->vel, h->radius, h->mass, h->force, ppartial);
+      LBMIMB_LAUNCH_CHECK(h, "diag_particles_static_kernel");
+    }
+    diag_final_static_kernel<3><<<1, kDiagThreads, 0, h->stream>>>(partial, nb, ppartial, nbp, h->P, out_dev);
+  }
+  LBMIMB_LAUNCH_CHECK(h, "diag_final_static_kernel");
+  return LBMIMB_OK;
+}
+
 }  // namespace lbmimb

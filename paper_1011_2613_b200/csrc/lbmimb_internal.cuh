@@ -258,6 +258,9 @@ lbmimb_status neighbor_list_prepare(lbmimb_lattice *h);   // (re)allocates the l
 void neighbor_list_release(lbmimb_lattice *h);
 lbmimb_status neighbor_list_invalidate(lbmimb_lattice *h);  // positions were replaced
 lbmimb_status launch_diagnostics(lbmimb_lattice *h, double eps_den);
+lbmimb_status launch_diagnostics_static(lbmimb_lattice *h, double eps_den, double *out_dev);   // scratch: a static device array
+int64_t diagnostics_static_max_particles();
+int64_t diagnostics_static_scratch_bytes();
 lbmimb_status launch_halo(lbmimb_lattice *h, int side, double *buf_dev, bool pack);
 int64_t halo_doubles(const lbmimb_lattice *h);
 constexpr int kDiagBlocksMax = 148 * 8;
