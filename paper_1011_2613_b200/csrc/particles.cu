@@ -783,6 +783,46 @@ __device__ __forceinline__ void dem_contact_sum(const DemArgs &a, int64_t i, dou
   wall_force<D>(a, n, xi, vi, Ri, mi, F);
 }
 
+// The same sum by ONE THREAD: the 3^D cells one after the other (oz, oy, ox ascending).  For large sets
+// (P > kDemWarpMaxP) there are enough particles to hide the dependent latencies, and a warp per particle
+// only multiplies the threads: P2D (1,166,400 disks) 2.14 ms per step with warps against 0.44 ms with threads.
+template <int D>
+__device__ __forceinline__ void dem_contact_sum_serial(const DemArgs &a, int64_t i, double *F) {
+  const int n[3] = {a.g.nx, a.g.ny, a.g.nz};
+  double xi[3], vi[3];
+  F[0] = F[1] = F[2] = 0.0;
+  for (int c = 0; c < D; ++c) {
+    xi[c] = a.pos[(int64_t)c * a.P + i];
+    vi[c] = a.vel[(int64_t)c * a.P + i];
+  }
+  const double Ri = a.radius[i], mi = a.mass[i];
+  int cc[3] = {0, 0, 0};
+  for (int c = 0; c < D; ++c) cc[c] = cell_coord(xi[c], a.cg, c);
+  const int nc0 = a.cg.nc[0], nc1 = a.cg.nc[1], nc2 = D == 3 ? a.cg.nc[2] : 1;
+  for (int oz = D == 3 ? off_lo(nc2, a.cg.periodic[2]) : 0; oz <= (D == 3 ? off_hi(nc2, a.cg.periodic[2]) : 0); ++oz)
+    for (int oy = off_lo(nc1, a.cg.periodic[1]); oy <= off_hi(nc1, a.cg.periodic[1]); ++oy)
+      for (int ox = off_lo(nc0, a.cg.periodic[0]); ox <= off_hi(nc0, a.cg.periodic[0]); ++ox) {
+        int ex = cc[0] + ox, ey = cc[1] + oy, ez = cc[2] + oz;
+        if (a.cg.periodic[0]) ex = wrap_i(ex, nc0);
+        else if (ex < 0 || ex >= nc0) continue;
+        if (a.cg.periodic[1]) ey = wrap_i(ey, nc1);
+        else if (ey < 0 || ey >= nc1) continue;
+        if (D == 3) {
+          if (a.cg.periodic[2]) ez = wrap_i(ez, nc2);
+          else if (ez < 0 || ez >= nc2) continue;
+        }
+        const int c = (ez * nc1 + ey) * nc0 + ex;
+        for (int it = a.start[c]; it < a.start[c + 1]; ++it) {
+          const int j = a.items[it];
+          if (j == (int)i) continue;
+          pair_force<D>(a, n, xi, vi, Ri, mi, j, F);
+        }
+      }
+  wall_force<D>(a, n, xi, vi, Ri, mi, F);
+}
+
+constexpr int64_t kDemWarpMaxP = 16384;   // up to here one warp per particle, beyond one thread per particle
+
 // the same sums over the neighbour lists (ascending j).  Runs right after the three predicated
 // build kernels of this evaluation, so one thread commits their outcome to the list state.
 template <int D>
@@ -886,14 +926,19 @@ struct DemCellArgs {
   double *prec;
 };
 
-template <int D, bool FINISH>
+template <int D, bool FINISH, bool WARP>
 __global__ void __launch_bounds__(128) dem_first_half_kernel(const DemArgs a, const DemCellArgs b) {
-  const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;   // one warp per particle
+  const int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t p = WARP ? gid >> 5 : gid;   // one warp, or one thread, per particle
   if (p >= a.P) return;
   const int64_t P = a.P;
   double Fc[3];
-  dem_contact_sum<D>(a, p, Fc);
-  if ((threadIdx.x & 31) != 0) return;
+  if (WARP) {
+    dem_contact_sum<D>(a, p, Fc);
+    if ((threadIdx.x & 31) != 0) return;
+  } else {
+    dem_contact_sum_serial<D>(a, p, Fc);
+  }
   double Fh[3] = {0.0, 0.0, 0.0};
   if (FINISH) {
     constexpr int NV = D == 2 ? 3 : 6;
@@ -946,14 +991,19 @@ __global__ void __launch_bounds__(128) dem_first_half_kernel(const DemArgs a, co
 }
 
 // a.pos / a.vel = the half-step state (pos2 / vel2), a.start / a.items = the cell list of pos2
-template <int D>
+template <int D, bool WARP>
 __global__ void __launch_bounds__(128) dem_second_half_kernel(const DemArgs a, const DemCellArgs b) {
-  const int64_t p = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;   // one warp per particle
+  const int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t p = WARP ? gid >> 5 : gid;
   if (p >= a.P) return;
   const int64_t P = a.P;
   double Fc[3];
-  dem_contact_sum<D>(a, p, Fc);
-  if ((threadIdx.x & 31) != 0) return;
+  if (WARP) {
+    dem_contact_sum<D>(a, p, Fc);
+    if ((threadIdx.x & 31) != 0) return;
+  } else {
+    dem_contact_sum_serial<D>(a, p, Fc);
+  }
   const double m = a.mass[p], R = a.radius[p];
   double x[3] = {0.0, 0.0, 0.0}, v[3] = {0.0, 0.0, 0.0}, w[3] = {0.0, 0.0, 0.0};
 #pragma unroll
@@ -1252,9 +1302,15 @@ static lbmimb_status dem_impl(lbmimb_lattice *h, const lbmimb_dem_params *dem, b
   b.force_w = h->force;
   b.torque_w = h->torque;
   b.prec = h->prec;
-  const int nbw = blocks_for(h->P, 4);   // one warp per particle, four per block
-  if (finish) dem_first_half_kernel<D, true><<<nbw, 128, 0, h->stream>>>(a, b);
-  else dem_first_half_kernel<D, false><<<nbw, 128, 0, h->stream>>>(a, b);
+  const bool warp = h->P <= kDemWarpMaxP;
+  const int nbw = warp ? blocks_for(h->P, 4) : blocks_for(h->P, 128);   // a warp (four per block) or a thread per particle
+  if (warp) {
+    if (finish) dem_first_half_kernel<D, true, true><<<nbw, 128, 0, h->stream>>>(a, b);
+    else dem_first_half_kernel<D, false, true><<<nbw, 128, 0, h->stream>>>(a, b);
+  } else {
+    if (finish) dem_first_half_kernel<D, true, false><<<nbw, 128, 0, h->stream>>>(a, b);
+    else dem_first_half_kernel<D, false, false><<<nbw, 128, 0, h->stream>>>(a, b);
+  }
   LBMIMB_LAUNCH_CHECK(h, "dem_first_half_kernel");
   if (h->P <= kListSmallP && cl.ncells + 1 <= kListSmallCells) {
     cl_small_kernel<<<1, kListSmallThreads, 0, h->stream>>>(h->P, cl.ncells, cl.count, cl.start, cl.fill, cl.items,
@@ -1267,7 +1323,8 @@ static lbmimb_status dem_impl(lbmimb_lattice *h, const lbmimb_dem_params *dem, b
   h->cl_valid = true;
   a.pos = h->pos2;
   a.vel = h->vel2;
-  dem_second_half_kernel<D><<<nbw, 128, 0, h->stream>>>(a, b);
+  if (warp) dem_second_half_kernel<D, true><<<nbw, 128, 0, h->stream>>>(a, b);
+  else dem_second_half_kernel<D, false><<<nbw, 128, 0, h->stream>>>(a, b);
   LBMIMB_LAUNCH_CHECK(h, "dem_second_half_kernel");
   return LBMIMB_OK;   // cell list of the new positions and packed records are in place
 }

@@ -450,3 +450,31 @@ def test_set_particles_dev_rejects_bad_input_without_touching_the_handle(orc, lb
     eo, po = orc.map_particles(w.dim, w.n, w.bc, w.subsamples, w.pos, w.radius)
     assert np.array_equal(lat.fetch_fields(lb.FIELD_EPS_CNT), eo)
     lat.close()
+
+
+def test_dem_large_set_thread_per_particle_path_against_oracle(orc, lb):
+    """More than 16,384 particles: the DEM step takes its thread-per-particle kernels (smaller sets: a warp per
+    particle) and the multi-kernel counting sort of the cell list.  20,000 overlapping disks, walls in x and a
+    periodic seam in y, against the oracle's all-pairs step."""
+    rng = np.random.default_rng(12)
+    dim, n, bc, P = 2, (420, 380), (1, 0), 20000
+    pos = rng.random((dim, P)) * (np.array(n)[:, None] - 6.0) + 2.5
+    vel = rng.uniform(-0.02, 0.02, size=(dim, P))
+    om = rng.uniform(-1e-3, 1e-3, size=(1, P))
+    radius = 0.8 + 1.2 * rng.random(P)
+    mass = 50.0 + 100.0 * rng.random(P)
+    kn, e, gp = 3.0, 0.85, (1e-4, -2e-4)
+    lat = lb.Lattice(dim, n, bc, 0.8, (0, 0), 8, max_particles=P)
+    lat.set_particles(pos, vel, om, radius, mass)
+    z, zt = np.zeros((dim, P)), np.zeros((1, P))
+    p_o, v_o, o_o = pos, vel, om
+    for _ in range(4):
+        lat.dem_step(kn, e, gp, 1.0)
+        p_o, v_o, o_o = orc.dem_step(dim, n, bc, p_o, v_o, o_o, radius, mass, z, zt, kn, e, gp, 1.0)
+    p_g, v_g, o_g = lat.get_particles()
+    fc = orc.contact_forces(dim, n, bc, p_o, v_o, radius, mass, kn, e)
+    assert (np.abs(fc).max(axis=0) > 0).sum() > P // 4          # contacts are really exercised
+    assert np.abs(p_g - p_o).max() < 1e-11
+    assert np.abs(v_g - v_o).max() < 1e-12 * max(1.0, np.abs(v_o).max() / 1e-2)
+    assert np.array_equal(o_g, o_o)
+    lat.close()
