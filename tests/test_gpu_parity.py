@@ -452,16 +452,22 @@ def test_set_particles_dev_rejects_bad_input_without_touching_the_handle(orc, lb
     lat.close()
 
 
-def test_dem_large_set_thread_per_particle_path_against_oracle(orc, lb):
+@pytest.mark.parametrize("n,region,rlo,rhi", [((420, 380), None, 0.8, 2.0), ((1600, 1500), 300.0, 0.3, 0.5)])
+def test_dem_large_set_thread_per_particle_path_against_oracle(orc, lb, n, region, rlo, rhi):
     """More than 16,384 particles: the DEM step takes its thread-per-particle kernels (smaller sets: a warp per
-    particle) and the multi-kernel counting sort of the cell list.  20,000 overlapping disks, walls in x and a
-    periodic seam in y, against the oracle's all-pairs step."""
+    particle).  20,000 overlapping disks, walls in x and a periodic seam in y, against the oracle's all-pairs step.
+    First case: the single-block cell-list kernel (4,410 cells); second case: small disks crowded into a corner of
+    a large lattice, 284,000 cells, i.e. the multi-kernel counting sort inside the DEM step."""
     rng = np.random.default_rng(12)
-    dim, n, bc, P = 2, (420, 380), (1, 0), 20000
-    pos = rng.random((dim, P)) * (np.array(n)[:, None] - 6.0) + 2.5
+    dim, bc, P = 2, (1, 0), 20000
+    if region is None:
+        pos = rng.random((dim, P)) * (np.array(n)[:, None] - 6.0) + 2.5
+    else:
+        pos = rng.random((dim, P)) * region + np.array([[1.0], [n[1] - region / 2]])     # across the y seam
+        pos[1] = np.mod(pos[1], n[1])
     vel = rng.uniform(-0.02, 0.02, size=(dim, P))
     om = rng.uniform(-1e-3, 1e-3, size=(1, P))
-    radius = 0.8 + 1.2 * rng.random(P)
+    radius = rlo + (rhi - rlo) * rng.random(P)
     mass = 50.0 + 100.0 * rng.random(P)
     kn, e, gp = 3.0, 0.85, (1e-4, -2e-4)
     lat = lb.Lattice(dim, n, bc, 0.8, (0, 0), 8, max_particles=P)
