@@ -150,3 +150,43 @@ def test_degenerate_slabs_random_state_no_particles(orc, lb, dim, n, bc, nslabs)
     s.step(9)
     assert_fields_close(s.fetch_fields(lb.FIELD_F), f)
     s.close()
+
+
+def test_c3_full_size_two_slabs_bitwise_and_halo_cost(lb):
+    """BASELINE.json configs[2] at its full size (256 x 1008 x 256, 24,600 spheres) as two slabs of 504 rows on ONE
+    GPU against the undivided lattice: density, maps and every per-particle force / torque bit for bit after 6 steps
+    (the oracle covers the undivided lattice at this size in tests/test_gpu_fullsize.py).  Prints what a halo
+    exchange costs on the device (pack + unpack of 256 x 256 x 5 doubles per face)."""
+    import torch
+    w = inputs.c3()
+    steps = 6
+    one = lb.from_workload(w)
+    one.map_particles()
+    one.step(steps)
+    F1, T1 = one.reduce_particle_forces()
+    rho1 = one.fetch_fields(lb.FIELD_RHO)
+    eps1 = one.fetch_fields(lb.FIELD_EPS_CNT)
+    pid1 = one.fetch_fields(lb.FIELD_PID)
+    one.close()
+    del one
+    torch.cuda.empty_cache()
+    s = slabs.LocalSlabs(lb, w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, 2, max_particles=w.P)
+    s.set_particles(w.pos, w.vel, w.omega, w.radius, w.mass)
+    s.map_particles()
+    s.step(steps)
+    (F, T), _ = s.reduce_particle_forces()
+    assert np.array_equal(F, F1) and np.array_equal(T, T1)
+    assert np.array_equal(s.fetch_fields(lb.FIELD_EPS_CNT), eps1) and np.array_equal(s.fetch_fields(lb.FIELD_PID), pid1)
+    assert np.array_equal(s.fetch_fields(lb.FIELD_RHO), rho1)
+    cut = s.parts[1][0]
+    assert ((w.pos[1] - w.radius < cut) & (w.pos[1] + w.radius > cut)).sum() > 50      # spheres cut by the face
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record()
+    for _ in range(20):
+        s.exchange_halos()
+    b.record()
+    torch.cuda.synchronize()
+    print("halo exchange of a C3 face pair (2 packs + 2 unpacks of %d doubles, device-to-device): %.3f ms"
+          % (s.lat[0].halo_count(), a.elapsed_time(b) / 20))
+    s.close()
