@@ -30,8 +30,10 @@ __device__ __forceinline__ void fast_divmod(int b, int d, float inv_d, int &q, i
   }
 }
 
-// inside-sample count of one node, compile-time S (register arrays)
-template <int D, int S>
+// inside-sample count of one node, compile-time S (register arrays).  SEAM = false: the particle's box touches
+// no periodic seam (all but a few particles), so the minimum-image steps are compiled out (16 conditionals per
+// cell in 2D, 12 in 3D; the kernel is issue-bound).
+template <int D, int S, bool SEAM>
 __device__ __forceinline__ int thread_count_fixed(const Geom &g, const double *__restrict__ sub, int i, int j, int k,
                                                   double cx, double cy, double cz, double R2, bool wx, bool wy,
                                                   bool wz) {
@@ -42,13 +44,13 @@ __device__ __forceinline__ int thread_count_fixed(const Geom &g, const double *_
     const double so = sub[a];
     double dx = __dsub_rn(__dadd_rn(di, so), cx);
     double dy = __dsub_rn(__dadd_rn(dj, so), cy);
-    if (wx) dx = min_image_d(dx, g.nx);
-    if (wy) dy = min_image_d(dy, g.ny);
+    if (SEAM && wx) dx = min_image_d(dx, g.nx);
+    if (SEAM && wy) dy = min_image_d(dy, g.ny);
     dx2[a] = __dmul_rn(dx, dx);
     dy2[a] = __dmul_rn(dy, dy);
     if (D == 3) {
       double dz = __dsub_rn(__dadd_rn(dk, so), cz);
-      if (wz) dz = min_image_d(dz, g.nz);
+      if (SEAM && wz) dz = min_image_d(dz, g.nz);
       dz2[a] = __dmul_rn(dz, dz);
     } else {
       dz2[a] = 0.0;
@@ -314,8 +316,12 @@ __global__ void __launch_bounds__(128) map_particles_kernel(const MapArgs a) {
       row_of(row0 + r, j, k);
       if (wx) i = wrap_i(i, a.g.nx);
       int cnt;
-      if (SFIX > 0) cnt = thread_count_fixed<D, (SFIX > 0 ? SFIX : 1)>(a.g, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
-      else cnt = thread_count_generic<D>(a.g, a.S, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
+      if (SFIX > 0) {
+        if (wx || wy || wz) cnt = thread_count_fixed<D, (SFIX > 0 ? SFIX : 1), true>(a.g, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
+        else cnt = thread_count_fixed<D, (SFIX > 0 ? SFIX : 1), false>(a.g, sub, i, j, k, cx, cy, cz, R2, false, false, false);
+      } else {
+        cnt = thread_count_generic<D>(a.g, a.S, sub, i, j, k, cx, cy, cz, R2, wx, wy, wz);
+      }
       if (cnt > 0) commit(i, j, k, cnt);
     }
     group_sync<G>();

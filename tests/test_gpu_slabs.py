@@ -190,3 +190,40 @@ def test_c3_full_size_two_slabs_bitwise_and_halo_cost(lb):
     print("halo exchange of a C3 face pair (2 packs + 2 unpacks of %d doubles, device-to-device): %.3f ms"
           % (s.lat[0].halo_count(), a.elapsed_time(b) / 20))
     s.close()
+
+
+def test_rank_slab_with_the_real_library_one_rank(lb):
+    """slabs.RankSlab (the one-slab-per-rank plumbing, otherwise tested over gloo with a stand-in lattice) driving the
+    real library through device pointers: world_size 1, periodic in y, so the rank's single slab feeds its own ghost
+    rows and the force sums need no reduction.  Bitwise equal to the undivided lattice."""
+    import os
+    import torch
+    import torch.distributed as dist
+    w = inputs.reduced("P3D")
+    steps = 7
+    one, got1 = gpu_run(lb, w, steps, exchange_field=False)
+    created = False
+    if not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29591")
+        dist.init_process_group("gloo", rank=0, world_size=1)
+        created = True
+    try:
+        lat = lb.Lattice(w.dim, w.n, w.bc, w.tau, w.g_fluid, w.subsamples, max_particles=w.P, slab=(0, w.n[1]))
+        lat.set_particles(w.pos, w.vel, w.omega, w.radius, w.mass)
+        rs = slabs.RankSlab(lat, 0, 1, True, "cuda:0", pointers=True)
+        assert lat.slab_ghost_rows(0) == 1 and lat.slab_ghost_rows(1) == 1
+        lat.map_particles()
+        for _ in range(steps):
+            lat.step(1)
+            rs.exchange_halos()
+        rs.combine_force_sums()
+        F, T = lat.reduce_particle_forces()
+        assert np.array_equal(F, got1["force"]) and np.array_equal(T, got1["torque"])
+        assert np.array_equal(lat.fetch_fields(lb.FIELD_F), got1["f"])
+        assert np.array_equal(lat.fetch_fields(lb.FIELD_PID), got1["pid"])
+        lat.close()
+    finally:
+        if created:
+            dist.destroy_process_group()
+    one.close()
