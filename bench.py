@@ -40,14 +40,19 @@ UNIT = "MLUPS"
 
 def profiled_traffic(workload, streaming):
     """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused kernel, from the committed
-    `ncu --set full` capture of this round (profiles/r2_traffic.json names the capture, the kernel and the
-    commit it was taken at).  Not measured in this run: None where no capture exists for the combination."""
+    `ncu --set full` capture of this round (profiles/r2_traffic.csv names the capture, the kernel and the
+    commit it was taken at; commands in profiles/README.md).  Not measured in this run: None where no capture
+    exists for the combination."""
+    import csv
     try:
-        with open(os.path.join(ROOT, "profiles", "r2_traffic.json")) as fh:
-            rec = json.load(fh)["%s/%s" % (workload, streaming)]
-        return rec["dram_bytes_per_launch"], "profiles/r2_traffic.json (%s, commit %s)" % (rec["kernel"], rec["commit"])
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.csv"), newline="") as fh:
+            for rec in csv.DictReader(fh):
+                if rec["workload/streaming"] == "%s/%s" % (workload, streaming):
+                    return int(rec["dram_bytes_per_launch"]), "profiles/r2_traffic.csv (%s, commit %s)" % (
+                        rec["kernel"], rec["commit"])
     except Exception:
-        return None, None
+        pass
+    return None, None
 
 
 def measured_peak_gbs():
